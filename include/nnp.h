@@ -1,0 +1,169 @@
+/*
+ * nnp.h -- C ABI of the B200-native ANI-2x energy+force library (libnnp_b200.so).
+ *
+ * What it computes (arXiv 2201.08110 "NNP/MM"; citations are lines of /root/reference/PAPER.md):
+ *   V_NNP(Z_NNP, r_NNP): the neural-network-potential energy of the NNP region as a function of
+ *   its atomic numbers and positions (Eq. 2) and F_NNP = -grad V_NNP (Eq. 3,
+ *   PAPER.md:63-65), for the ANI family of potentials (modified Behler-Parrinello symmetry
+ *   functions, 5.1 A cutoff, H C N O F S Cl, ensemble of 8 networks: PAPER.md:36,77).
+ *   Mechanical embedding (Eq. 1 and 4): the NNP forces are simply ADDED to the MM
+ *   force buffer on the device; "neither atomic positions nor atomic forces need to be
+ *   transferred between the CPU and GPU".  The molecule is fixed across MD steps
+ *   ("the same molecule is computed repeatedly"), so species, weights, element
+ *   grouping and workspaces are set up once in nnp_create.
+ *   The paper prints no formulas; the exact definitions (cutoff function, radial/angular terms,
+ *   feature layout, CELU MLPs, ensemble mean, units) are O1-O7 / S1-S20 in DESIGN.md.
+ *
+ * Conventions
+ *   - Every function returns an int status (NNP_OK = 0, negative = error); nothing throws.
+ *   - "host" / "device" is stated for every pointer.  Device pointers must belong to the CUDA
+ *     device that was current when nnp_create ran.  No torch types, no C++ types.
+ *   - nnp_compute is asynchronous on the caller's stream and never synchronises the host.
+ *     Device-detected conditions (neighbour capacity overflow, non-finite input) set a sticky
+ *     device flag that nnp_status() reports.
+ *   - One handle may be used by one stream at a time.
+ *   - There is no CPU fallback and no other backend: on a machine without an sm_100 GPU
+ *     nnp_create fails with NNP_ERR_UNSUPPORTED_ARCH / NNP_ERR_CUDA.
+ */
+#ifndef NNP_B200_H
+#define NNP_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NNP_OK 0
+#define NNP_ERR_INVALID_ARG (-1)
+#define NNP_ERR_CUDA (-2)
+#define NNP_ERR_UNSUPPORTED_ARCH (-3)
+#define NNP_ERR_CAPACITY (-4)  /* a centre has more neighbours than the row capacity */
+#define NNP_ERR_NONFINITE (-5) /* NaN/Inf position seen on the device */
+#define NNP_ERR_ALLOC (-6)
+
+typedef struct nnp_handle nnp_handle; /* opaque; owned by the library */
+
+/*
+ * Model description.  All pointers are HOST pointers and are copied by nnp_create (the caller may
+ * free them afterwards).  Values for ANI-2x: BASELINE.json configs[0] (restated in DESIGN.md).
+ */
+typedef struct {
+  int32_t n_species;       /* S; species index 0..S-1 (ANI-2x: 7, order H C N O F S Cl, reading S5) */
+  int32_t n_models;        /* M; ensemble size (8; 1 = the "1 NN" variant) */
+  float rc_radial;         /* radial cutoff in A (5.1) */
+  float rc_angular;        /* angular cutoff in A (3.5) */
+  float eta_r;             /* 19.7 */
+  int32_t n_shf_r;         /* 16 (<= 32) */
+  const float *shf_r;      /* host [n_shf_r] */
+  float eta_a;             /* 12.5 */
+  float zeta;              /* 14.1 */
+  int32_t n_shf_a;         /* 8 */
+  const float *shf_a;      /* host [n_shf_a] */
+  int32_t n_shf_z;         /* 4;  n_shf_a*n_shf_z <= 64 */
+  const float *shf_z;      /* host [n_shf_z] */
+  float cos_scale;         /* 0.95 (reading S6) */
+  float celu_alpha;        /* 0.1 */
+  int32_t n_layers;        /* 4 (must be >= 2; the last layer has 1 output) */
+  const int32_t *layer_dims; /* host [S][n_layers+1]; [e][0] must equal the AEV length */
+  const float *const *weights; /* host [M*S*n_layers] pointers, index (m*S+e)*n_layers+l, each row-major [out][in] */
+  const float *const *biases;  /* same indexing, each [out]; the array or any entry may be NULL => zeros */
+  const double *self_energy;   /* host [S] per-species energy shift in model units, or NULL */
+  double energy_scale;     /* output energy unit per model unit (627.5094740631: Hartree -> kcal/mol, S8) */
+  double length_scale;     /* A per caller length unit (1.0 = caller works in A; 10.0 = nm) */
+  int32_t max_radial_neighbors;  /* row capacity of the radial list; 0 = library default */
+  int32_t max_angular_neighbors; /* row capacity of the angular list; 0 = library default */
+  int32_t flags;           /* NNP_FLAG_* */
+} nnp_config;
+
+#define NNP_FLAG_NO_GRAPH 1 /* launch kernels one by one instead of replaying a CUDA graph */
+
+/*
+ * nnp_create: build a handle for a fixed set of atoms.
+ *   out               host; receives the handle
+ *   cfg               host; model description, copied
+ *   n_atoms           number of NNP atoms N (>= 0; N == 0 gives a handle whose compute is a no-op)
+ *   species_host      host i32[N], values in 0..S-1
+ *   n_molecules       number of independent molecules in the batch (>= 1)
+ *   mol_offsets_host  host i32[n_molecules+1] CSR offsets, molecules are contiguous atom ranges
+ *                     (mol_offsets[0]=0, last=N); NULL => one molecule.  Atoms of different
+ *                     molecules never interact (BASELINE.json configs[2]).
+ * Allocates all device memory; uploads and re-packs the weights; groups atoms by element.
+ */
+int nnp_create(nnp_handle **out, const nnp_config *cfg, int32_t n_atoms, const int32_t *species_host,
+               int32_t n_molecules, const int32_t *mol_offsets_host);
+
+/*
+ * nnp_compute: one energy+force evaluation (one MD step), enqueued on `cuda_stream`.
+ *   d_pos               device f32; position of NNP atom a is at d_pos[row(a)*pos_stride_floats + 0..2]
+ *                       in caller length units (x length_scale = A)
+ *   pos_stride_floats   3 (xyz) or 4 (float4 "posq") or any stride >= 3
+ *   d_atom_index        device i32[N] row(a) of NNP atom a in the caller's position/force buffers,
+ *                       or NULL => row(a) = a
+ *   d_energy            device f64[n_molecules]; WRITTEN (not accumulated): E_mol in output energy units
+ *   d_force_accum       device f32; F_NNP (output energy unit per caller length unit) is ADDED in place at
+ *                       d_force_accum[row(a)*force_stride_floats + 0..2]; may be NULL (energy only still
+ *                       runs the whole path)
+ *   force_stride_floats >= 3
+ *   cuda_stream         a cudaStream_t (0 = legacy default stream); borrowed
+ * No host synchronisation; buffers are borrowed until the enqueued work has run.
+ */
+int nnp_compute(nnp_handle *h, const float *d_pos, int32_t pos_stride_floats, const int32_t *d_atom_index,
+                double *d_energy, float *d_force_accum, int32_t force_stride_floats, void *cuda_stream);
+
+/*
+ * nnp_compute_host: the same evaluation for HOST buffers (used for end-to-end timing and by callers
+ * without device data): copies pos_host f32[N][3] to the device, runs nnp_compute, copies back
+ * energy_host f64[n_molecules] and force_host f32[N][3] (forces are WRITTEN, not accumulated), and
+ * synchronises the stream before returning.  Every step of the path still runs on the GPU.
+ */
+int nnp_compute_host(nnp_handle *h, const float *pos_host, double *energy_host, float *force_host,
+                     void *cuda_stream);
+
+/* nnp_status: synchronises the last used stream and returns the sticky device status (NNP_OK or
+ * NNP_ERR_CAPACITY / NNP_ERR_NONFINITE / NNP_ERR_CUDA); the flag is cleared by the call. */
+int nnp_status(nnp_handle *h);
+
+/* nnp_destroy: frees everything owned by the handle (NULL is allowed). */
+void nnp_destroy(nnp_handle *h);
+
+/* nnp_error_string: static string for a status code. */
+const char *nnp_error_string(int code);
+
+/* Number of kernel launches (graph nodes) one nnp_compute enqueues. */
+int nnp_launches_per_compute(nnp_handle *h);
+
+/*
+ * Stage timing (measurement only).  nnp_set_profiling(h,1) makes nnp_compute launch its kernels one by
+ * one with CUDA events between stages; nnp_get_stage_times then synchronises and returns, for the last
+ * compute, the duration in ms of each stage (ms_host f32[capacity]) and the stage count; names via
+ * nnp_stage_name.  Profiling mode is not the timed configuration.
+ */
+int nnp_set_profiling(nnp_handle *h, int32_t enable);
+int nnp_get_stage_times(nnp_handle *h, float *ms_host, int32_t capacity, int32_t *n_stages);
+const char *nnp_stage_name(nnp_handle *h, int32_t stage);
+
+/* Algorithmic bytes / flops of one compute, for roofline accounting:
+ * what[0] = weight bytes the MLP layers must read once, what[1] = MLP flops (2 per MAC, forward +
+ * input-gradient backward), what[2] = AEV bytes (write+read), what[3] = layer-1 weight bytes. */
+int nnp_get_work(nnp_handle *h, double *what_host, int32_t n);
+
+/*
+ * Debug / parity exports: copy device workspace of the LAST compute to the host after synchronising.
+ * Not on the timed path.  Atom indices are the caller's NNP atom order (0..N-1).
+ *   nnp_debug_pairs   which = 0 radial / 1 angular; writes directed pairs (i,j) as i32 pairs, row-major
+ *                     by centre i; *n_pairs receives the total even when it exceeds `capacity` pairs
+ *   nnp_debug_aev     f32[N][n_features]
+ *   nnp_debug_atomic_energies  f64[M][N], model units (before mean/scale)
+ *   nnp_debug_daev    f32[N][n_features] = dE_model_units/dAEV (mean over the ensemble)
+ */
+int nnp_debug_pairs(nnp_handle *h, int32_t which, int64_t *n_pairs, int32_t *ij_host, int64_t capacity);
+int nnp_debug_aev(nnp_handle *h, float *aev_host);
+int nnp_debug_atomic_energies(nnp_handle *h, double *e_host);
+int nnp_debug_daev(nnp_handle *h, float *g_host);
+int nnp_n_features(nnp_handle *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NNP_B200_H */

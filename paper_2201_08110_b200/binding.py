@@ -1,0 +1,273 @@
+"""Thin ctypes binding of include/nnp.h (argument marshalling only; every step runs in the CUDA kernels).
+
+Names follow the header: create / compute / compute_host / status / destroy and the debug exports.
+There is no CPU fallback: if libnnp_b200.so is missing or no sm_100 GPU is present this raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libnnp_b200.so")
+
+NNP_OK = 0
+NNP_FLAG_NO_GRAPH = 1
+ERRORS = {
+    -1: "NNP_ERR_INVALID_ARG",
+    -2: "NNP_ERR_CUDA",
+    -3: "NNP_ERR_UNSUPPORTED_ARCH",
+    -4: "NNP_ERR_CAPACITY",
+    -5: "NNP_ERR_NONFINITE",
+    -6: "NNP_ERR_ALLOC",
+}
+
+# every symbol include/nnp.h declares (tests check the library exports exactly these)
+SYMBOLS = (
+    "nnp_create", "nnp_compute", "nnp_compute_host", "nnp_status", "nnp_destroy", "nnp_error_string",
+    "nnp_launches_per_compute", "nnp_set_profiling", "nnp_get_stage_times", "nnp_stage_name", "nnp_get_work",
+    "nnp_debug_pairs", "nnp_debug_aev", "nnp_debug_atomic_energies", "nnp_debug_daev", "nnp_n_features",
+)
+
+
+class NNPError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {ERRORS.get(code, code)}")
+
+
+class _Config(C.Structure):
+    _fields_ = [
+        ("n_species", C.c_int32),
+        ("n_models", C.c_int32),
+        ("rc_radial", C.c_float),
+        ("rc_angular", C.c_float),
+        ("eta_r", C.c_float),
+        ("n_shf_r", C.c_int32),
+        ("shf_r", C.POINTER(C.c_float)),
+        ("eta_a", C.c_float),
+        ("zeta", C.c_float),
+        ("n_shf_a", C.c_int32),
+        ("shf_a", C.POINTER(C.c_float)),
+        ("n_shf_z", C.c_int32),
+        ("shf_z", C.POINTER(C.c_float)),
+        ("cos_scale", C.c_float),
+        ("celu_alpha", C.c_float),
+        ("n_layers", C.c_int32),
+        ("layer_dims", C.POINTER(C.c_int32)),
+        ("weights", C.POINTER(C.c_void_p)),
+        ("biases", C.POINTER(C.c_void_p)),
+        ("self_energy", C.POINTER(C.c_double)),
+        ("energy_scale", C.c_double),
+        ("length_scale", C.c_double),
+        ("max_radial_neighbors", C.c_int32),
+        ("max_angular_neighbors", C.c_int32),
+        ("flags", C.c_int32),
+    ]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libnnp_b200.so (built in-tree by paper_2201_08110_b200.build); raises if missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(
+                f"{LIB_PATH} not built: run `python -m paper_2201_08110_b200.build` (there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        lib.nnp_create.restype = C.c_int
+        lib.nnp_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(_Config), C.c_int32, C.c_void_p, C.c_int32,
+                                   C.c_void_p]
+        lib.nnp_compute.restype = C.c_int
+        lib.nnp_compute.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
+                                    C.c_void_p]
+        lib.nnp_compute_host.restype = C.c_int
+        lib.nnp_compute_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.nnp_status.restype = C.c_int
+        lib.nnp_status.argtypes = [C.c_void_p]
+        lib.nnp_destroy.restype = None
+        lib.nnp_destroy.argtypes = [C.c_void_p]
+        lib.nnp_error_string.restype = C.c_char_p
+        lib.nnp_error_string.argtypes = [C.c_int]
+        lib.nnp_launches_per_compute.restype = C.c_int
+        lib.nnp_launches_per_compute.argtypes = [C.c_void_p]
+        lib.nnp_set_profiling.restype = C.c_int
+        lib.nnp_set_profiling.argtypes = [C.c_void_p, C.c_int32]
+        lib.nnp_get_stage_times.restype = C.c_int
+        lib.nnp_get_stage_times.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(C.c_int32)]
+        lib.nnp_stage_name.restype = C.c_char_p
+        lib.nnp_stage_name.argtypes = [C.c_void_p, C.c_int32]
+        lib.nnp_get_work.restype = C.c_int
+        lib.nnp_get_work.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
+        lib.nnp_debug_pairs.restype = C.c_int
+        lib.nnp_debug_pairs.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_int64), C.c_void_p, C.c_int64]
+        for name in ("nnp_debug_aev", "nnp_debug_atomic_energies", "nnp_debug_daev"):
+            getattr(lib, name).restype = C.c_int
+            getattr(lib, name).argtypes = [C.c_void_p, C.c_void_p]
+        lib.nnp_n_features.restype = C.c_int
+        lib.nnp_n_features.argtypes = [C.c_void_p]
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int, where: str):
+    if rc != NNP_OK:
+        raise NNPError(rc, where)
+
+
+class NNP:
+    """One nnp_handle: a fixed set of NNP atoms + one model."""
+
+    def __init__(self, params, weights, biases, species, mol_offsets=None, self_energy=None, energy_scale=None,
+                 length_scale: float = 1.0, max_radial_neighbors: int = 0, max_angular_neighbors: int = 0,
+                 flags: int = 0):
+        self.lib = load_library()
+        S = int(params.n_species)
+        M = len(weights)
+        dims = np.ascontiguousarray(params.layer_dims, dtype=np.int32)
+        L = dims.shape[1] - 1
+        keep = []
+        f32 = lambda v: np.ascontiguousarray(v, dtype=np.float32)
+        shf_r, shf_a, shf_z = f32(params.shf_r), f32(params.shf_a), f32(params.shf_z)
+        wptr = (C.c_void_p * (M * S * L))()
+        bptr = (C.c_void_p * (M * S * L))()
+        for m in range(M):
+            for e in range(S):
+                for l in range(L):
+                    idx = (m * S + e) * L + l
+                    w = f32(weights[m][e][l])
+                    assert w.shape == (dims[e, l + 1], dims[e, l])
+                    keep.append(w)
+                    wptr[idx] = w.ctypes.data
+                    if biases is not None:
+                        b = f32(biases[m][e][l])
+                        keep.append(b)
+                        bptr[idx] = b.ctypes.data
+        fp = lambda a: a.ctypes.data_as(C.POINTER(C.c_float))
+        cfg = _Config()
+        cfg.n_species, cfg.n_models = S, M
+        cfg.rc_radial, cfg.rc_angular = float(params.rc_radial), float(params.rc_angular)
+        cfg.eta_r, cfg.n_shf_r, cfg.shf_r = float(params.eta_r), shf_r.size, fp(shf_r)
+        cfg.eta_a, cfg.zeta = float(params.eta_a), float(params.zeta)
+        cfg.n_shf_a, cfg.shf_a, cfg.n_shf_z, cfg.shf_z = shf_a.size, fp(shf_a), shf_z.size, fp(shf_z)
+        cfg.cos_scale, cfg.celu_alpha = float(params.cos_scale), float(params.celu_alpha)
+        cfg.n_layers, cfg.layer_dims = L, dims.ctypes.data_as(C.POINTER(C.c_int32))
+        cfg.weights = C.cast(wptr, C.POINTER(C.c_void_p))
+        cfg.biases = C.cast(bptr, C.POINTER(C.c_void_p)) if biases is not None else None
+        se = None
+        if self_energy is not None:
+            se = np.ascontiguousarray(self_energy, dtype=np.float64)
+            cfg.self_energy = se.ctypes.data_as(C.POINTER(C.c_double))
+        cfg.energy_scale = float(params.energy_scale if energy_scale is None else energy_scale)
+        cfg.length_scale = float(length_scale)
+        cfg.max_radial_neighbors, cfg.max_angular_neighbors, cfg.flags = max_radial_neighbors, max_angular_neighbors, flags
+        spc = np.ascontiguousarray(species, dtype=np.int32)
+        self.n_atoms = int(spc.size)
+        off = None
+        self.n_molecules = 1
+        if mol_offsets is not None:
+            off = np.ascontiguousarray(mol_offsets, dtype=np.int32)
+            self.n_molecules = int(off.size - 1)
+        self.n_models = M
+        h = C.c_void_p()
+        rc = self.lib.nnp_create(C.byref(h), C.byref(cfg), self.n_atoms, spc.ctypes.data if spc.size else None,
+                                 self.n_molecules, off.ctypes.data if off is not None else None)
+        _check(rc, "nnp_create")
+        self.h = h
+        self.n_features = int(self.lib.nnp_n_features(self.h))
+
+    # ---- the hot path
+    def compute(self, d_pos: int, pos_stride: int, d_atom_index, d_energy: int, d_force, force_stride: int,
+                stream: int = 0):
+        """nnp_compute with raw device addresses (ints)."""
+        _check(self.lib.nnp_compute(self.h, d_pos, pos_stride, d_atom_index, d_energy, d_force, force_stride,
+                                    stream or None), "nnp_compute")
+
+    def compute_torch(self, pos, energy, force=None, atom_index=None, stream=None):
+        """nnp_compute on torch CUDA tensors (device memory + stream plumbing only)."""
+        import torch
+
+        assert pos.is_cuda and pos.dtype == torch.float32 and pos.stride(-1) == 1
+        assert energy.is_cuda and energy.dtype == torch.float64
+        s = torch.cuda.current_stream().cuda_stream if stream is None else stream
+        self.compute(pos.data_ptr(), int(pos.stride(0)), atom_index.data_ptr() if atom_index is not None else None,
+                     energy.data_ptr(), force.data_ptr() if force is not None else None,
+                     int(force.stride(0)) if force is not None else 3, s)
+
+    def compute_host(self, pos_host: np.ndarray, stream: int = 0):
+        """nnp_compute_host: host positions in, host (E f64[n_mol], F f32[N,3]) out."""
+        pos = np.ascontiguousarray(pos_host, dtype=np.float32)
+        E = np.empty(self.n_molecules, dtype=np.float64)
+        F = np.empty((self.n_atoms, 3), dtype=np.float32)
+        _check(self.lib.nnp_compute_host(self.h, pos.ctypes.data, E.ctypes.data, F.ctypes.data, stream or None),
+               "nnp_compute_host")
+        return E, F
+
+    def compute_host_into(self, pos_ptr: int, e_ptr: int, f_ptr: int, stream: int = 0):
+        _check(self.lib.nnp_compute_host(self.h, pos_ptr, e_ptr, f_ptr, stream or None), "nnp_compute_host")
+
+    def status(self) -> int:
+        return int(self.lib.nnp_status(self.h))
+
+    def check(self):
+        _check(self.status(), "nnp_status")
+
+    # ---- measurement helpers
+    @property
+    def launches_per_compute(self) -> int:
+        return int(self.lib.nnp_launches_per_compute(self.h))
+
+    def set_profiling(self, on: bool):
+        _check(self.lib.nnp_set_profiling(self.h, 1 if on else 0), "nnp_set_profiling")
+
+    def stage_times(self):
+        n = C.c_int32()
+        _check(self.lib.nnp_get_stage_times(self.h, None, 0, C.byref(n)), "nnp_get_stage_times")
+        ms = np.zeros(n.value, dtype=np.float32)
+        _check(self.lib.nnp_get_stage_times(self.h, ms.ctypes.data, n.value, C.byref(n)), "nnp_get_stage_times")
+        names = [self.lib.nnp_stage_name(self.h, k).decode() for k in range(n.value)]
+        return dict(zip(names, ms.tolist()))
+
+    def work(self):
+        w = np.zeros(4, dtype=np.float64)
+        _check(self.lib.nnp_get_work(self.h, w.ctypes.data, 4), "nnp_get_work")
+        return {"weight_bytes": w[0], "mlp_flops": w[1], "aev_bytes": w[2], "layer1_weight_bytes": w[3]}
+
+    # ---- debug / parity exports
+    def debug_pairs(self, which: str = "radial") -> np.ndarray:
+        w = 0 if which == "radial" else 1
+        n = C.c_int64()
+        _check(self.lib.nnp_debug_pairs(self.h, w, C.byref(n), None, 0), "nnp_debug_pairs")
+        ij = np.empty((max(n.value, 1), 2), dtype=np.int32)
+        _check(self.lib.nnp_debug_pairs(self.h, w, C.byref(n), ij.ctypes.data, n.value), "nnp_debug_pairs")
+        return ij[: n.value]
+
+    def debug_aev(self) -> np.ndarray:
+        out = np.empty((self.n_atoms, self.n_features), dtype=np.float32)
+        _check(self.lib.nnp_debug_aev(self.h, out.ctypes.data), "nnp_debug_aev")
+        return out
+
+    def debug_daev(self) -> np.ndarray:
+        out = np.empty((self.n_atoms, self.n_features), dtype=np.float32)
+        _check(self.lib.nnp_debug_daev(self.h, out.ctypes.data), "nnp_debug_daev")
+        return out
+
+    def debug_atomic_energies(self) -> np.ndarray:
+        out = np.empty((self.n_models, self.n_atoms), dtype=np.float64)
+        _check(self.lib.nnp_debug_atomic_energies(self.h, out.ctypes.data), "nnp_debug_atomic_energies")
+        return out
+
+    def destroy(self):
+        if getattr(self, "h", None) is not None and self.h:
+            self.lib.nnp_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

@@ -1,0 +1,558 @@
+// C-ABI entry points of libnnp_b200 (include/nnp.h): handle set-up (A0), the per-step launch chain
+// (A1..A8) replayed as one CUDA graph, status, profiling and the debug/parity exports.
+#include <math.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+
+#include "nnp_internal.h"
+
+int aev_set_smem_attributes(nnp_handle* h);
+
+#define CK(call)                                  \
+  do {                                            \
+    cudaError_t _e = (call);                      \
+    if (_e != cudaSuccess) return NNP_ERR_CUDA;   \
+  } while (0)
+
+namespace {
+
+template <typename T>
+int dev_alloc(T** p, size_t n) {
+  *p = nullptr;
+  if (n == 0) n = 1;
+  return cudaMalloc((void**)p, n * sizeof(T)) == cudaSuccess ? 0 : -1;
+}
+
+template <typename T>
+int upload(T** p, const std::vector<T>& v) {
+  if (dev_alloc(p, v.size())) return -1;
+  if (!v.empty() && cudaMemcpy(*p, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess) return -1;
+  return 0;
+}
+
+long long align_up(long long x, long long a) { return (x + a - 1) / a * a; }
+
+int upload_launch(GemmLaunch& g, const std::vector<GemmProblem>& probs) {
+  std::vector<GemmTile> tiles;
+  build_gemm_tiles(probs, tiles);
+  g.n_tiles = (int)tiles.size();
+  if (upload(&g.d_probs, probs)) return -1;
+  if (upload(&g.d_tiles, tiles)) return -1;
+  return 0;
+}
+
+}  // namespace
+
+extern "C" const char* nnp_error_string(int code) {
+  switch (code) {
+    case NNP_OK: return "ok";
+    case NNP_ERR_INVALID_ARG: return "invalid argument";
+    case NNP_ERR_CUDA: return "CUDA error";
+    case NNP_ERR_UNSUPPORTED_ARCH: return "unsupported GPU architecture (need sm_100)";
+    case NNP_ERR_CAPACITY: return "neighbour row capacity exceeded";
+    case NNP_ERR_NONFINITE: return "non-finite position";
+    case NNP_ERR_ALLOC: return "allocation failed";
+    default: return "unknown error";
+  }
+}
+
+extern "C" void nnp_destroy(nnp_handle* h) {
+  if (!h) return;
+  cudaSetDevice(h->device);
+  if (h->last_stream) cudaStreamSynchronize(h->last_stream);
+  cudaDeviceSynchronize();
+  if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+  for (auto e : h->events) cudaEventDestroy(e);
+  void* ptrs[] = {h->d_species, h->d_mol_off, h->d_mol_id, h->d_sortpos, h->d_perm, h->d_grp_off, h->d_self_energy,
+                  h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_aev, h->d_daev, h->d_phi,
+                  h->d_eatom, h->d_status, h->d_W, h->d_b, h->d_last_act_off, h->d_last_w_off, h->d_last_b_off,
+                  h->d_last_H, h->d_hpos, h->d_hforce, h->d_henergy};
+  for (void* p : ptrs)
+    if (p) cudaFree(p);
+  for (int l = 0; l < NNP_MAX_LAYERS; ++l)
+    if (h->d_act[l]) cudaFree(h->d_act[l]);
+  for (auto* v : {&h->fwd, &h->bwd})
+    for (auto& g : *v) {
+      if (g.d_probs) cudaFree(g.d_probs);
+      if (g.d_tiles) cudaFree(g.d_tiles);
+    }
+  delete h;
+}
+
+extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_atoms, const int32_t* species_host,
+                          int32_t n_molecules, const int32_t* mol_offsets_host) {
+  if (!out) return NNP_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!cfg || n_atoms < 0 || (n_atoms > 0 && !species_host) || n_molecules < 1) return NNP_ERR_INVALID_ARG;
+  const int S = cfg->n_species, M = cfg->n_models, L = cfg->n_layers;
+  if (S < 1 || S > NNP_MAX_SPECIES || M < 1 || L < 2 || L > NNP_MAX_LAYERS) return NNP_ERR_INVALID_ARG;
+  if (cfg->n_shf_r < 1 || cfg->n_shf_r > NNP_MAX_SHF_R || cfg->n_shf_a < 1 || cfg->n_shf_a > NNP_MAX_SHF_A ||
+      cfg->n_shf_z < 1 || cfg->n_shf_z > NNP_MAX_SHF_Z || cfg->n_shf_a * cfg->n_shf_z > NNP_MAX_SUB)
+    return NNP_ERR_INVALID_ARG;
+  if (!cfg->shf_r || !cfg->shf_a || !cfg->shf_z || !cfg->layer_dims || !cfg->weights) return NNP_ERR_INVALID_ARG;
+  if (!(cfg->rc_radial > 0.f) || !(cfg->rc_angular > 0.f) || cfg->rc_angular > cfg->rc_radial)
+    return NNP_ERR_INVALID_ARG;
+  if (!(cfg->celu_alpha > 0.f) || !(cfg->length_scale > 0.0)) return NNP_ERR_INVALID_ARG;
+  const int n_sub = cfg->n_shf_a * cfg->n_shf_z;
+  const int n_radial = S * cfg->n_shf_r;
+  const int n_feat = n_radial + (S * (S + 1) / 2) * n_sub;
+  for (int e = 0; e < S; ++e) {
+    const int32_t* d = cfg->layer_dims + (size_t)e * (L + 1);
+    if (d[0] != n_feat || d[L] != 1) return NNP_ERR_INVALID_ARG;
+    for (int l = 0; l < L; ++l)
+      if (d[l] < 1 || d[l] % 4 != 0) return NNP_ERR_INVALID_ARG;  // float4 row loads
+  }
+  for (int i = 0; i < n_atoms; ++i)
+    if (species_host[i] < 0 || species_host[i] >= S) return NNP_ERR_INVALID_ARG;
+  std::vector<int> mol_off(n_molecules + 1);
+  if (mol_offsets_host) {
+    for (int m = 0; m <= n_molecules; ++m) mol_off[m] = mol_offsets_host[m];
+    if (mol_off[0] != 0 || mol_off[n_molecules] != n_atoms) return NNP_ERR_INVALID_ARG;
+    for (int m = 0; m < n_molecules; ++m)
+      if (mol_off[m + 1] < mol_off[m]) return NNP_ERR_INVALID_ARG;
+  } else {
+    if (n_molecules != 1) return NNP_ERR_INVALID_ARG;
+    mol_off[0] = 0;
+    mol_off[1] = n_atoms;
+  }
+
+  int dev = 0;
+  CK(cudaGetDevice(&dev));
+  cudaDeviceProp prop;
+  CK(cudaGetDeviceProperties(&prop, dev));
+  if (prop.major != 10) return NNP_ERR_UNSUPPORTED_ARCH;  // binary holds sm_100a code only
+
+  nnp_handle* h = new (std::nothrow) nnp_handle();
+  if (!h) return NNP_ERR_ALLOC;
+  h->device = dev;
+  h->N = n_atoms; h->n_mol = n_molecules; h->S = S; h->M = M; h->L = L; h->n_feat = n_feat;
+  h->flags = cfg->flags;
+  h->energy_scale = cfg->energy_scale;
+  h->length_scale = cfg->length_scale;
+  h->dims.assign(cfg->layer_dims, cfg->layer_dims + (size_t)S * (L + 1));
+
+  AevConst& a = h->aev;
+  memset(&a, 0, sizeof(a));
+  a.S = S; a.n_shf_r = cfg->n_shf_r; a.n_shf_a = cfg->n_shf_a; a.n_shf_z = cfg->n_shf_z;
+  a.n_sub = n_sub; a.n_radial = n_radial; a.n_feat = n_feat;
+  a.rc_r = cfg->rc_radial; a.rc_a = cfg->rc_angular; a.eta_r = cfg->eta_r; a.eta_a = cfg->eta_a;
+  a.zeta = cfg->zeta; a.cos_scale = cfg->cos_scale; a.length_scale = (float)cfg->length_scale;
+  a.rc_r2 = (double)cfg->rc_radial * (double)cfg->rc_radial;
+  a.rc_a2 = (double)cfg->rc_angular * (double)cfg->rc_angular;
+  for (int k = 0; k < cfg->n_shf_r; ++k) a.shf_r[k] = cfg->shf_r[k];
+  for (int k = 0; k < cfg->n_shf_a; ++k) a.shf_a[k] = cfg->shf_a[k];
+  for (int k = 0; k < cfg->n_shf_z; ++k) {
+    a.cos_z[k] = (float)cos((double)cfg->shf_z[k]);
+    a.sin_z[k] = (float)sin((double)cfg->shf_z[k]);
+  }
+
+  // ---- A0: group atoms by element (stable), molecule ids, capacities
+  const int N = n_atoms;
+  std::vector<int> species(species_host, species_host + N), perm(N), sortpos(N), mol_id(N);
+  h->grp_off.assign(S + 1, 0);
+  for (int i = 0; i < N; ++i) h->grp_off[species[i] + 1]++;
+  for (int e = 0; e < S; ++e) h->grp_off[e + 1] += h->grp_off[e];
+  {
+    std::vector<int> cur(h->grp_off.begin(), h->grp_off.end() - 1);
+    for (int i = 0; i < N; ++i) {
+      const int p = cur[species[i]]++;
+      perm[p] = i;
+      sortpos[i] = p;
+    }
+  }
+  int max_mol = 1;
+  for (int m = 0; m < n_molecules; ++m) {
+    for (int i = mol_off[m]; i < mol_off[m + 1]; ++i) mol_id[i] = m;
+    max_mol = std::max(max_mol, mol_off[m + 1] - mol_off[m]);
+  }
+  h->capR = cfg->max_radial_neighbors > 0 ? cfg->max_radial_neighbors : std::min(std::max(max_mol - 1, 1), 256);
+  h->capA = cfg->max_angular_neighbors > 0 ? cfg->max_angular_neighbors : std::min(std::max(max_mol - 1, 1), 128);
+  if (h->capA > h->capR) h->capA = h->capR;
+
+  int rc = NNP_OK;
+  auto fail = [&](int code) {
+    nnp_destroy(h);
+    return code;
+  };
+  if (aev_smem_bytes(h, true) > (size_t)prop.sharedMemPerBlockOptin || aev_set_smem_attributes(h) != 0)
+    return fail(NNP_ERR_INVALID_ARG);
+
+  if (upload(&h->d_species, species) || upload(&h->d_mol_off, mol_off) || upload(&h->d_mol_id, mol_id) ||
+      upload(&h->d_sortpos, sortpos) || upload(&h->d_perm, perm) || upload(&h->d_grp_off, h->grp_off))
+    return fail(NNP_ERR_ALLOC);
+  if (cfg->self_energy) {
+    std::vector<double> se(cfg->self_energy, cfg->self_energy + S);
+    if (upload(&h->d_self_energy, se)) return fail(NNP_ERR_ALLOC);
+  }
+
+  // ---- weights: arena ordered (element, layer, model); models of one (e,l) are contiguous so the
+  // layer-1 backward over the whole ensemble is a single GEMM with K = M*H1.
+  h->w_off.assign((size_t)S * L, 0);
+  h->b_off.assign((size_t)S * L, 0);
+  long long wo = 0, bo = 0;
+  for (int e = 0; e < S; ++e)
+    for (int l = 0; l < L; ++l) {
+      const int nin = h->dims[e * (L + 1) + l], nout = h->dims[e * (L + 1) + l + 1];
+      h->w_off[e * L + l] = wo;
+      h->b_off[e * L + l] = bo;
+      wo = align_up(wo + (long long)M * nout * nin, 64);
+      bo = align_up(bo + (long long)M * nout, 64);
+    }
+  h->w_floats = (size_t)wo;
+  h->b_floats = (size_t)bo;
+  {
+    std::vector<float> W((size_t)wo, 0.f), B((size_t)bo, 0.f);
+    for (int m = 0; m < M; ++m)
+      for (int e = 0; e < S; ++e)
+        for (int l = 0; l < L; ++l) {
+          const int nin = h->dims[e * (L + 1) + l], nout = h->dims[e * (L + 1) + l + 1];
+          const size_t idx = ((size_t)m * S + e) * L + l;
+          const float* src = cfg->weights[idx];
+          if (!src) return fail(NNP_ERR_INVALID_ARG);
+          memcpy(&W[h->w_off[e * L + l] + (size_t)m * nout * nin], src, sizeof(float) * (size_t)nout * nin);
+          if (cfg->biases && cfg->biases[idx])
+            memcpy(&B[h->b_off[e * L + l] + (size_t)m * nout], cfg->biases[idx], sizeof(float) * nout);
+        }
+    if (upload(&h->d_W, W) || upload(&h->d_b, B)) return fail(NNP_ERR_ALLOC);
+  }
+
+  // ---- workspaces
+  if (dev_alloc(&h->d_pos4, (size_t)N) || dev_alloc(&h->d_nbr_r, (size_t)N * h->capR) ||
+      dev_alloc(&h->d_nbr_a, (size_t)N * h->capA) || dev_alloc(&h->d_cnt_r, (size_t)N) ||
+      dev_alloc(&h->d_cnt_a, (size_t)N) || dev_alloc(&h->d_aev, (size_t)N * n_feat) ||
+      dev_alloc(&h->d_daev, (size_t)N * n_feat) || dev_alloc(&h->d_phi, (size_t)N * h->capR * 3) ||
+      dev_alloc(&h->d_eatom, (size_t)N * M) || dev_alloc(&h->d_status, 1) || dev_alloc(&h->d_hpos, (size_t)N * 3) ||
+      dev_alloc(&h->d_hforce, (size_t)N * 3) || dev_alloc(&h->d_henergy, (size_t)n_molecules))
+    return fail(NNP_ERR_ALLOC);
+  cudaMemset(h->d_status, 0, sizeof(int));
+  cudaMemset(h->d_nbr_r, 0, sizeof(int) * std::max<size_t>((size_t)N * h->capR, 1));
+  cudaMemset(h->d_nbr_a, 0, sizeof(int) * std::max<size_t>((size_t)N * h->capA, 1));
+  cudaMemset(h->d_cnt_r, 0, sizeof(int) * std::max<size_t>(N, 1));
+  cudaMemset(h->d_cnt_a, 0, sizeof(int) * std::max<size_t>(N, 1));
+  cudaMemset(h->d_phi, 0, sizeof(float) * std::max<size_t>((size_t)N * h->capR * 3, 1));
+  cudaMemset(h->d_eatom, 0, sizeof(double) * std::max<size_t>((size_t)N * M, 1));
+
+  // activations act[l], l = 1..L-1, layout per element group: [atom][model][H_l]
+  for (int l = 1; l < L; ++l) {
+    h->act_off[l].assign(S, 0);
+    long long o = 0;
+    for (int e = 0; e < S; ++e) {
+      h->act_off[l][e] = o;
+      const long long ne = h->grp_off[e + 1] - h->grp_off[e];
+      o = align_up(o + ne * M * h->dims[e * (L + 1) + l], 64);
+    }
+    if (dev_alloc(&h->d_act[l], (size_t)o)) return fail(NNP_ERR_ALLOC);
+  }
+
+  // ---- MLP launches (grouped GEMMs), shapes fixed at create time
+  const float alpha = cfg->celu_alpha;
+  double flops = 0, wbytes = 0, w1bytes = 0;
+  for (int l = 1; l < L; ++l) {  // forward hidden layers
+    std::vector<GemmProblem> probs;
+    for (int e = 0; e < S; ++e) {
+      const int ne = h->grp_off[e + 1] - h->grp_off[e];
+      if (ne == 0) continue;
+      const int nin = h->dims[e * (L + 1) + l - 1], nout = h->dims[e * (L + 1) + l];
+      for (int m = 0; m < M; ++m) {
+        GemmProblem p;
+        memset(&p, 0, sizeof(p));
+        if (l == 1) {
+          p.A = h->d_aev + (size_t)h->grp_off[e] * n_feat;
+          p.lda = n_feat;
+        } else {
+          p.A = h->d_act[l - 1] + h->act_off[l - 1][e] + (size_t)m * nin;
+          p.lda = M * nin;
+        }
+        p.B = h->d_W + h->w_off[e * L + l - 1] + (size_t)m * nout * nin;
+        p.ldb = nin;
+        p.transB = 0;
+        p.C = h->d_act[l] + h->act_off[l][e] + (size_t)m * nout;
+        p.ldc = M * nout;
+        p.bias = h->d_b + h->b_off[e * L + l - 1] + (size_t)m * nout;
+        p.M = ne; p.N = nout; p.K = nin;
+        p.epi = EPI_BIAS_CELU;
+        p.alpha = alpha;
+        probs.push_back(p);
+        flops += 4.0 * ne * (double)nout * nin;
+        wbytes += 4.0 * nout * nin;
+        if (l == 1) w1bytes += 4.0 * nout * nin;
+      }
+    }
+    GemmLaunch g;
+    g.name = "mlp_fwd_l" + std::to_string(l);
+    if (upload_launch(g, probs)) return fail(NNP_ERR_ALLOC);
+    h->fwd.push_back(g);
+  }
+  for (int l = L - 1; l >= 1; --l) {  // backward through hidden layer l: delta_{l-1} = delta_l W_l (.) CELU'
+    std::vector<GemmProblem> probs;
+    for (int e = 0; e < S; ++e) {
+      const int ne = h->grp_off[e + 1] - h->grp_off[e];
+      if (ne == 0) continue;
+      const int nin = h->dims[e * (L + 1) + l - 1], nout = h->dims[e * (L + 1) + l];
+      if (l > 1) {
+        for (int m = 0; m < M; ++m) {
+          GemmProblem p;
+          memset(&p, 0, sizeof(p));
+          p.A = h->d_act[l] + h->act_off[l][e] + (size_t)m * nout;
+          p.lda = M * nout;
+          p.B = h->d_W + h->w_off[e * L + l - 1] + (size_t)m * nout * nin;
+          p.ldb = nin;
+          p.transB = 1;
+          p.C = h->d_act[l - 1] + h->act_off[l - 1][e] + (size_t)m * nin;
+          p.ldc = M * nin;
+          p.aux = p.C;
+          p.ldaux = p.ldc;
+          p.M = ne; p.N = nin; p.K = nout;
+          p.epi = EPI_MUL_DCELU;
+          p.alpha = alpha;
+          probs.push_back(p);
+        }
+      } else {  // layer 1: dE/dAEV = (1/M) sum_m delta_1^(m) W_1^(m): one GEMM with K = M*H1
+        GemmProblem p;
+        memset(&p, 0, sizeof(p));
+        p.A = h->d_act[1] + h->act_off[1][e];
+        p.lda = M * nout;
+        p.B = h->d_W + h->w_off[e * L + 0];
+        p.ldb = nin;
+        p.transB = 1;
+        p.C = h->d_daev + (size_t)h->grp_off[e] * n_feat;
+        p.ldc = n_feat;
+        p.M = ne; p.N = nin; p.K = M * nout;
+        p.epi = EPI_SCALE;
+        p.scale = 1.0f / (float)M;
+        probs.push_back(p);
+      }
+    }
+    GemmLaunch g;
+    g.name = "mlp_bwd_l" + std::to_string(l);
+    if (upload_launch(g, probs)) return fail(NNP_ERR_ALLOC);
+    h->bwd.push_back(g);
+  }
+  // last layer
+  {
+    std::vector<long long> ao(S), wo2(S), bo2(S);
+    std::vector<int> Hs(S);
+    for (int e = 0; e < S; ++e) {
+      ao[e] = h->act_off[L - 1][e];
+      wo2[e] = h->w_off[e * L + L - 1];
+      bo2[e] = h->b_off[e * L + L - 1];
+      Hs[e] = h->dims[e * (L + 1) + L - 1];
+      const int ne = h->grp_off[e + 1] - h->grp_off[e];
+      flops += 4.0 * ne * (double)M * Hs[e];
+      if (ne) wbytes += 4.0 * M * Hs[e];
+    }
+    if (upload(&h->d_last_act_off, ao) || upload(&h->d_last_w_off, wo2) || upload(&h->d_last_b_off, bo2) ||
+        upload(&h->d_last_H, Hs))
+      return fail(NNP_ERR_ALLOC);
+    LastLayerArgs& la = h->last;
+    la.act = h->d_act[L - 1]; la.W = h->d_W; la.bias = h->d_b; la.e_out = h->d_eatom;
+    la.grp_off = h->d_grp_off; la.act_off = h->d_last_act_off; la.w_off = h->d_last_w_off;
+    la.b_off = h->d_last_b_off; la.H = h->d_last_H;
+    la.S = S; la.M = M; la.n_sorted = N; la.alpha = alpha;
+  }
+  h->work[0] = wbytes;
+  h->work[1] = flops;
+  h->work[2] = 2.0 * 4.0 * (double)N * n_feat;
+  h->work[3] = w1bytes;
+
+  h->stage_names = {"nbr", "aev_fwd"};
+  for (auto& g : h->fwd) h->stage_names.push_back(g.name);
+  h->stage_names.push_back("mlp_last");
+  for (auto& g : h->bwd) h->stage_names.push_back(g.name);
+  h->stage_names.push_back("aev_bwd");
+  h->stage_names.push_back("finish");
+  h->n_launches = N > 0 ? (int)h->stage_names.size() : 0;
+  h->events.resize(h->stage_names.size() + 1);
+  for (auto& e : h->events)
+    if (cudaEventCreate(&e) != cudaSuccess) return fail(NNP_ERR_CUDA);
+  if (cudaDeviceSynchronize() != cudaSuccess) return fail(NNP_ERR_CUDA);
+  (void)rc;
+  *out = h;
+  return NNP_OK;
+}
+
+// enqueue the launch chain A1..A8 on `s`; with `ev` record an event before the first and after each stage
+static void enqueue_chain(nnp_handle* h, const float* d_pos, int ps, const int* d_idx, double* d_energy,
+                          float* d_force, int fs, cudaStream_t s, bool ev) {
+  int k = 0;
+  auto mark = [&]() {
+    if (ev) cudaEventRecord(h->events[k], s);
+    ++k;
+  };
+  mark();
+  launch_neighbors(h, d_pos, ps, d_idx, s); mark();
+  launch_aev_forward(h, s); mark();
+  for (auto& g : h->fwd) { launch_gemm(g, s); mark(); }
+  launch_last_layer(h, s); mark();
+  for (auto& g : h->bwd) { launch_gemm(g, s); mark(); }
+  launch_aev_backward(h, s); mark();
+  launch_finish(h, d_idx, d_energy, d_force, fs, s); mark();
+}
+
+extern "C" int nnp_compute(nnp_handle* h, const float* d_pos, int32_t pos_stride_floats,
+                           const int32_t* d_atom_index, double* d_energy, float* d_force_accum,
+                           int32_t force_stride_floats, void* cuda_stream) {
+  if (!h) return NNP_ERR_INVALID_ARG;
+  if (h->N == 0) return NNP_OK;
+  if (!d_pos || pos_stride_floats < 3 || (d_force_accum && force_stride_floats < 3)) return NNP_ERR_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  h->last_stream = s;
+  if (h->profiling || (h->flags & NNP_FLAG_NO_GRAPH)) {
+    enqueue_chain(h, d_pos, pos_stride_floats, d_atom_index, d_energy, d_force_accum, force_stride_floats, s,
+                  h->profiling);
+    return cudaGetLastError() == cudaSuccess ? NNP_OK : NNP_ERR_CUDA;
+  }
+  const bool same = h->graph_exec && h->g_pos == d_pos && h->g_idx == d_atom_index && h->g_energy == d_energy &&
+                    h->g_force == d_force_accum && h->g_ps == pos_stride_floats && h->g_fs == force_stride_floats;
+  if (!same) {
+    if (h->graph_exec) {
+      cudaGraphExecDestroy(h->graph_exec);
+      h->graph_exec = nullptr;
+    }
+    cudaStream_t cs;
+    CK(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+    cudaGraph_t graph = nullptr;
+    if (cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+      cudaStreamDestroy(cs);
+      return NNP_ERR_CUDA;
+    }
+    enqueue_chain(h, d_pos, pos_stride_floats, d_atom_index, d_energy, d_force_accum, force_stride_floats, cs, false);
+    cudaError_t e = cudaStreamEndCapture(cs, &graph);
+    cudaStreamDestroy(cs);
+    if (e != cudaSuccess || !graph) return NNP_ERR_CUDA;
+    e = cudaGraphInstantiate(&h->graph_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) {
+      h->graph_exec = nullptr;
+      return NNP_ERR_CUDA;
+    }
+    h->g_pos = d_pos; h->g_idx = d_atom_index; h->g_energy = d_energy; h->g_force = d_force_accum;
+    h->g_ps = pos_stride_floats; h->g_fs = force_stride_floats;
+  }
+  CK(cudaGraphLaunch(h->graph_exec, s));
+  return NNP_OK;
+}
+
+extern "C" int nnp_compute_host(nnp_handle* h, const float* pos_host, double* energy_host, float* force_host,
+                                void* cuda_stream) {
+  if (!h || (h->N > 0 && !pos_host)) return NNP_ERR_INVALID_ARG;
+  if (h->N == 0) return NNP_OK;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  CK(cudaMemcpyAsync(h->d_hpos, pos_host, sizeof(float) * 3 * (size_t)h->N, cudaMemcpyHostToDevice, s));
+  CK(cudaMemsetAsync(h->d_hforce, 0, sizeof(float) * 3 * (size_t)h->N, s));
+  int rc = nnp_compute(h, h->d_hpos, 3, nullptr, h->d_henergy, h->d_hforce, 3, cuda_stream);
+  if (rc != NNP_OK) return rc;
+  if (energy_host)
+    CK(cudaMemcpyAsync(energy_host, h->d_henergy, sizeof(double) * (size_t)h->n_mol, cudaMemcpyDeviceToHost, s));
+  if (force_host)
+    CK(cudaMemcpyAsync(force_host, h->d_hforce, sizeof(float) * 3 * (size_t)h->N, cudaMemcpyDeviceToHost, s));
+  CK(cudaStreamSynchronize(s));
+  return NNP_OK;
+}
+
+extern "C" int nnp_status(nnp_handle* h) {
+  if (!h) return NNP_ERR_INVALID_ARG;
+  if (cudaStreamSynchronize(h->last_stream) != cudaSuccess) return NNP_ERR_CUDA;
+  int st = 0;
+  if (cudaMemcpy(&st, h->d_status, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return NNP_ERR_CUDA;
+  if (cudaGetLastError() != cudaSuccess) return NNP_ERR_CUDA;
+  if (st) cudaMemset(h->d_status, 0, sizeof(int));
+  if (st & NNP_ST_NONFINITE) return NNP_ERR_NONFINITE;
+  if (st & NNP_ST_CAPACITY) return NNP_ERR_CAPACITY;
+  return NNP_OK;
+}
+
+extern "C" int nnp_launches_per_compute(nnp_handle* h) { return h ? h->n_launches : 0; }
+extern "C" int nnp_n_features(nnp_handle* h) { return h ? h->n_feat : 0; }
+
+extern "C" int nnp_set_profiling(nnp_handle* h, int32_t enable) {
+  if (!h) return NNP_ERR_INVALID_ARG;
+  h->profiling = enable != 0;
+  return NNP_OK;
+}
+
+extern "C" int nnp_get_stage_times(nnp_handle* h, float* ms_host, int32_t capacity, int32_t* n_stages) {
+  if (!h || !n_stages) return NNP_ERR_INVALID_ARG;
+  const int n = (int)h->stage_names.size();
+  *n_stages = n;
+  if (!ms_host) return NNP_OK;
+  CK(cudaStreamSynchronize(h->last_stream));
+  for (int k = 0; k < n && k < capacity; ++k) {
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, h->events[k], h->events[k + 1]));
+    ms_host[k] = ms;
+  }
+  return NNP_OK;
+}
+
+extern "C" const char* nnp_stage_name(nnp_handle* h, int32_t stage) {
+  if (!h || stage < 0 || stage >= (int)h->stage_names.size()) return "";
+  return h->stage_names[stage].c_str();
+}
+
+extern "C" int nnp_get_work(nnp_handle* h, double* what_host, int32_t n) {
+  if (!h || !what_host) return NNP_ERR_INVALID_ARG;
+  for (int k = 0; k < n && k < 4; ++k) what_host[k] = h->work[k];
+  return NNP_OK;
+}
+
+// ---------------------------------------------------------------- debug / parity exports
+extern "C" int nnp_debug_pairs(nnp_handle* h, int32_t which, int64_t* n_pairs, int32_t* ij_host, int64_t capacity) {
+  if (!h || !n_pairs || (which != 0 && which != 1)) return NNP_ERR_INVALID_ARG;
+  CK(cudaStreamSynchronize(h->last_stream));
+  const int N = h->N;
+  std::vector<int> nr((size_t)N * h->capR), cr(N), na((size_t)N * h->capA), ca(N);
+  if (N) {
+    CK(cudaMemcpy(nr.data(), h->d_nbr_r, nr.size() * sizeof(int), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(cr.data(), h->d_cnt_r, cr.size() * sizeof(int), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(na.data(), h->d_nbr_a, na.size() * sizeof(int), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(ca.data(), h->d_cnt_a, ca.size() * sizeof(int), cudaMemcpyDeviceToHost));
+  }
+  int64_t cnt = 0;
+  for (int i = 0; i < N; ++i) {
+    const int n = which == 0 ? cr[i] : ca[i];
+    for (int q = 0; q < n; ++q) {
+      const int j = which == 0 ? nr[(size_t)i * h->capR + q] : nr[(size_t)i * h->capR + na[(size_t)i * h->capA + q]];
+      if (ij_host && cnt < capacity) {
+        ij_host[2 * cnt] = i;
+        ij_host[2 * cnt + 1] = j;
+      }
+      ++cnt;
+    }
+  }
+  *n_pairs = cnt;
+  return NNP_OK;
+}
+
+static int export_rows(nnp_handle* h, const float* d_rows, float* host) {
+  if (!h || !host) return NNP_ERR_INVALID_ARG;
+  CK(cudaStreamSynchronize(h->last_stream));
+  std::vector<float> tmp((size_t)h->N * h->n_feat);
+  std::vector<int> sortpos(h->N);
+  if (h->N) {
+    CK(cudaMemcpy(tmp.data(), d_rows, tmp.size() * sizeof(float), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(sortpos.data(), h->d_sortpos, sortpos.size() * sizeof(int), cudaMemcpyDeviceToHost));
+  }
+  for (int i = 0; i < h->N; ++i)
+    memcpy(host + (size_t)i * h->n_feat, &tmp[(size_t)sortpos[i] * h->n_feat], sizeof(float) * h->n_feat);
+  return NNP_OK;
+}
+
+extern "C" int nnp_debug_aev(nnp_handle* h, float* aev_host) { return export_rows(h, h ? h->d_aev : nullptr, aev_host); }
+extern "C" int nnp_debug_daev(nnp_handle* h, float* g_host) { return export_rows(h, h ? h->d_daev : nullptr, g_host); }
+
+extern "C" int nnp_debug_atomic_energies(nnp_handle* h, double* e_host) {
+  if (!h || !e_host) return NNP_ERR_INVALID_ARG;
+  CK(cudaStreamSynchronize(h->last_stream));
+  std::vector<double> tmp((size_t)h->N * h->M);
+  std::vector<int> sortpos(h->N);
+  if (h->N) {
+    CK(cudaMemcpy(tmp.data(), h->d_eatom, tmp.size() * sizeof(double), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(sortpos.data(), h->d_sortpos, sortpos.size() * sizeof(int), cudaMemcpyDeviceToHost));
+  }
+  for (int i = 0; i < h->N; ++i)
+    for (int m = 0; m < h->M; ++m) e_host[(size_t)m * h->N + i] = tmp[(size_t)sortpos[i] * h->M + m];
+  return NNP_OK;
+}

@@ -1,0 +1,137 @@
+// Internal declarations of libnnp_b200 (CUDA, sm_100a).  Not part of the C ABI (include/nnp.h).
+// Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "nnp.h"
+
+#define NNP_MAX_SHF_R 32
+#define NNP_MAX_SHF_A 16
+#define NNP_MAX_SHF_Z 8
+#define NNP_MAX_SUB 64
+#define NNP_MAX_SPECIES 16
+#define NNP_MAX_LAYERS 8
+
+// device status bits (sticky)
+#define NNP_ST_CAPACITY 1
+#define NNP_ST_NONFINITE 2
+
+// AEV constants, passed by value to kernels.
+struct AevConst {
+  int S, n_shf_r, n_shf_a, n_shf_z, n_sub, n_radial, n_feat;
+  float rc_r, rc_a, eta_r, eta_a, zeta, cos_scale, length_scale;
+  double rc_r2, rc_a2;  // ((double)(float)Rc)^2, the O2 predicate thresholds
+  float shf_r[NNP_MAX_SHF_R];
+  float shf_a[NNP_MAX_SHF_A];
+  float cos_z[NNP_MAX_SHF_Z];  // cos(ShfZ_z), sin(ShfZ_z): cos(theta - ShfZ) = c cosZ + s sinZ
+  float sin_z[NNP_MAX_SHF_Z];
+};
+
+// One GEMM of a grouped launch: C[m][n] = epi( sum_k A[m][k] * Bop[k][n] ).
+struct GemmProblem {
+  const float* A;
+  const float* B;
+  float* C;
+  const float* bias;  // [N] or null (EPI_BIAS_CELU)
+  const float* aux;   // [M][ldaux] activations h for EPI_MUL_DCELU (may alias C)
+  int M, N, K;
+  int lda, ldb, ldc, ldaux;
+  int transB;  // 0: B is [N][K] (k contiguous, forward);  1: B is [K][N] (n contiguous, backward)
+  int epi;
+  float scale;
+  float alpha;  // CELU alpha
+};
+enum { EPI_BIAS_CELU = 0, EPI_MUL_DCELU = 1, EPI_SCALE = 2 };
+
+struct GemmTile {
+  int prob, m0, n0, cfg;
+};
+
+struct GemmLaunch {
+  GemmProblem* d_probs = nullptr;
+  GemmTile* d_tiles = nullptr;
+  int n_tiles = 0;
+  std::string name;
+  double flops = 0, weight_bytes = 0;
+};
+
+// Final layer (1 output) + start of the backward pass.
+struct LastLayerArgs {
+  float* act;          // [n_atoms_sorted][M][H] per element group (arena), overwritten with delta
+  const float* W;      // arena
+  const float* bias;   // arena
+  double* e_out;       // [n_sorted][M]
+  const int* grp_off;  // [S+1]
+  const long long* act_off;  // [S] float offset of the group's block in act
+  const long long* w_off;    // [S] float offset of W_L for (e, m=0); models contiguous with stride H
+  const long long* b_off;    // [S]
+  const int* H;        // [S]
+  int S, M, n_sorted;
+  float alpha;
+};
+
+struct nnp_handle {
+  int device = 0;
+  int N = 0, n_mol = 0, S = 0, M = 0, L = 0, n_feat = 0;
+  int capR = 0, capA = 0;
+  int flags = 0;
+  double energy_scale = 1.0, length_scale = 1.0;
+  AevConst aev;
+  std::vector<int> dims;     // [S][L+1]
+  std::vector<int> grp_off;  // [S+1] host
+  // device: topology
+  int *d_species = nullptr, *d_mol_off = nullptr, *d_mol_id = nullptr, *d_sortpos = nullptr, *d_perm = nullptr,
+      *d_grp_off = nullptr;
+  double* d_self_energy = nullptr;
+  // device: per-step workspace
+  float4* d_pos4 = nullptr;
+  int *d_nbr_r = nullptr, *d_nbr_a = nullptr, *d_cnt_r = nullptr, *d_cnt_a = nullptr;
+  float* d_aev = nullptr;   // [N sorted][n_feat]
+  float* d_daev = nullptr;  // [N sorted][n_feat]
+  float* d_phi = nullptr;   // [N][capR][3]
+  double* d_eatom = nullptr;  // [N sorted][M]
+  int* d_status = nullptr;
+  // weights
+  float *d_W = nullptr, *d_b = nullptr;
+  std::vector<long long> w_off, b_off;  // [S][L] float offsets of the (e,l) block, models contiguous
+  size_t w_floats = 0, b_floats = 0;
+  // activations: act[l] for l = 1..L-1
+  float* d_act[NNP_MAX_LAYERS] = {nullptr};
+  std::vector<long long> act_off[NNP_MAX_LAYERS];  // [S] float offsets
+  // MLP launches
+  std::vector<GemmLaunch> fwd, bwd;  // fwd: layers 1..L-1; bwd: layers L-1..1
+  LastLayerArgs last;
+  long long *d_last_act_off = nullptr, *d_last_w_off = nullptr, *d_last_b_off = nullptr;
+  int* d_last_H = nullptr;
+  // host staging for nnp_compute_host
+  float *d_hpos = nullptr, *d_hforce = nullptr;
+  double* d_henergy = nullptr;
+  // graph
+  cudaGraphExec_t graph_exec = nullptr;
+  const void* g_pos = nullptr;
+  const void* g_idx = nullptr;
+  void *g_energy = nullptr, *g_force = nullptr;
+  int g_ps = 0, g_fs = 0;
+  cudaStream_t last_stream = nullptr;
+  // profiling
+  bool profiling = false;
+  std::vector<cudaEvent_t> events;
+  std::vector<std::string> stage_names;
+  int n_launches = 0;
+  double work[4] = {0, 0, 0, 0};
+};
+
+// kernels (launch wrappers)
+void launch_neighbors(nnp_handle* h, const float* d_pos, int pos_stride, const int* d_atom_index, cudaStream_t s);
+void launch_aev_forward(nnp_handle* h, cudaStream_t s);
+void launch_aev_backward(nnp_handle* h, cudaStream_t s);
+void launch_gemm(const GemmLaunch& g, cudaStream_t s);
+void launch_last_layer(nnp_handle* h, cudaStream_t s);
+void launch_finish(nnp_handle* h, const int* d_atom_index, double* d_energy, float* d_force, int force_stride,
+                   cudaStream_t s);
+size_t aev_smem_bytes(const nnp_handle* h, bool backward);
+void build_gemm_tiles(const std::vector<GemmProblem>& probs, std::vector<GemmTile>& tiles);
