@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(128) nbr_allpairs_kernel(
     if (in_r && slot_r < capR) nbr_r[(size_t)i * capR + slot_r] = j;
     if (in_a) {
       const int slot_a = na + __popc(ba & below);
-      if (slot_a < capA) nbr_a[(size_t)i * capA + slot_a] = slot_r;
+      if (slot_a < capA && slot_r < capR) nbr_a[(size_t)i * capA + slot_a] = slot_r;
     }
     nr += __popc(br);
     na += __popc(ba);
@@ -79,8 +79,10 @@ __device__ __forceinline__ int pair_index(int s, int t, int S) {
 
 // per angular neighbour, 8 floats in shared memory
 struct PairData {
-  float ux, uy, uz, r, fc, dfc;
-  int spec, slot;
+  float ux, uy, uz, r, rlo, fc, dfc;  // r + rlo = the FP64 distance to ~2^-48
+  int ss;                             // slot * 16 + species
+  __device__ __forceinline__ int spec() const { return ss & 15; }
+  __device__ __forceinline__ int slot() const { return ss >> 4; }
 };
 
 // geometry of a directed pair in FP64 from the f32 coordinates (cheap on B200, removes the
@@ -97,9 +99,18 @@ __device__ __forceinline__ void pair_geometry(const float4 pi, const float4 pj, 
   uz = (float)(dz * inv);
 }
 
-__device__ __forceinline__ float cutoff_f(float r, float rc) { return 0.5f * cosf(CUDART_PI_F * r / rc) + 0.5f; }
+// O1: f_C = 0.5 cos(pi r/Rc) + 0.5 = cos^2(pi r / 2Rc) (the squared form keeps relative accuracy near Rc);
+//     f_C' = -(pi/2Rc) sin(pi r/Rc) = -(pi/Rc) sin(pi r/2Rc) cos(pi r/2Rc)
+// cospif/sincospif take the argument in units of pi, so no rounded pi enters the argument (a rounded
+// pi biases every f_C by ~ -5e-8 relative, which adds up coherently over the whole AEV).
+__device__ __forceinline__ float cutoff_f(float r, float rc) {
+  const float ch = cospif(0.5f * r / rc);
+  return ch * ch;
+}
 __device__ __forceinline__ float dcutoff_f(float r, float rc) {
-  return -(CUDART_PI_F / (2.0f * rc)) * sinf(CUDART_PI_F * r / rc);
+  float sh, ch;
+  sincospif(0.5f * r / rc, &sh, &ch);
+  return -(CUDART_PI_F / rc) * sh * ch;
 }
 
 size_t aev_smem_bytes(const nnp_handle* h, bool backward) {
@@ -122,10 +133,10 @@ __device__ __forceinline__ void load_pair_data(PairData* pd, int na, int i, cons
     PairData d;
     pair_geometry(pi, pj, r, d.ux, d.uy, d.uz);
     d.r = (float)r;
+    d.rlo = (float)(r - (double)d.r);
     d.fc = cutoff_f(d.r, rc_a);
     d.dfc = dcutoff_f(d.r, rc_a);
-    d.spec = __float_as_int(pj.w);
-    d.slot = slot;
+    d.ss = slot * 16 + __float_as_int(pj.w);
     pd[q] = d;
   }
 }
@@ -183,6 +194,7 @@ __global__ void __launch_bounds__(AEV_WARPS * 32) aev_forward_kernel(
   for (int t = lane; t < c.n_sub; t += 32) {
     const int ia = t / c.n_shf_z, iz = t % c.n_shf_z;
     const float shfa = c.shf_a[ia], cz = c.cos_z[iz], sz = c.sin_z[iz];
+    const float czl = c.cos_z_lo[iz], szl = c.sin_z_lo[iz];
     for (int a = 0; a < na; ++a) {
       const PairData A = pd[a];
       for (int b = a + 1; b < na; ++b) {
@@ -190,12 +202,12 @@ __global__ void __launch_bounds__(AEV_WARPS * 32) aev_forward_kernel(
         const float cth = A.ux * B.ux + A.uy * B.uy + A.uz * B.uz;
         const float cc = c.cos_scale * cth;
         const float ss = sqrtf(fmaxf(1.0f - cc * cc, 0.0f));
-        const float u = 0.5f + 0.5f * (cc * cz + ss * sz);
+        const float u = 0.5f + 0.5f * ((cc * cz + ss * sz) + (cc * czl + ss * szl));
         const float F1 = exp2f(c.zeta * log2f(u));
-        const float d = 0.5f * (A.r + B.r) - shfa;
+        const float d = 0.5f * (((A.r - shfa) + (B.r - shfa)) + (A.rlo + B.rlo));
         const float F2 = expf(-c.eta_a * d * d);
         const float val = 2.0f * F1 * F2 * (A.fc * B.fc);
-        ang[pair_index(A.spec, B.spec, c.S) * c.n_sub + t] += val;
+        ang[pair_index(A.spec(), B.spec(), c.S) * c.n_sub + t] += val;
       }
     }
   }
@@ -276,17 +288,16 @@ __global__ void __launch_bounds__(AEV_WARPS * 32) aev_backward_kernel(
       const float cc = c.cos_scale * cth;
       const float ss = sqrtf(fmaxf(1.0f - cc * cc, 0.0f));
       const float cot = cc / ss;
-      const float rbar = 0.5f * (A.r + B.r);
-      const float* gb = gang + pair_index(A.spec, B.spec, c.S) * c.n_sub;
+      const float* gb = gang + pair_index(A.spec(), B.spec(), c.S) * c.n_sub;
       float R0 = 0.f, R1 = 0.f, R2 = 0.f;
       for (int t = lane; t < c.n_sub; t += 32) {
         const int ia = t / c.n_shf_z, iz = t % c.n_shf_z;
-        const float cz = c.cos_z[iz], sz = c.sin_z[iz];
-        const float u = 0.5f + 0.5f * (cc * cz + ss * sz);
+        const float cz = c.cos_z[iz], sz = c.sin_z[iz], shfa = c.shf_a[ia];
+        const float u = 0.5f + 0.5f * ((cc * cz + ss * sz) + (cc * c.cos_z_lo[iz] + ss * c.sin_z_lo[iz]));
         const float pw1 = exp2f((c.zeta - 1.0f) * log2f(u));  // u^(zeta-1)
         const float F1 = pw1 * u;
         const float dF1dc = c.zeta * pw1 * 0.5f * (cz - cot * sz);
-        const float d = rbar - c.shf_a[ia];
+        const float d = 0.5f * (((A.r - shfa) + (B.r - shfa)) + (A.rlo + B.rlo));
         const float F2 = expf(-c.eta_a * d * d);
         const float gt = gb[t];
         R0 += gt * F1 * F2;
@@ -303,8 +314,8 @@ __global__ void __launch_bounds__(AEV_WARPS * 32) aev_backward_kernel(
         const float coefC = 2.0f * W * R2 * c.cos_scale;
         const float ua = lane == 0 ? A.ux : (lane == 1 ? A.uy : A.uz);
         const float ub = lane == 0 ? B.ux : (lane == 1 ? B.uy : B.uz);
-        ph[3 * A.slot + lane] += coefA * ua + coefC * (ub - cth * ua) / A.r;
-        ph[3 * B.slot + lane] += coefB * ub + coefC * (ua - cth * ub) / B.r;
+        ph[3 * A.slot() + lane] += coefA * ua + coefC * (ub - cth * ua) / A.r;
+        ph[3 * B.slot() + lane] += coefB * ub + coefC * (ua - cth * ub) / B.r;
       }
       __syncwarp();
     }

@@ -106,6 +106,13 @@ __device__ __forceinline__ void gemm_tile(const GemmProblem& p, int m0, int n0, 
   for (int kt = 0; kt < nk; ++kt) {
     const int buf = kt & 1;
     if (kt + 1 < nk) load_global((kt + 1) * BK);
+    // two-level accumulation: a fresh partial sum per k-tile, added to the running total once.  The
+    // rounding error of a 1008-long FP32 dot product then grows with sqrt(K/BK), not sqrt(K).
+    float part[TM][TN];
+#pragma unroll
+    for (int i = 0; i < TM; ++i)
+#pragma unroll
+      for (int j = 0; j < TN; ++j) part[i][j] = 0.0f;
 #pragma unroll
     for (int kk = 0; kk < BK; ++kk) {
       float a[TM], b[TN];
@@ -119,8 +126,12 @@ __device__ __forceinline__ void gemm_tile(const GemmProblem& p, int m0, int n0, 
 #pragma unroll
       for (int i = 0; i < TM; ++i)
 #pragma unroll
-        for (int j = 0; j < TN; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+        for (int j = 0; j < TN; ++j) part[i][j] = fmaf(a[i], b[j], part[i][j]);
     }
+#pragma unroll
+    for (int i = 0; i < TM; ++i)
+#pragma unroll
+      for (int j = 0; j < TN; ++j) acc[i][j] += part[i][j];
     if (kt + 1 < nk) {
       store_smem(buf ^ 1);
       __syncthreads();

@@ -144,8 +144,11 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   for (int k = 0; k < cfg->n_shf_r; ++k) a.shf_r[k] = cfg->shf_r[k];
   for (int k = 0; k < cfg->n_shf_a; ++k) a.shf_a[k] = cfg->shf_a[k];
   for (int k = 0; k < cfg->n_shf_z; ++k) {
-    a.cos_z[k] = (float)cos((double)cfg->shf_z[k]);
-    a.sin_z[k] = (float)sin((double)cfg->shf_z[k]);
+    const double cz = cos((double)cfg->shf_z[k]), sz = sin((double)cfg->shf_z[k]);
+    a.cos_z[k] = (float)cz;
+    a.sin_z[k] = (float)sz;
+    a.cos_z_lo[k] = (float)(cz - (double)a.cos_z[k]);
+    a.sin_z_lo[k] = (float)(sz - (double)a.sin_z[k]);
   }
 
   // ---- A0: group atoms by element (stable), molecule ids, capacities
@@ -171,7 +174,6 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   h->capA = cfg->max_angular_neighbors > 0 ? cfg->max_angular_neighbors : std::min(std::max(max_mol - 1, 1), 128);
   if (h->capA > h->capR) h->capA = h->capR;
 
-  int rc = NNP_OK;
   auto fail = [&](int code) {
     nnp_destroy(h);
     return code;
@@ -368,7 +370,6 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   for (auto& e : h->events)
     if (cudaEventCreate(&e) != cudaSuccess) return fail(NNP_ERR_CUDA);
   if (cudaDeviceSynchronize() != cudaSuccess) return fail(NNP_ERR_CUDA);
-  (void)rc;
   *out = h;
   return NNP_OK;
 }

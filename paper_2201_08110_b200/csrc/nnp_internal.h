@@ -29,6 +29,8 @@ struct AevConst {
   float shf_a[NNP_MAX_SHF_A];
   float cos_z[NNP_MAX_SHF_Z];  // cos(ShfZ_z), sin(ShfZ_z): cos(theta - ShfZ) = c cosZ + s sinZ
   float sin_z[NNP_MAX_SHF_Z];
+  float cos_z_lo[NNP_MAX_SHF_Z];  // low parts: cos_z + cos_z_lo = cos(ShfZ) to ~2^-48 (a rounded constant
+  float sin_z_lo[NNP_MAX_SHF_Z];  // is a coherent error amplified by zeta)
 };
 
 // One GEMM of a grouped launch: C[m][n] = epi( sum_k A[m][k] * Bop[k][n] ).

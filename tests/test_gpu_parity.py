@@ -65,8 +65,8 @@ def check_stages(gpu, ref, orc, pos, mol_offsets):
         got = set(map(tuple, gpu[key].tolist()))
         assert len(got) == len(gpu[key]), "duplicate directed pairs"
         assert got == want, f"{which} pair set differs: {len(got)} vs {len(want)}"
-    assert np.abs(gpu["G"] - ref["G"]).max() <= AEV_TOL
-    assert np.array_equal(gpu["G"] == 0.0, ref["G"] == 0.0) or np.abs(ref["G"][gpu["G"] == 0.0]).max() < 1e-30
+    assert np.abs(gpu["G"] - ref["G"]).max() <= AEV_TOL * max(1.0, np.abs(ref["G"]).max())
+    assert np.all(gpu["G"][ref["G"] == 0.0] == 0.0)  # structural zeros (absent species / pairs) stay exact
     e_scale = max(1.0, np.abs(ref["e_atom"]).max())
     assert np.abs(gpu["e_atom"] - ref["e_atom"]).max() <= 5e-7 * e_scale
     assert np.abs(gpu["dG"] - ref["dG"]).max() <= DAEV_TOL
