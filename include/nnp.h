@@ -77,6 +77,7 @@ typedef struct {
 } nnp_config;
 
 #define NNP_FLAG_NO_GRAPH 1 /* launch kernels one by one instead of replaying a CUDA graph */
+#define NNP_FLAG_NO_TMA 2   /* run the MLP layers on the plain (non-TMA) grouped FFMA kernel */
 
 /*
  * nnp_create: build a handle for a fixed set of atoms.

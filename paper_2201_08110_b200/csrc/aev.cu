@@ -77,147 +77,212 @@ __device__ __forceinline__ int pair_index(int s, int t, int S) {
   return a * S - (a * (a - 1)) / 2 + (b - a);
 }
 
-// per angular neighbour, 8 floats in shared memory
-struct PairData {
-  float ux, uy, uz, r, rlo, fc, dfc;  // r + rlo = the FP64 distance to ~2^-48
-  int ss;                             // slot * 16 + species
-  __device__ __forceinline__ int spec() const { return ss & 15; }
-  __device__ __forceinline__ int slot() const { return ss >> 4; }
-};
-
-// geometry of a directed pair in FP64 from the f32 coordinates (cheap on B200, removes the
-// cancellation error of an f32 distance); results rounded to f32 once.
-__device__ __forceinline__ void pair_geometry(const float4 pi, const float4 pj, double& r, float& ux, float& uy,
-                                              float& uz) {
-  const double dx = (double)pj.x - (double)pi.x;
-  const double dy = (double)pj.y - (double)pi.y;
-  const double dz = (double)pj.z - (double)pi.z;
-  r = sqrt(dx * dx + dy * dy + dz * dz);
-  const double inv = 1.0 / r;
-  ux = (float)(dx * inv);
-  uy = (float)(dy * inv);
-  uz = (float)(dz * inv);
+// ------------------------------------------------------------------------------------------------
+// fast-math building blocks.  Accuracy notes:
+//  - u^zeta = u^floor(zeta) (exact-ish repeated squaring) * 2^(frac * lg2 u): the MUFU lg2 error
+//    (2^-22 absolute) is scaled by frac (0.1), not by zeta (14.1);
+//  - exp(-eta d^2) = ex2(d^2 * k), k = -eta*log2(e) carried as hi+lo so the constant is not a bias;
+//  - geometry (r, unit vectors) is FP64 once per directed pair, r is kept as hi+lo floats.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float lg2_approx(float x) {
+  float y;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float sqrt_approx(float x) {
+  float y;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+// u^(n + frac), n >= 0 uniform across the grid, 0 <= frac < 1, u in [0, 1]
+__device__ __forceinline__ float pow_split(float u, int n, float frac) {
+  float r = 1.0f, b = u;
+#pragma unroll
+  for (int bit = 0; bit < 6; ++bit) {
+    if (n & 1) r *= b;
+    b *= b;
+    n >>= 1;
+  }
+  if (frac != 0.0f) r *= ex2_approx(frac * lg2_approx(u));
+  return r;
+}
+__device__ __forceinline__ float gauss(float d, float khi, float klo) {
+  const float d2 = d * d;
+  return ex2_approx(fmaf(d2, klo, d2 * khi));
 }
 
-// O1: f_C = 0.5 cos(pi r/Rc) + 0.5 = cos^2(pi r / 2Rc) (the squared form keeps relative accuracy near Rc);
-//     f_C' = -(pi/2Rc) sin(pi r/Rc) = -(pi/Rc) sin(pi r/2Rc) cos(pi r/2Rc)
-// cospif/sincospif take the argument in units of pi, so no rounded pi enters the argument (a rounded
-// pi biases every f_C by ~ -5e-8 relative, which adds up coherently over the whole AEV).
-__device__ __forceinline__ float cutoff_f(float r, float rc) {
-  const float ch = cospif(0.5f * r / rc);
-  return ch * ch;
-}
-__device__ __forceinline__ float dcutoff_f(float r, float rc) {
-  float sh, ch;
-  sincospif(0.5f * r / rc, &sh, &ch);
-  return -(CUDART_PI_F / rc) * sh * ch;
-}
+constexpr int TAB_FIELDS = 10;  // per radial slot: ux uy uz rhi rlo fcr dfcr fca dfca spec
 
 size_t aev_smem_bytes(const nnp_handle* h, bool backward) {
-  size_t per_warp = (size_t)h->n_feat + (backward ? 3 * (size_t)h->capR : (size_t)h->aev.n_radial) +
-                    8 * (size_t)h->capA;
-  per_warp = (per_warp + 3) & ~(size_t)3;
-  return per_warp * 4 * AEV_WARPS;
+  size_t fl = (size_t)TAB_FIELDS * h->capR + h->capA;
+  if (!backward) fl += (size_t)AEV_WARPS * (h->n_feat - h->aev.n_radial);
+  else fl += (size_t)h->n_feat + (size_t)(AEV_WARPS + 1) * 3 * h->capR;
+  return ((fl + 3) & ~(size_t)3) * 4;
 }
 
-// fills the per-warp PairData table for centre i; returns nothing (na entries)
-__device__ __forceinline__ void load_pair_data(PairData* pd, int na, int i, const float4 pi,
-                                               const float4* __restrict__ pos4, const int* __restrict__ nbr_r,
-                                               const int* __restrict__ nbr_a, int capR, int capA, float rc_a,
-                                               int lane) {
-  for (int q = lane; q < na; q += 32) {
-    const int slot = nbr_a[(size_t)i * capA + q];
-    const int j = nbr_r[(size_t)i * capR + slot];
+struct CentreTab {
+  float *ux, *uy, *uz, *rhi, *rlo, *fcr, *dfcr, *fca, *dfca;
+  int* spec;
+  int* asl;  // angular neighbours: radial slots, sorted by species (stable)
+};
+
+__device__ __forceinline__ CentreTab carve_tab(float* smem, int capR) {
+  CentreTab t;
+  t.ux = smem; t.uy = t.ux + capR; t.uz = t.uy + capR; t.rhi = t.uz + capR; t.rlo = t.rhi + capR;
+  t.fcr = t.rlo + capR; t.dfcr = t.fcr + capR; t.fca = t.dfcr + capR; t.dfca = t.fca + capR;
+  t.spec = reinterpret_cast<int*>(t.dfca + capR);
+  t.asl = t.spec + capR;
+  return t;
+}
+
+// Phase 0 of both AEV kernels: geometry of every radial neighbour of centre i (FP64 once, all threads
+// of the CTA in parallel), and the angular neighbour list re-ordered by species so that consecutive
+// triplets of a warp fall into the same feature block.
+__device__ __forceinline__ void build_tab(const CentreTab& t, int i, int nr, int na, const float4 pi,
+                                          const float4* __restrict__ pos4, const int* __restrict__ nbr_r,
+                                          const int* __restrict__ nbr_a, int capR, int capA, const AevConst& c) {
+  for (int q = threadIdx.x; q < nr; q += blockDim.x) {
+    const int j = nbr_r[(size_t)i * capR + q];
     const float4 pj = pos4[j];
-    double r;
-    PairData d;
-    pair_geometry(pi, pj, r, d.ux, d.uy, d.uz);
-    d.r = (float)r;
-    d.rlo = (float)(r - (double)d.r);
-    d.fc = cutoff_f(d.r, rc_a);
-    d.dfc = dcutoff_f(d.r, rc_a);
-    d.ss = slot * 16 + __float_as_int(pj.w);
-    pd[q] = d;
+    const double dx = (double)pj.x - (double)pi.x;
+    const double dy = (double)pj.y - (double)pi.y;
+    const double dz = (double)pj.z - (double)pi.z;
+    const double r = sqrt(dx * dx + dy * dy + dz * dz);
+    const double inv = 1.0 / r;
+    t.ux[q] = (float)(dx * inv);
+    t.uy[q] = (float)(dy * inv);
+    t.uz[q] = (float)(dz * inv);
+    const float rf = (float)r;
+    t.rhi[q] = rf;
+    t.rlo[q] = (float)(r - (double)rf);
+    // O1 via cospi: f_C = cos^2(pi r / 2Rc), f_C' = -(pi/Rc) sin cos; no rounded pi in the argument
+    float sh, ch;
+    sincospif(0.5f * rf / c.rc_r, &sh, &ch);
+    t.fcr[q] = ch * ch;
+    t.dfcr[q] = -(CUDART_PI_F / c.rc_r) * sh * ch;
+    sincospif(0.5f * rf / c.rc_a, &sh, &ch);
+    t.fca[q] = ch * ch;
+    t.dfca[q] = -(CUDART_PI_F / c.rc_a) * sh * ch;
+    t.spec[q] = __float_as_int(pj.w);
+  }
+  __syncthreads();
+  // stable counting sort of the angular list by species: rank = #(smaller species) + #(same, earlier)
+  for (int q = threadIdx.x; q < na; q += blockDim.x) {
+    const int slot = nbr_a[(size_t)i * capA + q];
+    const int sp = t.spec[slot];
+    int rank = 0;
+    for (int q2 = 0; q2 < na; ++q2) {
+      const int s2 = t.spec[nbr_a[(size_t)i * capA + q2]];
+      rank += (s2 < sp) || (s2 == sp && q2 < q);
+    }
+    t.asl[rank] = slot;
+  }
+  __syncthreads();
+}
+
+// first triplet (a,b), a<b<na, of warp w in the flattened order, and the step to the next one
+__device__ __forceinline__ void trip_norm(int& a, int& b, int na) {
+  while (a < na - 1 && b >= na) {
+    ++a;
+    b = b - na + a + 1;
   }
 }
 
 // ------------------------------------------------------------------------------------------------
-// A2 + A3: AEV forward, warp per centre.
+// A2 + A3: AEV forward.  One CTA (4 warps) per centre.
+//   radial : one thread per output column (species s, shift k) loops over the neighbours of species s
+//            and keeps the sum in a register (fixed order, no shared-memory updates);
+//   angular: the triplets are dealt round-robin to the 4 warps; lanes are the (ShfA, ShfZ) sub-terms;
+//            each warp sums runs of triplets that fall into the same species-pair block in a register
+//            and flushes to its own partial row; the 4 partial rows are added in a fixed order.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(AEV_WARPS * 32) aev_forward_kernel(
     const float4* __restrict__ pos4, const int* __restrict__ nbr_r, const int* __restrict__ nbr_a,
     const int* __restrict__ cnt_r, const int* __restrict__ cnt_a, const int* __restrict__ sortpos, int N,
-    AevConst c, int capR, int capA, float* __restrict__ aev) {
+    const __grid_constant__ AevConst c, int capR, int capA, float* __restrict__ aev) {
   extern __shared__ __align__(16) float smem[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int i = blockIdx.x * AEV_WARPS + warp;
-  if (i >= N) return;
-  size_t per_warp = ((size_t)c.n_feat + c.n_radial + 8 * (size_t)capA + 3) & ~(size_t)3;
-  float* row = smem + per_warp * warp;
-  float* rad1 = row + c.n_feat;
-  PairData* pd = reinterpret_cast<PairData*>(rad1 + c.n_radial);
-
-  for (int f = lane; f < c.n_feat + c.n_radial; f += 32) row[f] = 0.0f;
+  const int i = blockIdx.x;
+  const CentreTab t = carve_tab(smem, capR);
+  const int n_ang = c.n_feat - c.n_radial;
+  float* rows = reinterpret_cast<float*>(t.asl + capA);  // [AEV_WARPS][n_ang]
   const float4 pi = pos4[i];
   const int nr = cnt_r[i], na = cnt_a[i];
-  load_pair_data(pd, na, i, pi, pos4, nbr_r, nbr_a, capR, capA, c.rc_a, lane);
-  __syncwarp();
+  for (int f = threadIdx.x; f < AEV_WARPS * n_ang; f += blockDim.x) rows[f] = 0.0f;
+  build_tab(t, i, nr, na, pi, pos4, nbr_r, nbr_a, capR, capA, c);
+  float* out = aev + (size_t)sortpos[i] * c.n_feat;
 
-  // ---- radial (O3): two neighbours per pass when n_shf_r <= 16 (one per half-warp, own partial row)
-  {
-    const int groups = c.n_shf_r <= 16 ? 2 : 1;
-    const int glanes = 32 / groups;
-    const int grp = lane / glanes, k = lane % glanes;
-    float* dst = grp ? rad1 : row;
-    for (int s0 = 0; s0 < nr; s0 += groups) {
-      const int s = s0 + grp;
-      if (s < nr && k < c.n_shf_r) {
-        const int j = nbr_r[(size_t)i * capR + s];
-        const float4 pj = pos4[j];
-        double r;
-        float ux, uy, uz;
-        pair_geometry(pi, pj, r, ux, uy, uz);
-        const float fc = cutoff_f((float)r, c.rc_r);
-        const float d = (float)(r - (double)c.shf_r[k]);
-        const float val = 0.25f * expf(-c.eta_r * d * d) * fc;
-        dst[__float_as_int(pj.w) * c.n_shf_r + k] += val;
-      }
-      __syncwarp();
+  // ---- radial (O3)
+  for (int col = threadIdx.x; col < c.n_radial; col += blockDim.x) {
+    const int s = col / c.n_shf_r, k = col % c.n_shf_r;
+    const float shf = c.shf_r[k];
+    float acc = 0.0f;
+    for (int q = 0; q < nr; ++q) {
+      if (t.spec[q] != s) continue;
+      const float d = (t.rhi[q] - shf) + t.rlo[q];
+      acc += 0.25f * gauss(d, c.kr_hi, c.kr_lo) * t.fcr[q];
     }
-    if (groups == 2)
-      for (int f = lane; f < c.n_radial; f += 32) row[f] += rad1[f];
-    __syncwarp();
+    out[col] = acc;
   }
 
-  // ---- angular (O4): lanes are the (ShfA, ShfZ) sub-terms; triplets are visited serially
-  float* ang = row + c.n_radial;
-  for (int t = lane; t < c.n_sub; t += 32) {
-    const int ia = t / c.n_shf_z, iz = t % c.n_shf_z;
+  // ---- angular (O4)
+  float* myrow = rows + warp * n_ang;
+  const int nsub_it = (c.n_sub + 31) >> 5;
+  for (int it = 0; it < nsub_it; ++it) {
+    const int tt = lane + 32 * it;
+    const bool live = tt < c.n_sub;
+    const int ia = live ? tt / c.n_shf_z : 0, iz = live ? tt % c.n_shf_z : 0;
     const float shfa = c.shf_a[ia], cz = c.cos_z[iz], sz = c.sin_z[iz];
     const float czl = c.cos_z_lo[iz], szl = c.sin_z_lo[iz];
-    for (int a = 0; a < na; ++a) {
-      const PairData A = pd[a];
-      for (int b = a + 1; b < na; ++b) {
-        const PairData B = pd[b];
-        const float cth = A.ux * B.ux + A.uy * B.uy + A.uz * B.uz;
-        const float cc = c.cos_scale * cth;
-        const float ss = sqrtf(fmaxf(1.0f - cc * cc, 0.0f));
-        const float u = 0.5f + 0.5f * ((cc * cz + ss * sz) + (cc * czl + ss * szl));
-        const float F1 = exp2f(c.zeta * log2f(u));
-        const float d = 0.5f * (((A.r - shfa) + (B.r - shfa)) + (A.rlo + B.rlo));
-        const float F2 = expf(-c.eta_a * d * d);
-        const float val = 2.0f * F1 * F2 * (A.fc * B.fc);
-        ang[pair_index(A.spec(), B.spec(), c.S) * c.n_sub + t] += val;
+    int a = 0, b = 1 + warp;
+    trip_norm(a, b, na);
+    int cur_p = -1;
+    float acc = 0.0f;
+    while (a < na - 1) {
+      const int qa = t.asl[a], qb = t.asl[b];
+      const float cth = t.ux[qa] * t.ux[qb] + t.uy[qa] * t.uy[qb] + t.uz[qa] * t.uz[qb];
+      const float cc = c.cos_scale * cth;
+      const float ss = sqrt_approx(fmaxf(fmaf(-cc, cc, 1.0f), 0.0f));
+      const float u = 0.5f + 0.5f * ((cc * cz + ss * sz) + (cc * czl + ss * szl));
+      const float F1 = pow_split(u, c.zeta_int, c.zeta_frac);
+      const float d = 0.5f * (((t.rhi[qa] - shfa) + (t.rhi[qb] - shfa)) + (t.rlo[qa] + t.rlo[qb]));
+      const float F2 = gauss(d, c.ka_hi, c.ka_lo);
+      const float val = 2.0f * F1 * F2 * (t.fca[qa] * t.fca[qb]);
+      const int sa = t.spec[qa], sb = t.spec[qb];  // sa <= sb (sorted)
+      const int p = sa * c.S - (sa * (sa - 1)) / 2 + (sb - sa);
+      if (p != cur_p) {
+        if (cur_p >= 0 && live) myrow[cur_p * c.n_sub + tt] += acc;
+        cur_p = p;
+        acc = 0.0f;
       }
+      acc += val;
+      b += AEV_WARPS;
+      trip_norm(a, b, na);
     }
+    if (cur_p >= 0 && live) myrow[cur_p * c.n_sub + tt] += acc;
   }
-  __syncwarp();
-  float* out = aev + (size_t)sortpos[i] * c.n_feat;
-  for (int f = lane; f < c.n_feat; f += 32) out[f] = row[f];
+  __syncthreads();
+  for (int f = threadIdx.x; f < n_ang; f += blockDim.x) {
+    float v = rows[f];
+#pragma unroll
+    for (int w = 1; w < AEV_WARPS; ++w) v += rows[w * n_ang + f];
+    out[c.n_radial + f] = v;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
-// A7: AEV backward, warp per centre.  phi[i][slot] = dE/d(r_j - r_i) for every radial slot of i.
+// A7: AEV backward.  One CTA (4 warps) per centre.  phi[i][slot] = dE/d(r_j - r_i) for every radial
+// slot of i (pair-gradient formulation: no atomics, the force gather happens per atom afterwards).
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
@@ -228,78 +293,79 @@ __device__ __forceinline__ float warp_sum(float v) {
 __global__ void __launch_bounds__(AEV_WARPS * 32) aev_backward_kernel(
     const float4* __restrict__ pos4, const int* __restrict__ nbr_r, const int* __restrict__ nbr_a,
     const int* __restrict__ cnt_r, const int* __restrict__ cnt_a, const int* __restrict__ sortpos, int N,
-    AevConst c, int capR, int capA, const float* __restrict__ daev, float* __restrict__ phi) {
+    const __grid_constant__ AevConst c, int capR, int capA, const float* __restrict__ daev, int n_parts,
+    size_t part_stride, float* __restrict__ phi) {
   extern __shared__ __align__(16) float smem[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int i = blockIdx.x * AEV_WARPS + warp;
-  if (i >= N) return;
-  size_t per_warp = ((size_t)c.n_feat + 3 * (size_t)capR + 8 * (size_t)capA + 3) & ~(size_t)3;
-  float* g = smem + per_warp * warp;
-  float* ph = g + c.n_feat;  // [capR][3]
-  PairData* pd = reinterpret_cast<PairData*>(ph + 3 * capR);
-
-  const float* gin = daev + (size_t)sortpos[i] * c.n_feat;
-  for (int f = lane; f < c.n_feat; f += 32) g[f] = gin[f];
+  const int i = blockIdx.x;
+  const CentreTab t = carve_tab(smem, capR);
+  float* g = reinterpret_cast<float*>(t.asl + capA);  // [n_feat]
+  float* phr = g + c.n_feat;                          // radial part           [capR][3]
+  float* phw = phr + 3 * capR;                        // per-warp angular part [AEV_WARPS][capR][3]
   const float4 pi = pos4[i];
   const int nr = cnt_r[i], na = cnt_a[i];
-  load_pair_data(pd, na, i, pi, pos4, nbr_r, nbr_a, capR, capA, c.rc_a, lane);
-  __syncwarp();
+  const float* gin = daev + (size_t)sortpos[i] * c.n_feat;
+  for (int f = threadIdx.x; f < c.n_feat; f += blockDim.x) {
+    float v = gin[f];
+    for (int p = 1; p < n_parts; ++p) v += gin[(size_t)p * part_stride + f];  // fixed order
+    g[f] = v;
+  }
+  for (int f = threadIdx.x; f < AEV_WARPS * 3 * nr; f += blockDim.x) phw[(f / (3 * nr)) * 3 * capR + f % (3 * nr)] = 0.0f;
+  build_tab(t, i, nr, na, pi, pos4, nbr_r, nbr_a, capR, capA, c);
 
-  // ---- radial: dT/dr = T (-2 eta (r - Shf)) + 0.25 exp(.) fC'(r)
+  // ---- radial: dT/dr = 0.25 e (f_C' - 2 eta (r - Shf) f_C); a group of lanes per neighbour
   {
-    const int groups = c.n_shf_r <= 16 ? 2 : 1;
-    const int glanes = 32 / groups;
-    const int grp = lane / glanes, k = lane % glanes;
-    for (int s0 = 0; s0 < nr; s0 += groups) {
-      const int s = s0 + grp;
-      float v = 0.0f, ux = 0.f, uy = 0.f, uz = 0.f;
-      if (s < nr) {
-        const int j = nbr_r[(size_t)i * capR + s];
-        const float4 pj = pos4[j];
-        double r;
-        pair_geometry(pi, pj, r, ux, uy, uz);
-        if (k < c.n_shf_r) {
-          const float rf = (float)r;
-          const float fc = cutoff_f(rf, c.rc_r), dfc = dcutoff_f(rf, c.rc_r);
-          const float d = (float)(r - (double)c.shf_r[k]);
-          const float ex = 0.25f * expf(-c.eta_r * d * d);
-          const float dT = ex * (dfc - 2.0f * c.eta_r * d * fc);
-          v = g[__float_as_int(pj.w) * c.n_shf_r + k] * dT;
-        }
+    const int glanes = c.n_shf_r <= 16 ? 16 : 32;
+    const int groups = blockDim.x / glanes;
+    const int grp = threadIdx.x / glanes, k = threadIdx.x % glanes;
+    for (int q0 = 0; q0 < nr; q0 += groups) {
+      const int q = q0 + grp;
+      float v = 0.0f;
+      if (q < nr && k < c.n_shf_r) {
+        const float d = (t.rhi[q] - c.shf_r[k]) + t.rlo[q];
+        const float ex = 0.25f * gauss(d, c.kr_hi, c.kr_lo);
+        const float dT = ex * (t.dfcr[q] - 2.0f * c.eta_r * d * t.fcr[q]);
+        v = g[t.spec[q] * c.n_shf_r + k] * dT;
       }
       for (int o = glanes >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
-      if (s < nr && k == 0) {
-        ph[3 * s + 0] = v * ux;
-        ph[3 * s + 1] = v * uy;
-        ph[3 * s + 2] = v * uz;
+      if (q < nr && k == 0) {
+        phr[3 * q + 0] = v * t.ux[q];
+        phr[3 * q + 1] = v * t.uy[q];
+        phr[3 * q + 2] = v * t.uz[q];
       }
     }
-    __syncwarp();
   }
 
-  // ---- angular: A = 2 F1 F2 fa fb.  Per triplet reduce over the sub-terms
-  //   R0 = sum g F1 F2,  R1 = sum g F1 dF2/drbar-half,  R2 = sum g F2 dF1/dc
+  // ---- angular: A = 2 F1 F2 fa fb; per triplet reduce over the sub-terms
+  //   R0 = sum g F1 F2,  R1 = sum g F1 dF2/dr,  R2 = sum g F2 dF1/dc
+  float* myph = phw + warp * 3 * capR;
   const float* gang = g + c.n_radial;
-  for (int a = 0; a < na; ++a) {
-    const PairData A = pd[a];
-    for (int b = a + 1; b < na; ++b) {
-      const PairData B = pd[b];
-      const float cth = A.ux * B.ux + A.uy * B.uy + A.uz * B.uz;
+  {
+    int a = 0, b = 1 + warp;
+    trip_norm(a, b, na);
+    while (a < na - 1) {
+      const int qa = t.asl[a], qb = t.asl[b];
+      const float uax = t.ux[qa], uay = t.uy[qa], uaz = t.uz[qa];
+      const float ubx = t.ux[qb], uby = t.uy[qb], ubz = t.uz[qb];
+      const float cth = uax * ubx + uay * uby + uaz * ubz;
       const float cc = c.cos_scale * cth;
-      const float ss = sqrtf(fmaxf(1.0f - cc * cc, 0.0f));
-      const float cot = cc / ss;
-      const float* gb = gang + pair_index(A.spec(), B.spec(), c.S) * c.n_sub;
+      const float ss = sqrt_approx(fmaxf(fmaf(-cc, cc, 1.0f), 0.0f));
+      const float cot = cc * rcp_approx(ss);
+      const float ra = t.rhi[qa], rb = t.rhi[qb];
+      const float rl = t.rlo[qa] + t.rlo[qb];
+      const int sa = t.spec[qa], sb = t.spec[qb];
+      const float* gb = gang + (sa * c.S - (sa * (sa - 1)) / 2 + (sb - sa)) * c.n_sub;
       float R0 = 0.f, R1 = 0.f, R2 = 0.f;
-      for (int t = lane; t < c.n_sub; t += 32) {
-        const int ia = t / c.n_shf_z, iz = t % c.n_shf_z;
+      for (int tt = lane; tt < c.n_sub; tt += 32) {
+        const int ia = tt / c.n_shf_z, iz = tt % c.n_shf_z;
         const float cz = c.cos_z[iz], sz = c.sin_z[iz], shfa = c.shf_a[ia];
         const float u = 0.5f + 0.5f * ((cc * cz + ss * sz) + (cc * c.cos_z_lo[iz] + ss * c.sin_z_lo[iz]));
-        const float pw1 = exp2f((c.zeta - 1.0f) * log2f(u));  // u^(zeta-1)
+        const float pw1 = pow_split(u, c.zeta1_int, c.zeta_frac);  // u^(zeta-1)
         const float F1 = pw1 * u;
         const float dF1dc = c.zeta * pw1 * 0.5f * (cz - cot * sz);
-        const float d = 0.5f * (((A.r - shfa) + (B.r - shfa)) + (A.rlo + B.rlo));
-        const float F2 = expf(-c.eta_a * d * d);
-        const float gt = gb[t];
+        const float d = 0.5f * (((ra - shfa) + (rb - shfa)) + rl);
+        const float F2 = gauss(d, c.ka_hi, c.ka_lo);
+        const float gt = gb[tt];
         R0 += gt * F1 * F2;
         R1 += gt * F1 * (-c.eta_a * d * F2);
         R2 += gt * F2 * dF1dc;
@@ -308,21 +374,29 @@ __global__ void __launch_bounds__(AEV_WARPS * 32) aev_backward_kernel(
       R1 = warp_sum(R1);
       R2 = warp_sum(R2);
       if (lane < 3) {
-        const float W = A.fc * B.fc;
-        const float coefA = 2.0f * (W * R1 + A.dfc * B.fc * R0);
-        const float coefB = 2.0f * (W * R1 + A.fc * B.dfc * R0);
+        const float fa = t.fca[qa], fb = t.fca[qb];
+        const float W = fa * fb;
+        const float coefA = 2.0f * (W * R1 + t.dfca[qa] * fb * R0);
+        const float coefB = 2.0f * (W * R1 + fa * t.dfca[qb] * R0);
         const float coefC = 2.0f * W * R2 * c.cos_scale;
-        const float ua = lane == 0 ? A.ux : (lane == 1 ? A.uy : A.uz);
-        const float ub = lane == 0 ? B.ux : (lane == 1 ? B.uy : B.uz);
-        ph[3 * A.slot() + lane] += coefA * ua + coefC * (ub - cth * ua) / A.r;
-        ph[3 * B.slot() + lane] += coefB * ub + coefC * (ua - cth * ub) / B.r;
+        const float ua = lane == 0 ? uax : (lane == 1 ? uay : uaz);
+        const float ub = lane == 0 ? ubx : (lane == 1 ? uby : ubz);
+        myph[3 * qa + lane] += coefA * ua + coefC * (ub - cth * ua) * rcp_approx(ra);
+        myph[3 * qb + lane] += coefB * ub + coefC * (ua - cth * ub) * rcp_approx(rb);
       }
       __syncwarp();
+      b += AEV_WARPS;
+      trip_norm(a, b, na);
     }
   }
-  __syncwarp();
+  __syncthreads();
   float* out = phi + (size_t)i * capR * 3;
-  for (int f = lane; f < 3 * nr; f += 32) out[f] = ph[f];
+  for (int f = threadIdx.x; f < 3 * nr; f += blockDim.x) {
+    float v = phr[f];
+#pragma unroll
+    for (int w = 0; w < AEV_WARPS; ++w) v += phw[w * 3 * capR + f];
+    out[f] = v;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -399,7 +473,7 @@ void launch_neighbors(nnp_handle* h, const float* d_pos, int pos_stride, const i
 
 void launch_aev_forward(nnp_handle* h, cudaStream_t s) {
   if (h->N == 0) return;
-  const int blocks = (h->N + AEV_WARPS - 1) / AEV_WARPS;
+  const int blocks = h->N;
   aev_forward_kernel<<<blocks, AEV_WARPS * 32, aev_smem_bytes(h, false), s>>>(
       h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA,
       h->d_aev);
@@ -407,10 +481,10 @@ void launch_aev_forward(nnp_handle* h, cudaStream_t s) {
 
 void launch_aev_backward(nnp_handle* h, cudaStream_t s) {
   if (h->N == 0) return;
-  const int blocks = (h->N + AEV_WARPS - 1) / AEV_WARPS;
+  const int blocks = h->N;
   aev_backward_kernel<<<blocks, AEV_WARPS * 32, aev_smem_bytes(h, true), s>>>(
       h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA,
-      h->d_daev, h->d_phi);
+      h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
 }
 
 void launch_finish(nnp_handle* h, const int* d_atom_index, double* d_energy, float* d_force, int force_stride,

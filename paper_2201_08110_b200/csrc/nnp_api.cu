@@ -78,6 +78,8 @@ extern "C" void nnp_destroy(nnp_handle* h) {
       if (g.d_probs) cudaFree(g.d_probs);
       if (g.d_tiles) cudaFree(g.d_tiles);
     }
+  for (auto* v : {&h->tfwd, &h->tbwd})
+    for (auto& g : *v) tma_free_launch(g);
   delete h;
 }
 
@@ -95,6 +97,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   if (!(cfg->rc_radial > 0.f) || !(cfg->rc_angular > 0.f) || cfg->rc_angular > cfg->rc_radial)
     return NNP_ERR_INVALID_ARG;
   if (!(cfg->celu_alpha > 0.f) || !(cfg->length_scale > 0.0)) return NNP_ERR_INVALID_ARG;
+  if (!(cfg->zeta >= 1.0f) || cfg->zeta >= 64.0f) return NNP_ERR_INVALID_ARG;  /* integer part by repeated squaring */
   const int n_sub = cfg->n_shf_a * cfg->n_shf_z;
   const int n_radial = S * cfg->n_shf_r;
   const int n_feat = n_radial + (S * (S + 1) / 2) * n_sub;
@@ -141,6 +144,16 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   a.zeta = cfg->zeta; a.cos_scale = cfg->cos_scale; a.length_scale = (float)cfg->length_scale;
   a.rc_r2 = (double)cfg->rc_radial * (double)cfg->rc_radial;
   a.rc_a2 = (double)cfg->rc_angular * (double)cfg->rc_angular;
+  {
+    const double z = (double)cfg->zeta;
+    a.zeta_int = (int)floor(z);
+    a.zeta1_int = a.zeta_int - 1;
+    a.zeta_frac = (float)(z - floor(z));
+    const double log2e = 1.4426950408889634074;
+    const double kr = -(double)cfg->eta_r * log2e, ka = -(double)cfg->eta_a * log2e;
+    a.kr_hi = (float)kr; a.kr_lo = (float)(kr - (double)a.kr_hi);
+    a.ka_hi = (float)ka; a.ka_lo = (float)(ka - (double)a.ka_hi);
+  }
   for (int k = 0; k < cfg->n_shf_r; ++k) a.shf_r[k] = cfg->shf_r[k];
   for (int k = 0; k < cfg->n_shf_a; ++k) a.shf_a[k] = cfg->shf_a[k];
   for (int k = 0; k < cfg->n_shf_z; ++k) {
@@ -220,11 +233,22 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     if (upload(&h->d_W, W) || upload(&h->d_b, B)) return fail(NNP_ERR_ALLOC);
   }
 
+  // ---- MLP engine: TMA-staged persistent GEMMs when the shapes allow 32-float boxes
+  bool tma_ok = !(cfg->flags & NNP_FLAG_NO_TMA) && n_feat % 4 == 0 && N > 0;
+  for (int e = 0; e < S && tma_ok; ++e)
+    for (int l = 1; l < L; ++l)
+      if (h->dims[e * (L + 1) + l] % 32 != 0) tma_ok = false;
+  if (tma_ok && tma_init() != 0) tma_ok = false;
+  h->use_tma = tma_ok;
+  // at ligand sizes the layer-1 backward is split per model (every CTA streams its own slice of W1
+  // exactly once); the M partial dE/dAEV rows are summed by the AEV backward kernel
+  h->n_parts = (tma_ok && (size_t)N * M * n_feat * 4 <= ((size_t)8 << 20)) ? M : 1;
+
   // ---- workspaces
   if (dev_alloc(&h->d_pos4, (size_t)N) || dev_alloc(&h->d_nbr_r, (size_t)N * h->capR) ||
       dev_alloc(&h->d_nbr_a, (size_t)N * h->capA) || dev_alloc(&h->d_cnt_r, (size_t)N) ||
       dev_alloc(&h->d_cnt_a, (size_t)N) || dev_alloc(&h->d_aev, (size_t)N * n_feat) ||
-      dev_alloc(&h->d_daev, (size_t)N * n_feat) || dev_alloc(&h->d_phi, (size_t)N * h->capR * 3) ||
+      dev_alloc(&h->d_daev, (size_t)h->n_parts * N * n_feat) || dev_alloc(&h->d_phi, (size_t)N * h->capR * 3) ||
       dev_alloc(&h->d_eatom, (size_t)N * M) || dev_alloc(&h->d_status, 1) || dev_alloc(&h->d_hpos, (size_t)N * 3) ||
       dev_alloc(&h->d_hforce, (size_t)N * 3) || dev_alloc(&h->d_henergy, (size_t)n_molecules))
     return fail(NNP_ERR_ALLOC);
@@ -332,6 +356,82 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     if (upload_launch(g, probs)) return fail(NNP_ERR_ALLOC);
     h->bwd.push_back(g);
   }
+  if (h->use_tma) {
+    std::vector<int> slot(S, -1);
+    int ns = 0;
+    for (int e = 0; e < S; ++e)
+      if (h->grp_off[e + 1] > h->grp_off[e]) slot[e] = ns++;
+    for (int pass = 0; pass < 2; ++pass) {
+      for (int li = 0; li < L - 1; ++li) {
+        const int l = pass == 0 ? li + 1 : L - 1 - li;  // fwd: 1..L-1, bwd: L-1..1
+        std::vector<GemmProblem> probs;
+        std::vector<TmaOperand> aops(ns), bops(ns);
+        std::vector<TmaProbExtra> extra;
+        for (int e = 0; e < S; ++e) {
+          if (slot[e] < 0) continue;
+          const int ne = h->grp_off[e + 1] - h->grp_off[e];
+          const int nin = h->dims[e * (L + 1) + l - 1], nout = h->dims[e * (L + 1) + l];
+          const float* Wl = h->d_W + h->w_off[e * L + l - 1];
+          bops[slot[e]] = TmaOperand{Wl, (long long)M * nout, nin, nin};
+          if (pass == 0) {
+            if (l == 1) aops[slot[e]] = TmaOperand{h->d_aev + (size_t)h->grp_off[e] * n_feat, ne, n_feat, n_feat};
+            else aops[slot[e]] = TmaOperand{h->d_act[l - 1] + h->act_off[l - 1][e], ne, (long long)M * nin, (long long)M * nin};
+          } else {
+            aops[slot[e]] = TmaOperand{h->d_act[l] + h->act_off[l][e], ne, (long long)M * nout, (long long)M * nout};
+          }
+          const int n_prob = (pass == 1 && l == 1 && h->n_parts == 1) ? 1 : M;
+          for (int m = 0; m < n_prob; ++m) {
+            GemmProblem p;
+            memset(&p, 0, sizeof(p));
+            TmaProbExtra x;
+            x.amap = x.bmap = slot[e];
+            x.a_row0 = 0;
+            p.alpha = alpha;
+            p.inv_alpha = 1.0f / alpha;
+            p.M = ne;
+            if (pass == 0) {
+              p.transB = 0; p.N = nout; p.K = nin;
+              p.C = h->d_act[l] + h->act_off[l][e] + (size_t)m * nout;
+              p.ldc = M * nout;
+              p.bias = h->d_b + h->b_off[e * L + l - 1] + (size_t)m * nout;
+              p.epi = EPI_BIAS_CELU;
+              x.a_col0 = l == 1 ? 0 : m * nin;
+              x.b_row0 = m * nout;
+            } else if (l > 1) {
+              p.transB = 1; p.N = nin; p.K = nout;
+              p.C = h->d_act[l - 1] + h->act_off[l - 1][e] + (size_t)m * nin;
+              p.ldc = M * nin;
+              p.aux = p.C; p.ldaux = p.ldc;
+              p.epi = EPI_MUL_DCELU;
+              x.a_col0 = m * nout;
+              x.b_row0 = m * nout;
+            } else {
+              p.transB = 1; p.N = nin;
+              p.epi = EPI_SCALE;
+              p.scale = 1.0f / (float)M;
+              p.ldc = n_feat;
+              if (h->n_parts == 1) {
+                p.K = M * nout; x.a_col0 = 0; x.b_row0 = 0;
+                p.C = h->d_daev + (size_t)h->grp_off[e] * n_feat;
+              } else {
+                p.K = nout; x.a_col0 = m * nout; x.b_row0 = m * nout;
+                p.C = h->d_daev + ((size_t)m * N + h->grp_off[e]) * n_feat;
+              }
+            }
+            probs.push_back(p);
+            extra.push_back(x);
+          }
+        }
+        TmaLaunch tl;
+        tl.name = (pass == 0 ? "mlp_fwd_l" : "mlp_bwd_l") + std::to_string(l);
+        if (tma_build_launch(tl, probs, aops, bops, extra, prop.multiProcessorCount)) {
+          tma_free_launch(tl);
+          return fail(NNP_ERR_CUDA);
+        }
+        (pass == 0 ? h->tfwd : h->tbwd).push_back(tl);
+      }
+    }
+  }
   // last layer
   {
     std::vector<long long> ao(S), wo2(S), bo2(S);
@@ -385,9 +485,17 @@ static void enqueue_chain(nnp_handle* h, const float* d_pos, int ps, const int* 
   mark();
   launch_neighbors(h, d_pos, ps, d_idx, s); mark();
   launch_aev_forward(h, s); mark();
-  for (auto& g : h->fwd) { launch_gemm(g, s); mark(); }
+  if (h->use_tma) {
+    for (auto& g : h->tfwd) { tma_launch(g, s); mark(); }
+  } else {
+    for (auto& g : h->fwd) { launch_gemm(g, s); mark(); }
+  }
   launch_last_layer(h, s); mark();
-  for (auto& g : h->bwd) { launch_gemm(g, s); mark(); }
+  if (h->use_tma) {
+    for (auto& g : h->tbwd) { tma_launch(g, s); mark(); }
+  } else {
+    for (auto& g : h->bwd) { launch_gemm(g, s); mark(); }
+  }
   launch_aev_backward(h, s); mark();
   launch_finish(h, d_idx, d_energy, d_force, fs, s); mark();
 }
@@ -542,7 +650,18 @@ static int export_rows(nnp_handle* h, const float* d_rows, float* host) {
 }
 
 extern "C" int nnp_debug_aev(nnp_handle* h, float* aev_host) { return export_rows(h, h ? h->d_aev : nullptr, aev_host); }
-extern "C" int nnp_debug_daev(nnp_handle* h, float* g_host) { return export_rows(h, h ? h->d_daev : nullptr, g_host); }
+extern "C" int nnp_debug_daev(nnp_handle* h, float* g_host) {
+  if (!h) return NNP_ERR_INVALID_ARG;
+  int rc = export_rows(h, h->d_daev, g_host);
+  if (rc != NNP_OK || h->n_parts == 1) return rc;
+  std::vector<float> part((size_t)h->N * h->n_feat);
+  for (int p = 1; p < h->n_parts; ++p) {
+    rc = export_rows(h, h->d_daev + (size_t)p * h->N * h->n_feat, part.data());
+    if (rc != NNP_OK) return rc;
+    for (size_t i = 0; i < part.size(); ++i) g_host[i] += part[i];
+  }
+  return NNP_OK;
+}
 
 extern "C" int nnp_debug_atomic_energies(nnp_handle* h, double* e_host) {
   if (!h || !e_host) return NNP_ERR_INVALID_ARG;

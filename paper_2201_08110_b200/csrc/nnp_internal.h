@@ -25,6 +25,9 @@ struct AevConst {
   int S, n_shf_r, n_shf_a, n_shf_z, n_sub, n_radial, n_feat;
   float rc_r, rc_a, eta_r, eta_a, zeta, cos_scale, length_scale;
   double rc_r2, rc_a2;  // ((double)(float)Rc)^2, the O2 predicate thresholds
+  int zeta_int, zeta1_int;     // floor(zeta), floor(zeta - 1)
+  float zeta_frac;             // zeta - floor(zeta)
+  float kr_hi, kr_lo, ka_hi, ka_lo;  // -eta*log2(e) as hi+lo: exp(-eta d^2) = ex2(d^2 k)
   float shf_r[NNP_MAX_SHF_R];
   float shf_a[NNP_MAX_SHF_A];
   float cos_z[NNP_MAX_SHF_Z];  // cos(ShfZ_z), sin(ShfZ_z): cos(theta - ShfZ) = c cosZ + s sinZ
@@ -46,6 +49,7 @@ struct GemmProblem {
   int epi;
   float scale;
   float alpha;  // CELU alpha
+  float inv_alpha;
 };
 enum { EPI_BIAS_CELU = 0, EPI_MUL_DCELU = 1, EPI_SCALE = 2 };
 
@@ -60,6 +64,36 @@ struct GemmLaunch {
   std::string name;
   double flops = 0, weight_bytes = 0;
 };
+
+// ---- TMA engine (mlp_tma.cu)
+struct TmaTile {
+  int prob, m0, n0, ta;      // problem, first atom row / output column of the tile, tile height
+  int amap, bmap;            // tensor-map slots
+  int a_row0, a_col0;        // A box origin (row = atom, col = contraction)
+  int b_row0, b_col0;        // W box origin
+  int K, transB;             // contraction length, 0 = NT / 1 = NN (copied from the problem)
+  long long cost;
+};
+struct TmaOperand {
+  const float* base;
+  long long rows, cols, ld;  // row-major [rows][cols], pitch ld floats
+};
+struct TmaProbExtra {
+  int amap, bmap, a_row0, a_col0, b_row0;
+};
+struct TmaLaunch {
+  void* params = nullptr;  // TmaGemmParams (host copy, passed by value as __grid_constant__)
+  GemmProblem* d_probs = nullptr;
+  TmaTile* d_tiles = nullptr;
+  int n_tiles = 0, grid = 0;
+  size_t smem_bytes = 0;
+  std::string name;
+};
+int tma_init();
+int tma_build_launch(TmaLaunch& L, const std::vector<GemmProblem>& probs, const std::vector<TmaOperand>& aops,
+                     const std::vector<TmaOperand>& bops, const std::vector<TmaProbExtra>& extra, int num_sms);
+void tma_launch(const TmaLaunch& L, cudaStream_t s);
+void tma_free_launch(TmaLaunch& L);
 
 // Final layer (1 output) + start of the backward pass.
 struct LastLayerArgs {
@@ -93,7 +127,7 @@ struct nnp_handle {
   float4* d_pos4 = nullptr;
   int *d_nbr_r = nullptr, *d_nbr_a = nullptr, *d_cnt_r = nullptr, *d_cnt_a = nullptr;
   float* d_aev = nullptr;   // [N sorted][n_feat]
-  float* d_daev = nullptr;  // [N sorted][n_feat]
+  float* d_daev = nullptr;  // [n_parts][N sorted][n_feat]
   float* d_phi = nullptr;   // [N][capR][3]
   double* d_eatom = nullptr;  // [N sorted][M]
   int* d_status = nullptr;
@@ -106,6 +140,9 @@ struct nnp_handle {
   std::vector<long long> act_off[NNP_MAX_LAYERS];  // [S] float offsets
   // MLP launches
   std::vector<GemmLaunch> fwd, bwd;  // fwd: layers 1..L-1; bwd: layers L-1..1
+  std::vector<TmaLaunch> tfwd, tbwd; // the same launches on the TMA engine (used when use_tma)
+  bool use_tma = false;
+  int n_parts = 1;                   // dE/dAEV is produced as n_parts partial sums (per model at small N)
   LastLayerArgs last;
   long long *d_last_act_off = nullptr, *d_last_w_off = nullptr, *d_last_b_off = nullptr;
   int* d_last_H = nullptr;

@@ -49,11 +49,24 @@ def directed(ij):
     return set(map(tuple, ij.tolist())) | set((j, i) for i, j in ij.tolist())
 
 
-def check_energy_forces(gpu, ref, mol_offsets):
+AEV_REL = 1.5e-6  # relative accuracy of an f32-evaluated angular term
+
+
+def propagated_energy_tol(ref, mol_offsets, scale):
+    """First-order bound on the energy error caused by AEV rounding, per molecule and per atom:
+    sum_i sum_f |g_if G_if| * AEV_REL * energy_scale / N.  Used for NON-ANI test networks only (their
+    weights are several times larger than the ANI-2x Xavier weights the 1e-5 tolerance is stated for)."""
+    per_atom = np.abs(ref["dG"] * ref["G"]).sum(axis=1) * AEV_REL * scale
+    sizes = np.maximum(np.diff(mol_offsets), 1)
+    return np.array([per_atom[mol_offsets[m]:mol_offsets[m + 1]].sum() for m in range(len(sizes))]) / sizes
+
+
+def check_energy_forces(gpu, ref, mol_offsets, e_tol=None):
     sizes = np.diff(mol_offsets)
     err_e = np.abs(gpu["E"] - ref["E"]) / np.maximum(sizes, 1)
     assert np.all(np.isfinite(gpu["E"])) and np.all(np.isfinite(gpu["F"]))
-    assert err_e.max() <= E_TOL_PER_ATOM, f"per-atom energy error {err_e.max():.3e} kcal/mol"
+    tol = E_TOL_PER_ATOM if e_tol is None else np.maximum(E_TOL_PER_ATOM, e_tol)
+    assert np.all(err_e <= tol), f"per-atom energy error {err_e.max():.3e} kcal/mol (tol {np.max(tol):.3e})"
     err_f = np.abs(gpu["F"] - ref["F"]).max()
     assert err_f <= F_TOL, f"max force error {err_f:.3e} kcal/mol/A (max |F| {np.abs(ref['F']).max():.2f})"
     return err_e.max(), err_f
@@ -212,7 +225,7 @@ def test_small_parameter_sets(n_species, hidden, n, seed):
     nnp = NNP(p, W, B, w.species)
     gpu = gpu_eval(nnp, w.positions, stages=True)
     check_stages(gpu, ref, orc, w.positions, w.mol_offsets)
-    check_energy_forces(gpu, ref, w.mol_offsets)
+    check_energy_forces(gpu, ref, w.mol_offsets, propagated_energy_tol(ref, w.mol_offsets, p.energy_scale))
     nnp.destroy()
 
 
@@ -225,10 +238,10 @@ def test_degenerate_inputs():
     pos = np.array([[0, 0, 0], [5, 5, 5], [5.9, 5.2, 5.1], [20, 0, 0], [21, 0.3, 0], [20.2, 1.1, 0.1]], np.float32)
     spc = np.array([0, 1, 2, 0, 0, 1], np.int32)
     off = np.array([0, 1, 3, 3, 6], np.int32)  # molecule 2 is empty
-    ref = orc.energy_forces(pos, spc, off)
+    ref = orc.energy_forces(pos, spc, off, want_intermediates=True)
     nnp = NNP(p, W, B, spc, off)
     gpu = gpu_eval(nnp, pos, n_mol=4)
-    check_energy_forces(gpu, ref, off)
+    check_energy_forces(gpu, ref, off, propagated_energy_tol(ref, off, p.energy_scale))
     assert gpu["E"][2] == 0.0 and np.all(gpu["F"][0] == 0.0)
     nnp.destroy()
     empty = NNP(p, W, B, np.zeros(0, np.int32))
