@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libnnp_b200.so")
 NNP_OK = 0
 NNP_FLAG_NO_GRAPH = 1
 NNP_FLAG_NO_TMA = 2
+NNP_FLAG_NO_UMMA = 4
 ERRORS = {
     -1: "NNP_ERR_INVALID_ARG",
     -2: "NNP_ERR_CUDA",

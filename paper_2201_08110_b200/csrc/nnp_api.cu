@@ -80,6 +80,8 @@ extern "C" void nnp_destroy(nnp_handle* h) {
     }
   for (auto* v : {&h->tfwd, &h->tbwd})
     for (auto& g : *v) tma_free_launch(g);
+  for (auto* v : {&h->ufwd, &h->ubwd})
+    for (auto& g : *v) umma_free_launch(g);
   delete h;
 }
 
@@ -239,7 +241,8 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     for (int l = 1; l < L; ++l)
       if (h->dims[e * (L + 1) + l] % 32 != 0) tma_ok = false;
   if (tma_ok && tma_init() != 0) tma_ok = false;
-  h->use_tma = tma_ok;
+  h->use_umma = tma_ok && !(cfg->flags & NNP_FLAG_NO_UMMA) && umma_init() == 0;
+  h->use_tma = tma_ok && !h->use_umma;
   // at ligand sizes the layer-1 backward is split per model (every CTA streams its own slice of W1
   // exactly once); the M partial dE/dAEV rows are summed by the AEV backward kernel
   h->n_parts = (tma_ok && (size_t)N * M * n_feat * 4 <= ((size_t)8 << 20)) ? M : 1;
@@ -432,6 +435,96 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       }
     }
   }
+  if (h->use_umma) {
+    // tcgen05 engine: D[f][a] = sum_k W[f][k] X[a][k].  Layer 1 forward runs all models of an element as ONE
+    // problem (their weight rows are contiguous and they share the AEV input): F = M*H1 is a multiple of 128.
+    std::vector<int> slot(S, -1);
+    int ns = 0;
+    for (int e = 0; e < S; ++e)
+      if (h->grp_off[e + 1] > h->grp_off[e]) slot[e] = ns++;
+    for (int pass = 0; pass < 2; ++pass) {
+      for (int li = 0; li < L - 1; ++li) {
+        const int l = pass == 0 ? li + 1 : L - 1 - li;  // fwd: 1..L-1, bwd: L-1..1
+        std::vector<UmmaProblem> probs;
+        std::vector<TmaOperand> aops(ns), bops(ns);
+        for (int e = 0; e < S; ++e) {
+          if (slot[e] < 0) continue;
+          const int ne = h->grp_off[e + 1] - h->grp_off[e];
+          const int nin = h->dims[e * (L + 1) + l - 1], nout = h->dims[e * (L + 1) + l];
+          const float* Wl = h->d_W + h->w_off[e * L + l - 1];
+          aops[slot[e]] = TmaOperand{Wl, (long long)M * nout, nin, nin};
+          if (pass == 0) {
+            if (l == 1) bops[slot[e]] = TmaOperand{h->d_aev + (size_t)h->grp_off[e] * n_feat, ne, n_feat, n_feat};
+            else bops[slot[e]] = TmaOperand{h->d_act[l - 1] + h->act_off[l - 1][e], ne, (long long)M * nin, (long long)M * nin};
+          } else {
+            bops[slot[e]] = TmaOperand{h->d_act[l] + h->act_off[l][e], ne, (long long)M * nout, (long long)M * nout};
+          }
+          UmmaProblem p;
+          memset(&p, 0, sizeof(p));
+          p.amap = p.bmap = slot[e];
+          p.n_atoms = ne;
+          p.alpha = alpha;
+          p.inv_alpha = 1.0f / alpha;
+          if (pass == 0 && l == 1) {
+            p.F = M * nout; p.K = nin;
+            p.a_c0 = 0; p.a_c1 = 0; p.b_c0 = 0; p.b_c1 = 0;
+            p.C = h->d_act[1] + h->act_off[1][e];
+            p.ldc = M * nout;
+            p.bias = h->d_b + h->b_off[e * L + 0];
+            p.epi = EPI_BIAS_CELU;
+            probs.push_back(p);
+          } else if (pass == 0) {
+            for (int m = 0; m < M; ++m) {
+              UmmaProblem q = p;
+              q.F = nout; q.K = nin;
+              q.a_c0 = 0; q.a_c1 = m * nout; q.b_c0 = m * nin; q.b_c1 = 0;
+              q.C = h->d_act[l] + h->act_off[l][e] + (size_t)m * nout;
+              q.ldc = M * nout;
+              q.bias = h->d_b + h->b_off[e * L + l - 1] + (size_t)m * nout;
+              q.epi = EPI_BIAS_CELU;
+              probs.push_back(q);
+            }
+          } else if (l > 1) {
+            for (int m = 0; m < M; ++m) {
+              UmmaProblem q = p;
+              q.F = nin; q.K = nout;
+              q.a_c0 = 0; q.a_c1 = m * nout; q.b_c0 = m * nout; q.b_c1 = 0;
+              q.C = h->d_act[l - 1] + h->act_off[l - 1][e] + (size_t)m * nin;
+              q.ldc = M * nin;
+              q.aux = q.C; q.ldaux = q.ldc;
+              q.epi = EPI_MUL_DCELU;
+              probs.push_back(q);
+            }
+          } else {
+            const int n_prob = h->n_parts == 1 ? 1 : M;
+            for (int m = 0; m < n_prob; ++m) {
+              UmmaProblem q = p;
+              q.F = nin;
+              q.epi = EPI_SCALE;
+              q.scale = 1.0f / (float)M;
+              q.ldc = n_feat;
+              q.a_c0 = 0; q.b_c1 = 0;
+              if (h->n_parts == 1) {
+                q.K = M * nout; q.a_c1 = 0; q.b_c0 = 0;
+                q.C = h->d_daev + (size_t)h->grp_off[e] * n_feat;
+              } else {
+                q.K = nout; q.a_c1 = m * nout; q.b_c0 = m * nout;
+                q.C = h->d_daev + ((size_t)m * N + h->grp_off[e]) * n_feat;
+              }
+              probs.push_back(q);
+            }
+          }
+        }
+        UmmaLaunch ul;
+        ul.name = (pass == 0 ? "mlp_fwd_l" : "mlp_bwd_l") + std::to_string(l);
+        if (umma_build_launch(ul, probs, aops, bops, pass, prop.multiProcessorCount)) {
+          umma_free_launch(ul);
+          return fail(NNP_ERR_CUDA);
+        }
+        (pass == 0 ? h->ufwd : h->ubwd).push_back(ul);
+      }
+    }
+  }
   // last layer
   {
     std::vector<long long> ao(S), wo2(S), bo2(S);
@@ -485,13 +578,17 @@ static void enqueue_chain(nnp_handle* h, const float* d_pos, int ps, const int* 
   mark();
   launch_neighbors(h, d_pos, ps, d_idx, s); mark();
   launch_aev_forward(h, s); mark();
-  if (h->use_tma) {
+  if (h->use_umma) {
+    for (auto& g : h->ufwd) { umma_launch(g, s); mark(); }
+  } else if (h->use_tma) {
     for (auto& g : h->tfwd) { tma_launch(g, s); mark(); }
   } else {
     for (auto& g : h->fwd) { launch_gemm(g, s); mark(); }
   }
   launch_last_layer(h, s); mark();
-  if (h->use_tma) {
+  if (h->use_umma) {
+    for (auto& g : h->ubwd) { umma_launch(g, s); mark(); }
+  } else if (h->use_tma) {
     for (auto& g : h->tbwd) { tma_launch(g, s); mark(); }
   } else {
     for (auto& g : h->bwd) { launch_gemm(g, s); mark(); }

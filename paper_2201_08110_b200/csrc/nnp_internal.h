@@ -95,6 +95,43 @@ int tma_build_launch(TmaLaunch& L, const std::vector<GemmProblem>& probs, const 
 void tma_launch(const TmaLaunch& L, cudaStream_t s);
 void tma_free_launch(TmaLaunch& L);
 
+// ---- tcgen05 engine (mlp_umma.cu): D[f][a] = sum_k A[f][k] B[a][k], f = output feature, a = atom
+struct UmmaItem {            // one tile of one GEMM, as the persistent CTAs consume it
+  int amap, bmap, a_mn;      // tensor-map slots; a_mn = 1: weights read as an MN-major operand (backward)
+  int a_c0, a_c1;            // weight box origin: K-major (k col, feature row) / MN-major (feature col, k row)
+  int b_c0, b_c1;            // activation box origin (k col, atom row)
+  int kb0, kb1;              // 32-wide contraction boxes [kb0, kb1)
+  int n_pad, n_valid, f_valid;  // MMA N (16/32/64/128), atoms and feature rows actually stored
+  int epi, ldc, ldaux;
+  float* C;                  // C[a * ldc + f]
+  const float* bias;         // [f] or null
+  const float* aux;          // aux[a * ldaux + f]: activations h for EPI_MUL_DCELU (may alias C)
+  float scale, alpha, inv_alpha;
+};
+struct UmmaProblem {
+  int amap, bmap;
+  int a_c0, a_c1, b_c0, b_c1;  // origins of feature 0 / atom 0 / contraction element 0
+  int F, n_atoms, K;
+  int epi, ldc, ldaux;
+  float* C;
+  const float* bias;
+  const float* aux;
+  float scale, alpha, inv_alpha;
+};
+struct UmmaLaunch {
+  void* params = nullptr;  // UmmaParams (host copy, passed by value as __grid_constant__)
+  UmmaItem* d_items = nullptr;
+  int* d_cta_off = nullptr;
+  int n_items = 0, grid = 0;
+  size_t smem_bytes = 0;
+  std::string name;
+};
+int umma_init();
+int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, const std::vector<TmaOperand>& aops,
+                      const std::vector<TmaOperand>& bops, int a_mn, int num_sms);
+void umma_launch(const UmmaLaunch& L, cudaStream_t s);
+void umma_free_launch(UmmaLaunch& L);
+
 // Final layer (1 output) + start of the backward pass.
 struct LastLayerArgs {
   float* act;          // [n_atoms_sorted][M][H] per element group (arena), overwritten with delta
@@ -140,8 +177,9 @@ struct nnp_handle {
   std::vector<long long> act_off[NNP_MAX_LAYERS];  // [S] float offsets
   // MLP launches
   std::vector<GemmLaunch> fwd, bwd;  // fwd: layers 1..L-1; bwd: layers L-1..1
-  std::vector<TmaLaunch> tfwd, tbwd; // the same launches on the TMA engine (used when use_tma)
-  bool use_tma = false;
+  std::vector<TmaLaunch> tfwd, tbwd; // the same launches on the TMA+FFMA engine (used when use_tma)
+  std::vector<UmmaLaunch> ufwd, ubwd; // the same launches on the tcgen05 engine (used when use_umma)
+  bool use_tma = false, use_umma = false;
   int n_parts = 1;                   // dE/dAEV is produced as n_parts partial sums (per model at small N)
   LastLayerArgs last;
   long long *d_last_act_off = nullptr, *d_last_w_off = nullptr, *d_last_b_off = nullptr;

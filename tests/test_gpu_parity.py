@@ -20,6 +20,7 @@ E_TOL_PER_ATOM = 1e-5  # kcal/mol
 F_TOL = 1e-3  # kcal/mol/A
 AEV_TOL = 2e-6
 DAEV_TOL = 2e-6  # Hartree per unit AEV
+E_ATOM_TOL = 1e-6  # Hartree, per (atom, model) network output: a diagnostic, see DESIGN.md section 7
 
 
 def _dev():
@@ -81,7 +82,7 @@ def check_stages(gpu, ref, orc, pos, mol_offsets):
     assert np.abs(gpu["G"] - ref["G"]).max() <= AEV_TOL * max(1.0, np.abs(ref["G"]).max())
     assert np.all(gpu["G"][ref["G"] == 0.0] == 0.0)  # structural zeros (absent species / pairs) stay exact
     e_scale = max(1.0, np.abs(ref["e_atom"]).max())
-    assert np.abs(gpu["e_atom"] - ref["e_atom"]).max() <= 5e-7 * e_scale
+    assert np.abs(gpu["e_atom"] - ref["e_atom"]).max() <= E_ATOM_TOL * e_scale
     assert np.abs(gpu["dG"] - ref["dG"]).max() <= DAEV_TOL
 
 
