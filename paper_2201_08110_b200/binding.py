@@ -17,6 +17,7 @@ NNP_OK = 0
 NNP_FLAG_NO_GRAPH = 1
 NNP_FLAG_NO_TMA = 2
 NNP_FLAG_NO_UMMA = 4
+NNP_FLAG_NO_SMALL = 8
 ERRORS = {
     -1: "NNP_ERR_INVALID_ARG",
     -2: "NNP_ERR_CUDA",

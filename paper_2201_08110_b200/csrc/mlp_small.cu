@@ -1,0 +1,397 @@
+// Ligand-size MLP engine (A4 forward, A5 per-atom energies, A6 input-gradient backward), FP32 FFMA.
+//
+// Mathematics: DESIGN.md O5/O7.  Regime: every element group of the molecule has at most a few dozen
+// atoms (BASELINE.json configs[0,1]: 12 and 50 atoms), so each layer is a set of very skinny GEMMs whose
+// cost is STREAMING THE WEIGHTS once (43 MB for layer 1 of the 8-model ensemble) -- tensor-core tiles of
+// 128 rows would be almost empty and their TMA -> MMA -> TMEM -> register chain only adds latency.  So
+// this engine is two weight-streaming kernels on the CUDA cores:
+//
+//   small_fwd_kernel   out[a][r] = CELU(b[r] + sum_k W[r][k] X[a][k])
+//       the item's activations X (<= 32 atoms x K) sit in shared memory; a warp owns two weight rows at
+//       a time, lanes split the contraction (coalesced 128-bit loads of W, 16 loads in flight per lane; X
+//       rows arrive by 1-D bulk async copies on an mbarrier while those loads are in flight),
+//       partial sums are tree-reduced with shuffles; every weight is read exactly once per item.
+//   small_bwd_kernel   out[a][n] = epi(sum_o D[a][o] W[o][n])
+//       lanes own 4 consecutive input columns (rows of the SAME row-major weights: the backward pass re-reads
+//       what the forward pass left in L2); the whole 128-column weight chunk of the item is put in flight at
+//       once as bulk async copies into shared memory (4 mbarrier groups, compute starts when the first
+//       lands); warps split atoms and/or output rows; the delta tile sits in shared memory; a fixed-order cross-warp sum in shared memory finishes the row split.
+//       The first backward launch forms delta_L-1 = w_L (.) CELU'(h_L-1) on the fly and also produces the
+//       per-atom energies e = b_L + w_L . h_L-1 (FP64), so the separate last-layer launch disappears.
+//
+// Grids are plain (one CTA per item, heavy items first) so the hardware block scheduler balances the
+// very uneven elements (23 H atoms vs 1 Cl atom in configs[1]).  Summation orders are fixed =>
+// bit-identical reruns.
+#include <algorithm>
+
+#include "nnp_internal.h"
+
+namespace {
+
+constexpr int SM_THREADS = 256;
+constexpr int SM_WARPS = SM_THREADS / 32;
+constexpr int BWD_GROUPS = 4;  // weight-row groups of the backward kernel, one mbarrier each
+
+__device__ __forceinline__ float celu_s(float x, float alpha, float inv_alpha) {
+  return x > 0.0f ? x : alpha * expm1f(x * inv_alpha);
+}
+// CELU'(x) from h = CELU(x):  x > 0 -> 1;  x <= 0 -> exp(x/alpha) = h/alpha + 1
+__device__ __forceinline__ float dcelu_s(float h, float inv_alpha) { return h > 0.0f ? 1.0f : fmaf(h, inv_alpha, 1.0f); }
+
+__device__ __forceinline__ float4 ldg_stream(const float4* p) {
+  float4 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+               : "l"(p));
+  return v;
+}
+
+__device__ __forceinline__ float dot4(const float4 w, const float4 x, float s) {
+  s = fmaf(w.x, x.x, s);
+  s = fmaf(w.y, x.y, s);
+  s = fmaf(w.z, x.z, s);
+  return fmaf(w.w, x.w, s);
+}
+
+// ---- mbarrier + 1-D bulk async copy (global -> shared), the staging path of both kernels
+__device__ __forceinline__ uint32_t s_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void sbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(s_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void sbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(s_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void sbar_wait(uint64_t* bar, uint32_t parity) {
+  const uint32_t addr = s_u32(bar);
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(addr), "r"(parity)
+        : "memory");
+  } while (!done);
+}
+// bytes % 16 == 0, both addresses 16-byte aligned
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(s_u32(dst)), "l"(src), "r"(bytes), "r"(s_u32(bar))
+               : "memory");
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+// forward
+// ------------------------------------------------------------------------------------------------
+template <int NJ>
+__global__ void __launch_bounds__(SM_THREADS, 2) small_fwd_kernel(const SmallFwdItem* __restrict__ items) {
+  extern __shared__ __align__(16) float smem_f[];
+  __shared__ __align__(8) uint64_t xbar;
+  const SmallFwdItem it = items[blockIdx.x];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int K4 = it.K >> 2;
+  float4* xs = reinterpret_cast<float4*>(smem_f);  // [n_atoms][K4]
+
+  // the first row pair of this warp: issue the weight loads before staging X so both latencies overlap
+  float4 w0[NJ], w1[NJ];
+  auto load_rows = [&](int r) {
+    const float4* p0 = reinterpret_cast<const float4*>(it.W + (size_t)r * it.K);
+    const float4* p1 = reinterpret_cast<const float4*>(it.W + (size_t)(r + 1) * it.K);
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      const int k4 = lane + 32 * j;
+      if (k4 < K4) {
+        w0[j] = ldg_stream(p0 + k4);
+        w1[j] = ldg_stream(p1 + k4);
+      } else {
+        w0[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+        w1[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+    }
+  };
+  int r = 2 * warp;
+  if (r < it.n_rows) load_rows(r);
+  // X rows (contiguous K floats per atom) arrive by bulk async copies, all in flight at once
+  if (threadIdx.x == 0) {
+    sbar_init(&xbar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    sbar_expect_tx(&xbar, (uint32_t)(it.n_atoms * it.K * 4));
+  }
+  __syncthreads();
+  if (threadIdx.x < it.n_atoms)
+    bulk_g2s(smem_f + (size_t)threadIdx.x * it.K, it.X + (size_t)threadIdx.x * it.ldx, (uint32_t)(it.K * 4), &xbar);
+  sbar_wait(&xbar, 0);
+
+  for (; r < it.n_rows; r += 2 * SM_WARPS) {
+    float keep0 = 0.0f, keep1 = 0.0f;
+    for (int a = 0; a < it.n_atoms; a += 2) {
+      const int a1 = min(a + 1, it.n_atoms - 1);
+      const float4* xa = xs + a * K4;
+      const float4* xb = xs + a1 * K4;
+      float s00 = 0.f, s01 = 0.f, s10 = 0.f, s11 = 0.f;
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) {
+        const int k4 = lane + 32 * j;
+        if (k4 < K4) {
+          const float4 x0 = xa[k4], x1 = xb[k4];
+          s00 = dot4(w0[j], x0, s00);
+          s01 = dot4(w0[j], x1, s01);
+          s10 = dot4(w1[j], x0, s10);
+          s11 = dot4(w1[j], x1, s11);
+        }
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        s00 += __shfl_xor_sync(0xffffffffu, s00, o);
+        s01 += __shfl_xor_sync(0xffffffffu, s01, o);
+        s10 += __shfl_xor_sync(0xffffffffu, s10, o);
+        s11 += __shfl_xor_sync(0xffffffffu, s11, o);
+      }
+      if (lane == a) { keep0 = s00; keep1 = s10; }
+      if (lane == a + 1) { keep0 = s01; keep1 = s11; }
+    }
+    if (lane < it.n_atoms) {
+      const float b0 = it.bias ? it.bias[r] : 0.0f, b1 = it.bias ? it.bias[r + 1] : 0.0f;
+      float2 v;
+      v.x = celu_s(keep0 + b0, it.alpha, it.inv_alpha);
+      v.y = celu_s(keep1 + b1, it.alpha, it.inv_alpha);
+      *reinterpret_cast<float2*>(it.out + (size_t)lane * it.ldc + r) = v;
+    }
+    if (r + 2 * SM_WARPS < it.n_rows) load_rows(r + 2 * SM_WARPS);  // items normally hold one pair per warp
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// backward
+// ------------------------------------------------------------------------------------------------
+// shared memory: ds [n_pad][n_out] | ws [n_out][128] | red [(n_slices-1)][n_pad][32] float4
+template <int AW>
+__device__ __forceinline__ void small_bwd_body(const SmallBwdItem& it, float* smem_f, uint64_t* bars) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int G = it.G, n_slices = SM_WARPS / G;
+  const int n_pad = G * AW;  // atoms incl. padding
+  float* ds = smem_f;
+  float* ws = ds + (size_t)n_pad * it.n_out;
+  float4* red = reinterpret_cast<float4*>(ws + (size_t)it.n_out * 128);
+  const int rpg = (((it.n_out + BWD_GROUPS - 1) / BWD_GROUPS) + 3) & ~3;  // weight rows per barrier group
+  uint64_t* dbar = bars + BWD_GROUPS;
+
+  // ---- every weight row of the chunk and the delta rows: bulk async copies, all in flight at once
+  if (threadIdx.x == 0) {
+    for (int g = 0; g < BWD_GROUPS; ++g) {
+      const int rows = max(0, min(it.n_out, (g + 1) * rpg) - g * rpg);
+      sbar_init(&bars[g], 1);
+      if (rows) sbar_expect_tx(&bars[g], (uint32_t)(rows * it.n_cols * 4));
+    }
+    sbar_init(dbar, 1);
+    if (!it.w_last) sbar_expect_tx(dbar, (uint32_t)(it.n_atoms * it.n_out * 4));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  for (int o = threadIdx.x; o < it.n_out; o += SM_THREADS)
+    bulk_g2s(ws + (size_t)o * 128, it.W + (size_t)o * it.ldw, (uint32_t)(it.n_cols * 4), &bars[o / rpg]);
+  if (!it.w_last) {
+    if (threadIdx.x < it.n_atoms)
+      bulk_g2s(ds + (size_t)threadIdx.x * it.n_out, it.D + (size_t)threadIdx.x * it.ldd, (uint32_t)(it.n_out * 4), dbar);
+    for (int idx = it.n_atoms * it.n_out + threadIdx.x; idx < n_pad * it.n_out; idx += SM_THREADS) ds[idx] = 0.0f;
+  } else {
+    // first backward layer: delta = w_L (.) CELU'(h), and the per-atom energies e = b_L + w_L . h (FP64)
+    const int no4 = it.n_out >> 2;
+    const float4* wl4 = reinterpret_cast<const float4*>(it.w_last);
+#pragma unroll 4
+    for (int idx = threadIdx.x; idx < n_pad * no4; idx += SM_THREADS) {
+      const int a = idx / no4, o4 = idx - a * no4;
+      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (a < it.n_atoms) {
+        const float4 h = __ldg(reinterpret_cast<const float4*>(it.D + (size_t)a * it.ldd) + o4);
+        const float4 w = __ldg(wl4 + o4);
+        v.x = w.x * dcelu_s(h.x, it.inv_alpha); v.y = w.y * dcelu_s(h.y, it.inv_alpha);
+        v.z = w.z * dcelu_s(h.z, it.inv_alpha); v.w = w.w * dcelu_s(h.w, it.inv_alpha);
+      }
+      reinterpret_cast<float4*>(ds)[idx] = v;
+    }
+    if (it.e_out) {
+      for (int a = warp; a < it.n_atoms; a += SM_WARPS) {
+        double acc = 0.0;
+        for (int o = lane; o < it.n_out; o += 32)
+          acc += (double)__ldg(it.w_last + o) * (double)__ldg(it.D + (size_t)a * it.ldd + o);
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+        if (lane == 0) it.e_out[(size_t)a * it.lde] = acc + (double)it.b_last;
+      }
+    }
+  }
+  __syncthreads();                     // generic-proxy writes of ds (zero fill / delta) visible
+  if (!it.w_last) sbar_wait(dbar, 0);  // bulk-copied delta rows landed
+
+  const int g = warp % G, s = warp / G;
+  const bool col_ok = 4 * lane < it.n_cols;
+  float4 acc[AW];
+#pragma unroll
+  for (int t = 0; t < AW; ++t) acc[t] = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (s < n_slices) {
+    const int rps = (((it.n_out + n_slices - 1) / n_slices) + 3) & ~3;
+    const int o0 = s * rps, o1 = min(it.n_out, o0 + rps);
+    const float4* wp = reinterpret_cast<const float4*>(ws) + lane;
+    const float* dbase = ds + (size_t)(g * AW) * it.n_out;
+    int ready = -1;  // last weight-row group known to have landed
+    for (int o = o0; o < o1; o += 4) {
+      const int grp = (o + 3) / rpg;  // rpg % 4 == 0: the four rows lie in one group
+      if (grp > ready) {
+        for (int q = ready + 1; q <= grp; ++q) sbar_wait(&bars[q], 0);
+        ready = grp;
+      }
+      if (col_ok) {
+        float4 w[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) w[i] = wp[(size_t)(o + i) * 32];
+#pragma unroll
+        for (int t = 0; t < AW; ++t) {
+          const float4 d = *reinterpret_cast<const float4*>(dbase + (size_t)t * it.n_out + o);
+          acc[t].x = fmaf(d.x, w[0].x, acc[t].x); acc[t].y = fmaf(d.x, w[0].y, acc[t].y);
+          acc[t].z = fmaf(d.x, w[0].z, acc[t].z); acc[t].w = fmaf(d.x, w[0].w, acc[t].w);
+          acc[t].x = fmaf(d.y, w[1].x, acc[t].x); acc[t].y = fmaf(d.y, w[1].y, acc[t].y);
+          acc[t].z = fmaf(d.y, w[1].z, acc[t].z); acc[t].w = fmaf(d.y, w[1].w, acc[t].w);
+          acc[t].x = fmaf(d.z, w[2].x, acc[t].x); acc[t].y = fmaf(d.z, w[2].y, acc[t].y);
+          acc[t].z = fmaf(d.z, w[2].z, acc[t].z); acc[t].w = fmaf(d.z, w[2].w, acc[t].w);
+          acc[t].x = fmaf(d.w, w[3].x, acc[t].x); acc[t].y = fmaf(d.w, w[3].y, acc[t].y);
+          acc[t].z = fmaf(d.w, w[3].z, acc[t].z); acc[t].w = fmaf(d.w, w[3].w, acc[t].w);
+        }
+      }
+    }
+  }
+  if (n_slices > 1) {  // fixed-order sum over the row slices
+    if (s > 0 && s < n_slices) {
+#pragma unroll
+      for (int t = 0; t < AW; ++t) red[((size_t)(s - 1) * n_pad + g * AW + t) * 32 + lane] = acc[t];
+    }
+    __syncthreads();
+    if (s == 0) {
+      for (int q = 1; q < n_slices; ++q) {
+#pragma unroll
+        for (int t = 0; t < AW; ++t) {
+          const float4 v = red[((size_t)(q - 1) * n_pad + g * AW + t) * 32 + lane];
+          acc[t].x += v.x; acc[t].y += v.y; acc[t].z += v.z; acc[t].w += v.w;
+        }
+      }
+    }
+  }
+  if (s == 0 && col_ok) {
+#pragma unroll
+    for (int t = 0; t < AW; ++t) {
+      const int a = g * AW + t;
+      if (a >= it.n_atoms) continue;
+      float4 v = acc[t];
+      if (it.epi == EPI_MUL_DCELU) {
+        const float4 h = *reinterpret_cast<const float4*>(it.aux + (size_t)a * it.ldaux + 4 * lane);
+        v.x *= dcelu_s(h.x, it.inv_alpha); v.y *= dcelu_s(h.y, it.inv_alpha);
+        v.z *= dcelu_s(h.z, it.inv_alpha); v.w *= dcelu_s(h.w, it.inv_alpha);
+      } else {
+        v.x *= it.scale; v.y *= it.scale; v.z *= it.scale; v.w *= it.scale;
+      }
+      *reinterpret_cast<float4*>(it.out + (size_t)a * it.ldo + 4 * lane) = v;
+    }
+  }
+}
+
+__global__ void __launch_bounds__(SM_THREADS) small_bwd_kernel(const SmallBwdItem* __restrict__ items) {
+  extern __shared__ __align__(16) float smem_f[];
+  __shared__ __align__(8) uint64_t bars[BWD_GROUPS + 1];
+  const SmallBwdItem it = items[blockIdx.x];
+  switch (it.AW) {  // atoms per warp: CTA-uniform
+    case 1: small_bwd_body<1>(it, smem_f, bars); break;
+    case 2: small_bwd_body<2>(it, smem_f, bars); break;
+    case 3: small_bwd_body<3>(it, smem_f, bars); break;
+    default: small_bwd_body<4>(it, smem_f, bars); break;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+static const size_t SMALL_SMEM_MAX = 200 * 1024;
+
+template <typename K>
+static int set_smem(K kernel, size_t bytes) {
+  return cudaFuncSetAttribute((const void*)kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) ==
+                 cudaSuccess ? 0 : -1;
+}
+
+int small_init() {
+  int rc = 0;
+  rc |= set_smem(small_fwd_kernel<1>, SMALL_SMEM_MAX);
+  rc |= set_smem(small_fwd_kernel<2>, SMALL_SMEM_MAX);
+  rc |= set_smem(small_fwd_kernel<4>, SMALL_SMEM_MAX);
+  rc |= set_smem(small_fwd_kernel<8>, SMALL_SMEM_MAX);
+  rc |= set_smem(small_bwd_kernel, SMALL_SMEM_MAX);
+  return rc;
+}
+
+void small_bwd_shape(int n_atoms, int* AW, int* G) {
+  if (n_atoms <= 4) { *G = 1; *AW = std::max(1, n_atoms); }
+  else if (n_atoms <= 8) { *G = 2; *AW = (n_atoms + 1) / 2; }
+  else if (n_atoms <= 16) { *G = 4; *AW = (n_atoms + 3) / 4; }
+  else { *G = 8; *AW = (n_atoms + 7) / 8; }
+}
+
+int small_build_fwd(SmallLaunch& L, std::vector<SmallFwdItem>& items) {
+  std::stable_sort(items.begin(), items.end(), [](const SmallFwdItem& a, const SmallFwdItem& b) {
+    return (long long)a.n_rows * a.K * (a.n_atoms + 16) > (long long)b.n_rows * b.K * (b.n_atoms + 16);
+  });
+  L.n_items = (int)items.size();
+  L.variant = 1;
+  L.smem_bytes = 0;
+  for (const auto& it : items) {
+    const int nj = (it.K + 127) / 128;
+    while (L.variant < nj) L.variant *= 2;
+    L.smem_bytes = std::max(L.smem_bytes, (size_t)it.n_atoms * it.K * 4);
+  }
+  if (L.variant > 8 || L.smem_bytes > SMALL_SMEM_MAX) return -1;
+  if (cudaMalloc(&L.d_items, std::max<size_t>(1, items.size()) * sizeof(SmallFwdItem)) != cudaSuccess) return -1;
+  if (!items.empty())
+    cudaMemcpy(L.d_items, items.data(), items.size() * sizeof(SmallFwdItem), cudaMemcpyHostToDevice);
+  return 0;
+}
+
+int small_build_bwd(SmallLaunch& L, std::vector<SmallBwdItem>& items) {
+  std::stable_sort(items.begin(), items.end(), [](const SmallBwdItem& a, const SmallBwdItem& b) {
+    return (long long)a.n_out * a.n_cols * (a.n_atoms + 16) > (long long)b.n_out * b.n_cols * (b.n_atoms + 16);
+  });
+  L.n_items = (int)items.size();
+  L.smem_bytes = 0;
+  for (const auto& it : items) {
+    if (it.AW < 1 || it.AW > 4) return -1;
+    const int n_pad = it.G * it.AW, n_slices = SM_WARPS / it.G;
+    const size_t b = (size_t)n_pad * it.n_out * 4 + (size_t)it.n_out * 512 + (size_t)std::max(0, n_slices - 1) * n_pad * 32 * 16;
+    L.smem_bytes = std::max(L.smem_bytes, b);
+  }
+  if (L.smem_bytes > SMALL_SMEM_MAX) return -1;
+  if (cudaMalloc(&L.d_items, std::max<size_t>(1, items.size()) * sizeof(SmallBwdItem)) != cudaSuccess) return -1;
+  if (!items.empty())
+    cudaMemcpy(L.d_items, items.data(), items.size() * sizeof(SmallBwdItem), cudaMemcpyHostToDevice);
+  return 0;
+}
+
+void small_launch_fwd(const SmallLaunch& L, cudaStream_t s) {
+  if (L.n_items == 0) return;
+  const SmallFwdItem* it = reinterpret_cast<const SmallFwdItem*>(L.d_items);
+  switch (L.variant) {
+    case 1: small_fwd_kernel<1><<<L.n_items, SM_THREADS, L.smem_bytes, s>>>(it); break;
+    case 2: small_fwd_kernel<2><<<L.n_items, SM_THREADS, L.smem_bytes, s>>>(it); break;
+    case 4: small_fwd_kernel<4><<<L.n_items, SM_THREADS, L.smem_bytes, s>>>(it); break;
+    default: small_fwd_kernel<8><<<L.n_items, SM_THREADS, L.smem_bytes, s>>>(it); break;
+  }
+}
+
+void small_launch_bwd(const SmallLaunch& L, cudaStream_t s) {
+  if (L.n_items == 0) return;
+  small_bwd_kernel<<<L.n_items, SM_THREADS, L.smem_bytes, s>>>(reinterpret_cast<const SmallBwdItem*>(L.d_items));
+}
+
+void small_free_launch(SmallLaunch& L) {
+  if (L.d_items) cudaFree(L.d_items);
+  L.d_items = nullptr;
+}

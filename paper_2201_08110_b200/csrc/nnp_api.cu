@@ -82,6 +82,8 @@ extern "C" void nnp_destroy(nnp_handle* h) {
     for (auto& g : *v) tma_free_launch(g);
   for (auto* v : {&h->ufwd, &h->ubwd})
     for (auto& g : *v) umma_free_launch(g);
+  for (auto* v : {&h->sfwd, &h->sbwd})
+    for (auto& g : *v) small_free_launch(g);
   delete h;
 }
 
@@ -219,8 +221,9 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     }
   h->w_floats = (size_t)wo;
   h->b_floats = (size_t)bo;
+  std::vector<float> B((size_t)bo, 0.f);  // host copy of the biases (the ligand-size engine folds b_L into its items)
   {
-    std::vector<float> W((size_t)wo, 0.f), B((size_t)bo, 0.f);
+    std::vector<float> W((size_t)wo, 0.f);
     for (int m = 0; m < M; ++m)
       for (int e = 0; e < S; ++e)
         for (int l = 0; l < L; ++l) {
@@ -241,11 +244,20 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     for (int l = 1; l < L; ++l)
       if (h->dims[e * (L + 1) + l] % 32 != 0) tma_ok = false;
   if (tma_ok && tma_init() != 0) tma_ok = false;
-  h->use_umma = tma_ok && !(cfg->flags & NNP_FLAG_NO_UMMA) && umma_init() == 0;
-  h->use_tma = tma_ok && !h->use_umma;
+  // ligand-size engine: every element group is small, so the layers are weight-streaming problems
+  int max_grp = 0, max_dim = n_feat;
+  for (int e = 0; e < S; ++e) {
+    max_grp = std::max(max_grp, h->grp_off[e + 1] - h->grp_off[e]);
+    for (int l = 1; l < L; ++l) max_dim = std::max(max_dim, h->dims[e * (L + 1) + l]);
+  }
+  const bool parts_fit = (size_t)N * M * n_feat * 4 <= ((size_t)8 << 20);
+  h->use_small = !(cfg->flags & NNP_FLAG_NO_SMALL) && N > 0 && n_feat % 4 == 0 && max_dim <= 1024 && max_grp <= 64 &&
+                 parts_fit && small_init() == 0;
+  h->use_umma = !h->use_small && tma_ok && !(cfg->flags & NNP_FLAG_NO_UMMA) && umma_init() == 0;
+  h->use_tma = !h->use_small && tma_ok && !h->use_umma;
   // at ligand sizes the layer-1 backward is split per model (every CTA streams its own slice of W1
   // exactly once); the M partial dE/dAEV rows are summed by the AEV backward kernel
-  h->n_parts = (tma_ok && (size_t)N * M * n_feat * 4 <= ((size_t)8 << 20)) ? M : 1;
+  h->n_parts = ((tma_ok || h->use_small) && parts_fit) ? M : 1;
 
   // ---- workspaces
   if (dev_alloc(&h->d_pos4, (size_t)N) || dev_alloc(&h->d_nbr_r, (size_t)N * h->capR) ||
@@ -525,6 +537,95 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       }
     }
   }
+  if (h->use_small) {
+    const float inv_alpha = 1.0f / alpha;
+    for (int l = 1; l < L; ++l) {  // forward
+      std::vector<SmallFwdItem> items;
+      for (int e = 0; e < S; ++e) {
+        const int ne = h->grp_off[e + 1] - h->grp_off[e];
+        if (ne == 0) continue;
+        const int nin = h->dims[e * (L + 1) + l - 1], nout = h->dims[e * (L + 1) + l];
+        const float* Wl = h->d_W + h->w_off[e * L + l - 1];
+        const float* bl = h->d_b + h->b_off[e * L + l - 1];
+        float* outl = h->d_act[l] + h->act_off[l][e];
+        for (int a0 = 0; a0 < ne; a0 += 32) {
+          const int na = std::min(32, ne - a0);
+          auto add = [&](int row0, int rows, const float* X, int ldx) {  // rows of the (e,l) block [M*nout][nin]
+            for (int r0 = 0; r0 < rows; r0 += 16) {  // one row pair per warp
+              SmallFwdItem it;
+              memset(&it, 0, sizeof(it));
+              it.W = Wl + (size_t)(row0 + r0) * nin;
+              it.X = X; it.ldx = ldx;
+              it.bias = bl + row0 + r0;
+              it.out = outl + (size_t)a0 * M * nout + row0 + r0;
+              it.ldc = M * nout;
+              it.n_atoms = na; it.K = nin; it.n_rows = std::min(16, rows - r0);
+              it.alpha = alpha; it.inv_alpha = inv_alpha;
+              items.push_back(it);
+            }
+          };
+          if (l == 1) {
+            add(0, M * nout, h->d_aev + (size_t)(h->grp_off[e] + a0) * n_feat, n_feat);
+          } else {
+            for (int m = 0; m < M; ++m)
+              add(m * nout, nout, h->d_act[l - 1] + h->act_off[l - 1][e] + (size_t)a0 * M * nin + (size_t)m * nin, M * nin);
+          }
+        }
+      }
+      SmallLaunch sl;
+      sl.name = "mlp_fwd_l" + std::to_string(l);
+      if (small_build_fwd(sl, items)) { small_free_launch(sl); return fail(NNP_ERR_CUDA); }
+      h->sfwd.push_back(sl);
+    }
+    for (int l = L - 1; l >= 1; --l) {  // backward
+      std::vector<SmallBwdItem> items;
+      for (int e = 0; e < S; ++e) {
+        const int ne = h->grp_off[e + 1] - h->grp_off[e];
+        if (ne == 0) continue;
+        const int nin = h->dims[e * (L + 1) + l - 1], nout = h->dims[e * (L + 1) + l];
+        const float* Wl = h->d_W + h->w_off[e * L + l - 1];
+        for (int a0 = 0; a0 < ne; a0 += 32) {
+          const int na = std::min(32, ne - a0);
+          for (int m = 0; m < M; ++m)
+            for (int n0 = 0; n0 < nin; n0 += 128) {
+              SmallBwdItem it;
+              memset(&it, 0, sizeof(it));
+              it.W = Wl + (size_t)m * nout * nin + n0;
+              it.ldw = nin;
+              it.D = h->d_act[l] + h->act_off[l][e] + (size_t)a0 * M * nout + (size_t)m * nout;
+              it.ldd = M * nout;
+              it.n_atoms = na; it.n_out = nout; it.n_cols = std::min(128, nin - n0);
+              small_bwd_shape(na, &it.AW, &it.G);
+              it.inv_alpha = inv_alpha;
+              if (l > 1) {
+                it.out = h->d_act[l - 1] + h->act_off[l - 1][e] + (size_t)a0 * M * nin + (size_t)m * nin + n0;
+                it.ldo = M * nin;
+                it.aux = it.out; it.ldaux = it.ldo;
+                it.epi = EPI_MUL_DCELU;
+              } else {
+                it.out = h->d_daev + ((size_t)m * N + h->grp_off[e] + a0) * n_feat + n0;
+                it.ldo = n_feat;
+                it.epi = EPI_SCALE;
+                it.scale = 1.0f / (float)M;
+              }
+              if (l == L - 1) {
+                it.w_last = h->d_W + h->w_off[e * L + L - 1] + (size_t)m * nout;
+                it.b_last = B[h->b_off[e * L + L - 1] + m];
+                if (n0 == 0) {
+                  it.e_out = h->d_eatom + (size_t)(h->grp_off[e] + a0) * M + m;
+                  it.lde = M;
+                }
+              }
+              items.push_back(it);
+            }
+        }
+      }
+      SmallLaunch sl;
+      sl.name = "mlp_bwd_l" + std::to_string(l);
+      if (small_build_bwd(sl, items)) { small_free_launch(sl); return fail(NNP_ERR_CUDA); }
+      h->sbwd.push_back(sl);
+    }
+  }
   // last layer
   {
     std::vector<long long> ao(S), wo2(S), bo2(S);
@@ -554,7 +655,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
 
   h->stage_names = {"nbr", "aev_fwd"};
   for (auto& g : h->fwd) h->stage_names.push_back(g.name);
-  h->stage_names.push_back("mlp_last");
+  if (!h->use_small) h->stage_names.push_back("mlp_last");
   for (auto& g : h->bwd) h->stage_names.push_back(g.name);
   h->stage_names.push_back("aev_bwd");
   h->stage_names.push_back("finish");
@@ -578,6 +679,13 @@ static void enqueue_chain(nnp_handle* h, const float* d_pos, int ps, const int* 
   mark();
   launch_neighbors(h, d_pos, ps, d_idx, s); mark();
   launch_aev_forward(h, s); mark();
+  if (h->use_small) {  // per-atom energies and delta_L-1 come out of the first backward launch
+    for (auto& g : h->sfwd) { small_launch_fwd(g, s); mark(); }
+    for (auto& g : h->sbwd) { small_launch_bwd(g, s); mark(); }
+    launch_aev_backward(h, s); mark();
+    launch_finish(h, d_idx, d_energy, d_force, fs, s); mark();
+    return;
+  }
   if (h->use_umma) {
     for (auto& g : h->ufwd) { umma_launch(g, s); mark(); }
   } else if (h->use_tma) {

@@ -132,6 +132,41 @@ int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, cons
 void umma_launch(const UmmaLaunch& L, cudaStream_t s);
 void umma_free_launch(UmmaLaunch& L);
 
+// ---- ligand-size engine (mlp_small.cu): weight-streaming FFMA kernels, one CTA per item
+struct SmallFwdItem {       // out[a*ldc + r] = CELU(bias[r] + sum_k W[r*K + k] X[a*ldx + k]),  r < n_rows, a < n_atoms
+  const float* W;           // first weight row of the item (row-major, pitch K)
+  const float* X;           // activations of the item's first atom (model columns already applied)
+  const float* bias;        // bias of the first row, or null
+  float* out;               // output of (first atom, first row)
+  int ldx, ldc, n_atoms, K, n_rows;  // n_atoms <= 32, n_rows even, K % 4 == 0
+  float alpha, inv_alpha;
+};
+struct SmallBwdItem {       // out[a*ldo + n] = epi(sum_o D[a*ldd + o] W[o*ldw + n]),  n < n_cols (<= 128)
+  const float* W;           // weights at (row 0, first column of the chunk)
+  const float* D;           // delta (or, with w_last, the activation h) of the item's first atom
+  float* out;               // output at (first atom, first column)
+  const float* aux;         // EPI_MUL_DCELU: stored activation at the same place as out (may alias it)
+  const float* w_last;      // non-null: D holds h of the last hidden layer, delta[o] = w_last[o] * CELU'(h[o])
+  double* e_out;            // non-null (with w_last): e_out[a*lde] = b_last + w_last . h  (FP64)
+  int ldw, ldd, ldo, ldaux, lde;
+  int n_atoms, n_out, n_cols;  // n_atoms <= 32, n_out % 4 == 0, n_cols % 4 == 0
+  int epi, AW, G;           // atoms per warp (1..4), atom groups (1,2,4,8): G*AW >= n_atoms
+  float scale, inv_alpha, b_last;
+};
+struct SmallLaunch {
+  void* d_items = nullptr;
+  int n_items = 0, variant = 1;
+  size_t smem_bytes = 0;
+  std::string name;
+};
+int small_init();
+void small_bwd_shape(int n_atoms, int* AW, int* G);
+int small_build_fwd(SmallLaunch& L, std::vector<SmallFwdItem>& items);
+int small_build_bwd(SmallLaunch& L, std::vector<SmallBwdItem>& items);
+void small_launch_fwd(const SmallLaunch& L, cudaStream_t s);
+void small_launch_bwd(const SmallLaunch& L, cudaStream_t s);
+void small_free_launch(SmallLaunch& L);
+
 // Final layer (1 output) + start of the backward pass.
 struct LastLayerArgs {
   float* act;          // [n_atoms_sorted][M][H] per element group (arena), overwritten with delta
@@ -179,7 +214,8 @@ struct nnp_handle {
   std::vector<GemmLaunch> fwd, bwd;  // fwd: layers 1..L-1; bwd: layers L-1..1
   std::vector<TmaLaunch> tfwd, tbwd; // the same launches on the TMA+FFMA engine (used when use_tma)
   std::vector<UmmaLaunch> ufwd, ubwd; // the same launches on the tcgen05 engine (used when use_umma)
-  bool use_tma = false, use_umma = false;
+  std::vector<SmallLaunch> sfwd, sbwd; // ligand-size engine (used when use_small); no separate last-layer launch
+  bool use_tma = false, use_umma = false, use_small = false;
   int n_parts = 1;                   // dE/dAEV is produced as n_parts partial sums (per model at small N)
   LastLayerArgs last;
   long long *d_last_act_off = nullptr, *d_last_w_off = nullptr, *d_last_b_off = nullptr;

@@ -14,7 +14,12 @@ torch = pytest.importorskip("torch")
 
 from oracle.ani_oracle import AniOracle  # noqa: E402
 from paper_2201_08110_b200 import workloads as wl  # noqa: E402
-from paper_2201_08110_b200.binding import NNP, NNP_FLAG_NO_GRAPH, NNPError  # noqa: E402
+from paper_2201_08110_b200.binding import (NNP, NNP_FLAG_NO_GRAPH, NNP_FLAG_NO_SMALL, NNP_FLAG_NO_TMA,  # noqa: E402
+                                            NNP_FLAG_NO_UMMA, NNPError)
+
+# MLP engines: ligand-size weight-streaming FFMA (default at these sizes), tcgen05 3xTF32, TMA+FFMA, plain FFMA
+ENGINES = {"small": 0, "umma": NNP_FLAG_NO_SMALL, "tma": NNP_FLAG_NO_SMALL | NNP_FLAG_NO_UMMA,
+           "ffma": NNP_FLAG_NO_SMALL | NNP_FLAG_NO_UMMA | NNP_FLAG_NO_TMA}
 
 E_TOL_PER_ATOM = 1e-5  # kcal/mol
 F_TOL = 1e-3  # kcal/mol/A
@@ -87,12 +92,13 @@ def check_stages(gpu, ref, orc, pos, mol_offsets):
 
 
 # ------------------------------------------------------------------------------------------------
-def test_config1_stagewise():
-    """BASELINE.json configs[0]: 12 atoms, 1 model; every stage export against the oracle."""
+@pytest.mark.parametrize("engine", list(ENGINES))
+def test_config1_stagewise(engine):
+    """BASELINE.json configs[0]: 12 atoms, 1 model; every stage export against the oracle, on every MLP engine."""
     w = wl.config1()
     W, B = w.weights()
     orc = AniOracle(w.params, W, B)
-    nnp = NNP(w.params, W, B, w.species)
+    nnp = NNP(w.params, W, B, w.species, flags=ENGINES[engine])
     ref = orc.energy_forces(w.positions, w.species, want_intermediates=True)
     gpu = gpu_eval(nnp, w.positions, stages=True)
     check_stages(gpu, ref, orc, w.positions, w.mol_offsets)
@@ -100,14 +106,15 @@ def test_config1_stagewise():
     nnp.destroy()
 
 
-def test_config2_trajectory_steps():
+@pytest.mark.parametrize("engine", ["small", "umma"])
+def test_config2_trajectory_steps(engine):
     """configs[1]: 50 atoms, 8 models, perturbed steps 0,1,10,100,999 of the 1000-step trajectory."""
     w = wl.config2()
     W, B = w.weights()
     orc = AniOracle(w.params, W, B)
-    nnp = NNP(w.params, W, B, w.species)
+    nnp = NNP(w.params, W, B, w.species, flags=ENGINES[engine])
     traj = w.trajectory(1000)
-    for t in (0, 1, 10, 100, 999):
+    for t in ((0, 1, 10, 100, 999) if engine == "small" else (0, 999)):
         ref = orc.energy_forces(traj[t], w.species, want_intermediates=True)
         gpu = gpu_eval(nnp, traj[t], stages=True)
         check_stages(gpu, ref, orc, traj[t], w.mol_offsets)
@@ -216,14 +223,15 @@ def test_biases_self_energy_scales_and_embedding():
 
 @pytest.mark.parametrize("n_species,hidden,n,seed", [(3, (16, 12, 8), 37, 1), (2, (32, 20, 4), 70, 2),
                                                       (5, (64, 32, 16), 150, 3)])
-def test_small_parameter_sets(n_species, hidden, n, seed):
+@pytest.mark.parametrize("engine", ["small", "umma"])
+def test_small_parameter_sets(n_species, hidden, n, seed, engine):
     """Generic nnp_config (other species counts / layer widths): ragged tiles in every GEMM."""
     p = wl.small_params(n_species, hidden)
     w = wl.random_molecule(n, n_species, seed=100 + seed, params=p, n_models=3)
     W, B = wl.make_weights(p, 3, seed=seed, random_biases=True)
     orc = AniOracle(p, W, B)
     ref = orc.energy_forces(w.positions, w.species, want_intermediates=True)
-    nnp = NNP(p, W, B, w.species)
+    nnp = NNP(p, W, B, w.species, flags=ENGINES[engine])
     gpu = gpu_eval(nnp, w.positions, stages=True)
     check_stages(gpu, ref, orc, w.positions, w.mol_offsets)
     check_energy_forces(gpu, ref, w.mol_offsets, propagated_energy_tol(ref, w.mol_offsets, p.energy_scale))
