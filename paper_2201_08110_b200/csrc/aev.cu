@@ -2,16 +2,15 @@
 // mechanical-embedding add / energy reduce (A5,A8) of the ANI hot path.  sm_100a.
 //
 // Definitions: DESIGN.md O1-O4, O6, O7 (the paper names ANI-2x, and gives no formulas).
-// Design: one warp per centre atom; the centre's 1008-float feature row (or dE/dAEV row) lives in
-// shared memory; the 32 lanes of the warp are the 32 (ShfA, ShfZ) sub-terms of an angular block, so a
-// triplet is one conflict-free shared-memory row update and no atomics are needed anywhere; forces
+// Design: one CTA per centre atom; the centre's feature row (or dE/dAEV row) and the geometry of its
+// neighbours live in shared memory; the angular work is one thread per TRIPLET (its powers and Gaussians
+// are evaluated once and combined in registers), summed in a fixed order with no atomics anywhere; forces
 // leave the kernel as one "pair gradient" phi_ij per directed pair, gathered per atom afterwards.
 #include <math_constants.h>
 
 #include "nnp_internal.h"
 
 #define FULL 0xffffffffu
-constexpr int AEV_WARPS = 4;  // warps (= centres) per CTA
 
 // ------------------------------------------------------------------------------------------------
 // A1: all-pairs neighbour search inside a molecule, warp per centre, ballot compaction.
@@ -121,33 +120,67 @@ __device__ __forceinline__ float gauss(float d, float khi, float klo) {
   return ex2_approx(fmaf(d2, klo, d2 * khi));
 }
 
-constexpr int TAB_FIELDS = 10;  // per radial slot: ux uy uz rhi rlo fcr dfcr fca dfca spec
+constexpr int AEV_THREADS = 256;  // one CTA per centre atom
+constexpr int TAB_FIELDS = 10;    // per radial slot: ux uy uz rhi rlo fcr dfcr fca dfca spec
+constexpr int TRIP_CHUNK_MAX = 1024;  // triplets of a centre processed per pass through shared memory
 
+// triplets per pass: enough for every centre of this handle, a multiple of 32, bounded
+static int trip_chunk(const nnp_handle* h) {
+  const long long t = (long long)h->capA * (h->capA - 1) / 2;
+  long long c = (t + 31) / 32 * 32;
+  if (c < 32) c = 32;
+  if (c > TRIP_CHUNK_MAX) c = TRIP_CHUNK_MAX;
+  return (int)c;
+}
+static int ang_row_pad(const nnp_handle* h) {  // floats per padded angular block of the staged dE/dAEV row
+  return h->aev.n_sub + 4;
+}
+
+// shared memory (floats): table | asl[capA] | sp_off[S+1] | pair_st[n_pairs] | kernel-specific part
+static size_t aev_common_floats(const nnp_handle* h) {
+  const int S = h->S;
+  return (size_t)TAB_FIELDS * h->capR + h->capA + (S + 1) + (size_t)S * (S + 1) / 2;
+}
 size_t aev_smem_bytes(const nnp_handle* h, bool backward) {
-  size_t fl = (size_t)TAB_FIELDS * h->capR + h->capA;
-  if (!backward) fl += (size_t)AEV_WARPS * (h->n_feat - h->aev.n_radial);
-  else fl += (size_t)h->n_feat + (size_t)(AEV_WARPS + 1) * 3 * h->capR;
-  return ((fl + 3) & ~(size_t)3) * 4;
+  size_t fl = aev_common_floats(h);
+  const int n_pairs = h->S * (h->S + 1) / 2;
+  const int CH = trip_chunk(h);
+  if (!backward) {
+    fl += (size_t)(h->n_feat - h->aev.n_radial);                       // angular part of the row
+    fl += (size_t)(h->aev.n_shf_z + h->aev.n_shf_a) * CH;              // F1 / F2 factors of a pass
+  } else {
+    fl += (size_t)h->aev.n_radial + (size_t)n_pairs * ang_row_pad(h);  // dE/dAEV row (angular blocks padded)
+    fl += (size_t)2 * 3 * h->capR;                                     // radial + angular pair gradients
+    fl += (size_t)6 * CH;                                              // per-triplet gradient pairs of a pass
+  }
+  return ((fl + 3) & ~(size_t)3) * 4 + 16;
 }
 
 struct CentreTab {
   float *ux, *uy, *uz, *rhi, *rlo, *fcr, *dfcr, *fca, *dfca;
   int* spec;
-  int* asl;  // angular neighbours: radial slots, sorted by species (stable)
+  int* asl;      // angular neighbours: radial slots, sorted by species (stable)
+  int* sp_off;   // [S+1] first position in asl of every species
+  int* pair_st;  // [n_pairs] (s << 8) | t of every species-pair block, s <= t
+  float* rest;   // kernel-specific part (16-byte aligned)
 };
 
-__device__ __forceinline__ CentreTab carve_tab(float* smem, int capR) {
+__device__ __forceinline__ CentreTab carve_tab(float* smem, int capR, int capA, int S) {
   CentreTab t;
   t.ux = smem; t.uy = t.ux + capR; t.uz = t.uy + capR; t.rhi = t.uz + capR; t.rlo = t.rhi + capR;
   t.fcr = t.rlo + capR; t.dfcr = t.fcr + capR; t.fca = t.dfcr + capR; t.dfca = t.fca + capR;
   t.spec = reinterpret_cast<int*>(t.dfca + capR);
   t.asl = t.spec + capR;
+  t.sp_off = t.asl + capA;
+  t.pair_st = t.sp_off + (S + 1);
+  const int used = TAB_FIELDS * capR + capA + (S + 1) + S * (S + 1) / 2;
+  t.rest = smem + ((used + 3) & ~3);
   return t;
 }
 
 // Phase 0 of both AEV kernels: geometry of every radial neighbour of centre i (FP64 once, all threads
-// of the CTA in parallel), and the angular neighbour list re-ordered by species so that consecutive
-// triplets of a warp fall into the same feature block.
+// of the CTA in parallel), the angular neighbour list re-ordered by species (so the triplets of one
+// species-pair block are index ranges), the species offsets and the block -> species-pair table.
 __device__ __forceinline__ void build_tab(const CentreTab& t, int i, int nr, int na, const float4 pi,
                                           const float4* __restrict__ pos4, const int* __restrict__ nbr_r,
                                           const int* __restrict__ nbr_a, int capR, int capA, const AevConst& c) {
@@ -175,6 +208,11 @@ __device__ __forceinline__ void build_tab(const CentreTab& t, int i, int nr, int
     t.dfca[q] = -(CUDART_PI_F / c.rc_a) * sh * ch;
     t.spec[q] = __float_as_int(pj.w);
   }
+  // block -> (s, t) table: row-major upper triangle
+  for (int s = threadIdx.x; s < c.S; s += blockDim.x) {
+    int p = s * c.S - (s * (s - 1)) / 2;
+    for (int u = s; u < c.S; ++u) t.pair_st[p++] = (s << 8) | u;
+  }
   __syncthreads();
   // stable counting sort of the angular list by species: rank = #(smaller species) + #(same, earlier)
   for (int q = threadIdx.x; q < na; q += blockDim.x) {
@@ -187,38 +225,53 @@ __device__ __forceinline__ void build_tab(const CentreTab& t, int i, int nr, int
     }
     t.asl[rank] = slot;
   }
+  for (int s = threadIdx.x; s <= c.S; s += blockDim.x) {
+    int cnt = 0;
+    for (int q2 = 0; q2 < na; ++q2) cnt += t.spec[nbr_a[(size_t)i * capA + q2]] < s;
+    t.sp_off[s] = cnt;
+  }
   __syncthreads();
 }
 
-// first triplet (a,b), a<b<na, of warp w in the flattened order, and the step to the next one
-__device__ __forceinline__ void trip_norm(int& a, int& b, int na) {
-  while (a < na - 1 && b >= na) {
-    ++a;
-    b = b - na + a + 1;
-  }
+// unordered triplets (a, b), a < b < na, in row-major order: flat index and its inverse
+__device__ __forceinline__ int trip_row_start(int a, int na) { return (a * (2 * na - a - 1)) >> 1; }
+__device__ __forceinline__ void trip_decode(int t, int na, int& a, int& b) {
+  const float m = (float)(2 * na - 1);
+  int r = (int)(0.5f * (m - sqrtf(fmaxf(m * m - 8.0f * (float)t, 0.0f))));
+  r = max(0, min(r, na - 2));
+  while (r > 0 && trip_row_start(r, na) > t) --r;
+  while (r < na - 2 && trip_row_start(r + 1, na) <= t) ++r;
+  a = r;
+  b = t - trip_row_start(r, na) + r + 1;
 }
 
 // ------------------------------------------------------------------------------------------------
-// A2 + A3: AEV forward.  One CTA (4 warps) per centre.
+// A2 + A3: AEV forward.  One CTA per centre.
 //   radial : one thread per output column (species s, shift k) loops over the neighbours of species s
 //            and keeps the sum in a register (fixed order, no shared-memory updates);
-//   angular: the triplets are dealt round-robin to the 4 warps; lanes are the (ShfA, ShfZ) sub-terms;
-//            each warp sums runs of triplets that fall into the same species-pair block in a register
-//            and flushes to its own partial row; the 4 partial rows are added in a fixed order.
+//   angular: the angular term is separable, A = F1_z(theta) * [2 F2_a(r_a, r_b) f_C f_C], so
+//            pass 1: one THREAD per triplet evaluates its n_shf_z powers and n_shf_a Gaussians once
+//                    (12 transcendental groups instead of 32 per triplet) into shared memory;
+//            pass 2: one thread per output column (block p, a, z) sums F1_z * F2_a over the triplets of
+//                    its species-pair block, which are index ranges because the angular list is sorted by
+//                    species.  Fixed order, no atomics.
+// NZ / NA are the register-array bounds (n_shf_z <= NZ, n_shf_a <= NA).
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(AEV_WARPS * 32) aev_forward_kernel(
+template <int NZ, int NA>
+__global__ void __launch_bounds__(AEV_THREADS) aev_forward_kernel(
     const float4* __restrict__ pos4, const int* __restrict__ nbr_r, const int* __restrict__ nbr_a,
     const int* __restrict__ cnt_r, const int* __restrict__ cnt_a, const int* __restrict__ sortpos, int N,
-    const __grid_constant__ AevConst c, int capR, int capA, float* __restrict__ aev) {
+    const __grid_constant__ AevConst c, int capR, int capA, int CH, float* __restrict__ aev) {
   extern __shared__ __align__(16) float smem[];
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int i = blockIdx.x;
-  const CentreTab t = carve_tab(smem, capR);
+  const CentreTab t = carve_tab(smem, capR, capA, c.S);
   const int n_ang = c.n_feat - c.n_radial;
-  float* rows = reinterpret_cast<float*>(t.asl + capA);  // [AEV_WARPS][n_ang]
+  float* row = t.rest;                 // [n_ang]
+  float* bF1 = row + n_ang;            // [n_shf_z][CH]
+  float* bF2 = bF1 + c.n_shf_z * CH;   // [n_shf_a][CH]
   const float4 pi = pos4[i];
   const int nr = cnt_r[i], na = cnt_a[i];
-  for (int f = threadIdx.x; f < AEV_WARPS * n_ang; f += blockDim.x) rows[f] = 0.0f;
+  for (int f = threadIdx.x; f < n_ang; f += blockDim.x) row[f] = 0.0f;
   build_tab(t, i, nr, na, pi, pos4, nbr_r, nbr_a, capR, capA, c);
   float* out = aev + (size_t)sortpos[i] * c.n_feat;
 
@@ -236,53 +289,66 @@ __global__ void __launch_bounds__(AEV_WARPS * 32) aev_forward_kernel(
   }
 
   // ---- angular (O4)
-  float* myrow = rows + warp * n_ang;
-  const int nsub_it = (c.n_sub + 31) >> 5;
-  for (int it = 0; it < nsub_it; ++it) {
-    const int tt = lane + 32 * it;
-    const bool live = tt < c.n_sub;
-    const int ia = live ? tt / c.n_shf_z : 0, iz = live ? tt % c.n_shf_z : 0;
-    const float shfa = c.shf_a[ia], cz = c.cos_z[iz], sz = c.sin_z[iz];
-    const float czl = c.cos_z_lo[iz], szl = c.sin_z_lo[iz];
-    int a = 0, b = 1 + warp;
-    trip_norm(a, b, na);
-    int cur_p = -1;
-    float acc = 0.0f;
-    while (a < na - 1) {
+  const int ntrip = (na * (na - 1)) >> 1;
+  for (int c0 = 0; c0 < ntrip; c0 += CH) {
+    const int cn = min(CH, ntrip - c0);
+    for (int tl = threadIdx.x; tl < cn; tl += blockDim.x) {
+      int a, b;
+      trip_decode(c0 + tl, na, a, b);
       const int qa = t.asl[a], qb = t.asl[b];
       const float cth = t.ux[qa] * t.ux[qb] + t.uy[qa] * t.uy[qb] + t.uz[qa] * t.uz[qb];
       const float cc = c.cos_scale * cth;
       const float ss = sqrt_approx(fmaxf(fmaf(-cc, cc, 1.0f), 0.0f));
-      const float u = 0.5f + 0.5f * ((cc * cz + ss * sz) + (cc * czl + ss * szl));
-      const float F1 = pow_split(u, c.zeta_int, c.zeta_frac);
-      const float d = 0.5f * (((t.rhi[qa] - shfa) + (t.rhi[qb] - shfa)) + (t.rlo[qa] + t.rlo[qb]));
-      const float F2 = gauss(d, c.ka_hi, c.ka_lo);
-      const float val = 2.0f * F1 * F2 * (t.fca[qa] * t.fca[qb]);
-      const int sa = t.spec[qa], sb = t.spec[qb];  // sa <= sb (sorted)
-      const int p = sa * c.S - (sa * (sa - 1)) / 2 + (sb - sa);
-      if (p != cur_p) {
-        if (cur_p >= 0 && live) myrow[cur_p * c.n_sub + tt] += acc;
-        cur_p = p;
-        acc = 0.0f;
-      }
-      acc += val;
-      b += AEV_WARPS;
-      trip_norm(a, b, na);
-    }
-    if (cur_p >= 0 && live) myrow[cur_p * c.n_sub + tt] += acc;
-  }
-  __syncthreads();
-  for (int f = threadIdx.x; f < n_ang; f += blockDim.x) {
-    float v = rows[f];
 #pragma unroll
-    for (int w = 1; w < AEV_WARPS; ++w) v += rows[w * n_ang + f];
-    out[c.n_radial + f] = v;
+      for (int iz = 0; iz < NZ; ++iz) {
+        if (iz < c.n_shf_z) {
+          const float u = 0.5f + 0.5f * ((cc * c.cos_z[iz] + ss * c.sin_z[iz]) + (cc * c.cos_z_lo[iz] + ss * c.sin_z_lo[iz]));
+          bF1[iz * CH + tl] = pow_split(u, c.zeta_int, c.zeta_frac);
+        }
+      }
+      const float w = 2.0f * (t.fca[qa] * t.fca[qb]);
+      const float ra = t.rhi[qa], rb = t.rhi[qb], rl = t.rlo[qa] + t.rlo[qb];
+#pragma unroll
+      for (int ia = 0; ia < NA; ++ia) {
+        if (ia < c.n_shf_a) {
+          const float shfa = c.shf_a[ia];
+          const float d = 0.5f * (((ra - shfa) + (rb - shfa)) + rl);
+          bF2[ia * CH + tl] = w * gauss(d, c.ka_hi, c.ka_lo);
+        }
+      }
+    }
+    __syncthreads();
+    for (int f = threadIdx.x; f < n_ang; f += blockDim.x) {
+      const int p = f / c.n_sub, sub = f - p * c.n_sub;
+      const int ia = sub / c.n_shf_z, iz = sub - ia * c.n_shf_z;
+      const int st = t.pair_st[p];
+      const int s = st >> 8, u = st & 255;
+      const int a0 = t.sp_off[s], a1 = t.sp_off[s + 1], b0 = t.sp_off[u], b1 = t.sp_off[u + 1];
+      if (a0 == a1 || b0 == b1) continue;
+      const float* f1 = bF1 + iz * CH;
+      const float* f2 = bF2 + ia * CH;
+      float acc = 0.0f;
+      for (int a = a0; a < a1; ++a) {
+        const int base = trip_row_start(a, na) - a - 1 - c0;  // local index of (a, b) is base + b
+        const int lo = max(s == u ? a + 1 : b0, -base);
+        const int hi = min(b1, cn - base);
+        for (int b = lo; b < hi; ++b) acc = fmaf(f1[base + b], f2[base + b], acc);
+      }
+      row[f] += acc;
+    }
+    __syncthreads();
   }
+  for (int f = threadIdx.x; f < n_ang; f += blockDim.x) out[c.n_radial + f] = row[f];
 }
 
 // ------------------------------------------------------------------------------------------------
-// A7: AEV backward.  One CTA (4 warps) per centre.  phi[i][slot] = dE/d(r_j - r_i) for every radial
-// slot of i (pair-gradient formulation: no atomics, the force gather happens per atom afterwards).
+// A7: AEV backward.  One CTA per centre.  phi[i][slot] = dE/d(r_j - r_i) for every radial slot of i
+// (pair-gradient formulation: no atomics, the force gather happens per atom afterwards).
+//   angular: one THREAD per triplet.  With G the n_shf_a x n_shf_z block of dE/dAEV of the triplet's
+//   species pair,  R0 = sum_a F2_a (G F1)_a,  R1 = sum_a dF2_a (G F1)_a,  R2 = sum_a F2_a (G dF1)_a  are
+//   register sums (4 powers + 8 Gaussians + 8 float4 shared-memory loads per triplet for ANI-2x); the
+//   triplet's two pair gradients go to a shared-memory buffer and one thread per (neighbour, component)
+//   adds them in triplet order (fixed order => bit-identical reruns).
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
@@ -290,27 +356,42 @@ __device__ __forceinline__ float warp_sum(float v) {
   return v;
 }
 
-__global__ void __launch_bounds__(AEV_WARPS * 32) aev_backward_kernel(
+template <int NZ, int NA>
+__global__ void __launch_bounds__(AEV_THREADS) aev_backward_kernel(
     const float4* __restrict__ pos4, const int* __restrict__ nbr_r, const int* __restrict__ nbr_a,
     const int* __restrict__ cnt_r, const int* __restrict__ cnt_a, const int* __restrict__ sortpos, int N,
-    const __grid_constant__ AevConst c, int capR, int capA, const float* __restrict__ daev, int n_parts,
+    const __grid_constant__ AevConst c, int capR, int capA, int CH, const float* __restrict__ daev, int n_parts,
     size_t part_stride, float* __restrict__ phi) {
   extern __shared__ __align__(16) float smem[];
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int i = blockIdx.x;
-  const CentreTab t = carve_tab(smem, capR);
-  float* g = reinterpret_cast<float*>(t.asl + capA);  // [n_feat]
-  float* phr = g + c.n_feat;                          // radial part           [capR][3]
-  float* phw = phr + 3 * capR;                        // per-warp angular part [AEV_WARPS][capR][3]
+  const CentreTab t = carve_tab(smem, capR, capA, c.S);
+  const int n_pairs = (c.S * (c.S + 1)) >> 1;
+  const int bpad = c.n_sub + 4;         // padded block pitch: blocks of different species pairs hit different banks
+  float* g = t.rest;                    // [n_radial]
+  float* gang = g + c.n_radial;         // [n_pairs][bpad]
+  float* phr = gang + n_pairs * bpad;   // radial part   [capR][3]
+  float* pha = phr + 3 * capR;          // angular part  [capR][3]
+  float* buf = pha + 3 * capR;          // [6][CH] pair gradients of the triplets of a pass
   const float4 pi = pos4[i];
   const int nr = cnt_r[i], na = cnt_a[i];
   const float* gin = daev + (size_t)sortpos[i] * c.n_feat;
+  // dE/dAEV row = fixed-order sum of the partial rows; the loads of a column are independent
   for (int f = threadIdx.x; f < c.n_feat; f += blockDim.x) {
     float v = gin[f];
-    for (int p = 1; p < n_parts; ++p) v += gin[(size_t)p * part_stride + f];  // fixed order
-    g[f] = v;
+    int p = 1;
+    for (; p + 4 <= n_parts; p += 4) {
+      const float v0 = gin[(size_t)p * part_stride + f], v1 = gin[(size_t)(p + 1) * part_stride + f];
+      const float v2 = gin[(size_t)(p + 2) * part_stride + f], v3 = gin[(size_t)(p + 3) * part_stride + f];
+      v += v0; v += v1; v += v2; v += v3;
+    }
+    for (; p < n_parts; ++p) v += gin[(size_t)p * part_stride + f];
+    if (f < c.n_radial) g[f] = v;
+    else {
+      const int fa = f - c.n_radial, blk = fa / c.n_sub;
+      gang[blk * bpad + (fa - blk * c.n_sub)] = v;
+    }
   }
-  for (int f = threadIdx.x; f < AEV_WARPS * 3 * nr; f += blockDim.x) phw[(f / (3 * nr)) * 3 * capR + f % (3 * nr)] = 0.0f;
+  for (int f = threadIdx.x; f < 3 * nr; f += blockDim.x) pha[f] = 0.0f;
   build_tab(t, i, nr, na, pi, pos4, nbr_r, nbr_a, capR, capA, c);
 
   // ---- radial: dT/dr = 0.25 e (f_C' - 2 eta (r - Shf) f_C); a group of lanes per neighbour
@@ -336,14 +417,14 @@ __global__ void __launch_bounds__(AEV_WARPS * 32) aev_backward_kernel(
     }
   }
 
-  // ---- angular: A = 2 F1 F2 fa fb; per triplet reduce over the sub-terms
-  //   R0 = sum g F1 F2,  R1 = sum g F1 dF2/dr,  R2 = sum g F2 dF1/dc
-  float* myph = phw + warp * 3 * capR;
-  const float* gang = g + c.n_radial;
-  {
-    int a = 0, b = 1 + warp;
-    trip_norm(a, b, na);
-    while (a < na - 1) {
+  // ---- angular: A = 2 F1 F2 fa fb
+  const int ntrip = (na * (na - 1)) >> 1;
+  const bool vec4 = (NZ == 4) && c.n_shf_z == 4 && (c.n_radial & 3) == 0;
+  for (int c0 = 0; c0 < ntrip; c0 += CH) {
+    const int cn = min(CH, ntrip - c0);
+    for (int tl = threadIdx.x; tl < cn; tl += blockDim.x) {
+      int a, b;
+      trip_decode(c0 + tl, na, a, b);
       const int qa = t.asl[a], qb = t.asl[b];
       const float uax = t.ux[qa], uay = t.uy[qa], uaz = t.uz[qa];
       const float ubx = t.ux[qb], uby = t.uy[qb], ubz = t.uz[qb];
@@ -353,50 +434,83 @@ __global__ void __launch_bounds__(AEV_WARPS * 32) aev_backward_kernel(
       const float cot = cc * rcp_approx(ss);
       const float ra = t.rhi[qa], rb = t.rhi[qb];
       const float rl = t.rlo[qa] + t.rlo[qb];
-      const int sa = t.spec[qa], sb = t.spec[qb];
-      const float* gb = gang + (sa * c.S - (sa * (sa - 1)) / 2 + (sb - sa)) * c.n_sub;
+      const int sa = t.spec[qa], sb = t.spec[qb];  // sa <= sb (sorted)
+      const float* gb = gang + (sa * c.S - (sa * (sa - 1)) / 2 + (sb - sa)) * bpad;
+      float F1[NZ], dF1[NZ];
+#pragma unroll
+      for (int iz = 0; iz < NZ; ++iz) {
+        F1[iz] = 0.0f; dF1[iz] = 0.0f;
+        if (iz < c.n_shf_z) {
+          const float cz = c.cos_z[iz], sz = c.sin_z[iz];
+          const float u = 0.5f + 0.5f * ((cc * cz + ss * sz) + (cc * c.cos_z_lo[iz] + ss * c.sin_z_lo[iz]));
+          const float pw1 = pow_split(u, c.zeta1_int, c.zeta_frac);  // u^(zeta-1)
+          F1[iz] = pw1 * u;
+          dF1[iz] = c.zeta * pw1 * 0.5f * (cz - cot * sz);
+        }
+      }
       float R0 = 0.f, R1 = 0.f, R2 = 0.f;
-      for (int tt = lane; tt < c.n_sub; tt += 32) {
-        const int ia = tt / c.n_shf_z, iz = tt % c.n_shf_z;
-        const float cz = c.cos_z[iz], sz = c.sin_z[iz], shfa = c.shf_a[ia];
-        const float u = 0.5f + 0.5f * ((cc * cz + ss * sz) + (cc * c.cos_z_lo[iz] + ss * c.sin_z_lo[iz]));
-        const float pw1 = pow_split(u, c.zeta1_int, c.zeta_frac);  // u^(zeta-1)
-        const float F1 = pw1 * u;
-        const float dF1dc = c.zeta * pw1 * 0.5f * (cz - cot * sz);
-        const float d = 0.5f * (((ra - shfa) + (rb - shfa)) + rl);
-        const float F2 = gauss(d, c.ka_hi, c.ka_lo);
-        const float gt = gb[tt];
-        R0 += gt * F1 * F2;
-        R1 += gt * F1 * (-c.eta_a * d * F2);
-        R2 += gt * F2 * dF1dc;
+#pragma unroll
+      for (int ia = 0; ia < NA; ++ia) {
+        if (ia < c.n_shf_a) {
+          const float shfa = c.shf_a[ia];
+          const float d = 0.5f * (((ra - shfa) + (rb - shfa)) + rl);
+          const float F2 = gauss(d, c.ka_hi, c.ka_lo);
+          float s1 = 0.f, s2 = 0.f;
+          if (vec4) {
+            const float4 gv = *reinterpret_cast<const float4*>(gb + 4 * ia);
+            s1 = gv.x * F1[0]; s2 = gv.x * dF1[0];
+            if (NZ > 1) { s1 = fmaf(gv.y, F1[1 % NZ], s1); s2 = fmaf(gv.y, dF1[1 % NZ], s2); }
+            if (NZ > 2) { s1 = fmaf(gv.z, F1[2 % NZ], s1); s2 = fmaf(gv.z, dF1[2 % NZ], s2); }
+            if (NZ > 3) { s1 = fmaf(gv.w, F1[3 % NZ], s1); s2 = fmaf(gv.w, dF1[3 % NZ], s2); }
+          } else {
+#pragma unroll
+            for (int iz = 0; iz < NZ; ++iz) {
+              if (iz < c.n_shf_z) {
+                const float gv = gb[ia * c.n_shf_z + iz];
+                s1 = fmaf(gv, F1[iz], s1);
+                s2 = fmaf(gv, dF1[iz], s2);
+              }
+            }
+          }
+          R0 = fmaf(F2, s1, R0);
+          R1 = fmaf(-c.eta_a * d * F2, s1, R1);
+          R2 = fmaf(F2, s2, R2);
+        }
       }
-      R0 = warp_sum(R0);
-      R1 = warp_sum(R1);
-      R2 = warp_sum(R2);
-      if (lane < 3) {
-        const float fa = t.fca[qa], fb = t.fca[qb];
-        const float W = fa * fb;
-        const float coefA = 2.0f * (W * R1 + t.dfca[qa] * fb * R0);
-        const float coefB = 2.0f * (W * R1 + fa * t.dfca[qb] * R0);
-        const float coefC = 2.0f * W * R2 * c.cos_scale;
-        const float ua = lane == 0 ? uax : (lane == 1 ? uay : uaz);
-        const float ub = lane == 0 ? ubx : (lane == 1 ? uby : ubz);
-        myph[3 * qa + lane] += coefA * ua + coefC * (ub - cth * ua) * rcp_approx(ra);
-        myph[3 * qb + lane] += coefB * ub + coefC * (ua - cth * ub) * rcp_approx(rb);
-      }
-      __syncwarp();
-      b += AEV_WARPS;
-      trip_norm(a, b, na);
+      const float fa = t.fca[qa], fb = t.fca[qb];
+      const float W = fa * fb;
+      const float coefA = 2.0f * (W * R1 + t.dfca[qa] * fb * R0);
+      const float coefB = 2.0f * (W * R1 + fa * t.dfca[qb] * R0);
+      const float coefC = 2.0f * W * R2 * c.cos_scale;
+      const float ia_r = coefC * rcp_approx(ra), ib_r = coefC * rcp_approx(rb);
+      buf[0 * CH + tl] = coefA * uax + ia_r * (ubx - cth * uax);
+      buf[1 * CH + tl] = coefA * uay + ia_r * (uby - cth * uay);
+      buf[2 * CH + tl] = coefA * uaz + ia_r * (ubz - cth * uaz);
+      buf[3 * CH + tl] = coefB * ubx + ib_r * (uax - cth * ubx);
+      buf[4 * CH + tl] = coefB * uby + ib_r * (uay - cth * uby);
+      buf[5 * CH + tl] = coefB * ubz + ib_r * (uaz - cth * ubz);
     }
+    __syncthreads();
+    // one thread per (angular neighbour s, component): add the gradients of the triplets that contain s
+    for (int w = threadIdx.x; w < 3 * na; w += blockDim.x) {
+      const int comp = w / na, s = w - comp * na;
+      float acc = 0.0f;
+      for (int a = 0; a < s; ++a) {  // triplets (a, s): s is the second member
+        const int tl = trip_row_start(a, na) + (s - a - 1) - c0;
+        if (tl >= 0 && tl < cn) acc += buf[(3 + comp) * CH + tl];
+      }
+      {  // triplets (s, b), b > s: a contiguous run
+        const int base = trip_row_start(s, na) - s - 1 - c0;
+        const int lo = max(s + 1, -base), hi = min(na, cn - base);
+        for (int b = lo; b < hi; ++b) acc += buf[comp * CH + base + b];
+      }
+      pha[3 * t.asl[s] + comp] += acc;
+    }
+    __syncthreads();
   }
   __syncthreads();
   float* out = phi + (size_t)i * capR * 3;
-  for (int f = threadIdx.x; f < 3 * nr; f += blockDim.x) {
-    float v = phr[f];
-#pragma unroll
-    for (int w = 0; w < AEV_WARPS; ++w) v += phw[w * 3 * capR + f];
-    out[f] = v;
-  }
+  for (int f = threadIdx.x; f < 3 * nr; f += blockDim.x) out[f] = phr[f] + pha[f];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -405,7 +519,10 @@ __global__ void __launch_bounds__(AEV_WARPS * 32) aev_backward_kernel(
 // (warp per atom), the remaining blocks do energies (warp per molecule).  Fixed reduction trees,
 // no atomics => bit-identical reruns.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) finish_kernel(
+constexpr int FIN_THREADS = 256;
+constexpr int FIN_WARPS = FIN_THREADS / 32;
+
+__global__ void __launch_bounds__(FIN_THREADS) finish_kernel(
     const int* __restrict__ nbr_r, const int* __restrict__ cnt_r, const float* __restrict__ phi, int N, int capR,
     const int* __restrict__ atom_index, float* __restrict__ force, int force_stride, float fscale,
     int n_force_blocks, const double* __restrict__ eatom, const int* __restrict__ sortpos,
@@ -414,7 +531,7 @@ __global__ void __launch_bounds__(128) finish_kernel(
   const int lane = threadIdx.x & 31;
   const int wib = threadIdx.x >> 5;
   if ((int)blockIdx.x < n_force_blocks) {
-    const int a = blockIdx.x * 4 + wib;
+    const int a = blockIdx.x * FIN_WARPS + wib;
     if (a >= N || force == nullptr) return;
     const int n = cnt_r[a];
     float fx = 0.f, fy = 0.f, fz = 0.f;
@@ -445,10 +562,12 @@ __global__ void __launch_bounds__(128) finish_kernel(
       f[2] += fscale * fz;
     }
   } else {
-    const int m = (blockIdx.x - n_force_blocks) * 4 + wib;
+    // one CTA per molecule: thread-strided atoms, warp tree, then the warps in order (fixed tree)
+    __shared__ double wsum[FIN_WARPS];
+    const int m = blockIdx.x - n_force_blocks;
     if (m >= n_mol || energy == nullptr) return;
     double acc = 0.0;
-    for (int i = mol_off[m] + lane; i < mol_off[m + 1]; i += 32) {
+    for (int i = mol_off[m] + (int)threadIdx.x; i < mol_off[m + 1]; i += FIN_THREADS) {
       const double* e = eatom + (size_t)sortpos[i] * M;
       double s = 0.0;
       for (int k = 0; k < M; ++k) s += e[k];
@@ -456,7 +575,13 @@ __global__ void __launch_bounds__(128) finish_kernel(
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(FULL, acc, o);
-    if (lane == 0) energy[m] = escale * acc;
+    if (lane == 0) wsum[wib] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      double tot = 0.0;
+      for (int w = 0; w < FIN_WARPS; ++w) tot += wsum[w];
+      energy[m] = escale * tot;
+    }
   }
 }
 
@@ -471,38 +596,58 @@ void launch_neighbors(nnp_handle* h, const float* d_pos, int pos_stride, const i
                                              h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_status);
 }
 
+static bool aev_small_shape(const nnp_handle* h) { return h->aev.n_shf_z <= 4 && h->aev.n_shf_a <= 8; }
+
 void launch_aev_forward(nnp_handle* h, cudaStream_t s) {
   if (h->N == 0) return;
   const int blocks = h->N;
-  aev_forward_kernel<<<blocks, AEV_WARPS * 32, aev_smem_bytes(h, false), s>>>(
-      h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA,
-      h->d_aev);
+  const size_t smem = aev_smem_bytes(h, false);
+  if (aev_small_shape(h))
+    aev_forward_kernel<4, 8><<<blocks, AEV_THREADS, smem, s>>>(h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a,
+                                                               h->d_sortpos, h->N, h->aev, h->capR, h->capA,
+                                                               trip_chunk(h), h->d_aev);
+  else
+    aev_forward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A><<<blocks, AEV_THREADS, smem, s>>>(
+        h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA,
+        trip_chunk(h), h->d_aev);
 }
 
 void launch_aev_backward(nnp_handle* h, cudaStream_t s) {
   if (h->N == 0) return;
   const int blocks = h->N;
-  aev_backward_kernel<<<blocks, AEV_WARPS * 32, aev_smem_bytes(h, true), s>>>(
-      h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA,
-      h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
+  const size_t smem = aev_smem_bytes(h, true);
+  if (aev_small_shape(h))
+    aev_backward_kernel<4, 8><<<blocks, AEV_THREADS, smem, s>>>(
+        h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA,
+        trip_chunk(h), h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
+  else
+    aev_backward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A><<<blocks, AEV_THREADS, smem, s>>>(
+        h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA,
+        trip_chunk(h), h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
 }
 
 void launch_finish(nnp_handle* h, const int* d_atom_index, double* d_energy, float* d_force, int force_stride,
                    cudaStream_t s) {
   if (h->N == 0) return;
-  const int nfb = (h->N + 3) / 4;
-  const int neb = (h->n_mol + 3) / 4;
+  const int nfb = (h->N + FIN_WARPS - 1) / FIN_WARPS;
+  const int neb = h->n_mol;
   const float fscale = (float)(h->energy_scale * h->length_scale);
-  finish_kernel<<<nfb + neb, 128, 0, s>>>(h->d_nbr_r, h->d_cnt_r, h->d_phi, h->N, h->capR, d_atom_index, d_force,
+  finish_kernel<<<nfb + neb, FIN_THREADS, 0, s>>>(h->d_nbr_r, h->d_cnt_r, h->d_phi, h->N, h->capR, d_atom_index, d_force,
                                           force_stride, fscale, nfb, h->d_eatom, h->d_sortpos, h->d_species,
                                           h->d_mol_off, h->n_mol, h->M, h->d_self_energy, h->energy_scale,
                                           d_energy);
 }
 
 int aev_set_smem_attributes(nnp_handle* h) {
-  cudaError_t e1 = cudaFuncSetAttribute(aev_forward_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        (int)aev_smem_bytes(h, false));
-  cudaError_t e2 = cudaFuncSetAttribute(aev_backward_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        (int)aev_smem_bytes(h, true));
-  return (e1 == cudaSuccess && e2 == cudaSuccess) ? 0 : -1;
+  const int fb = (int)aev_smem_bytes(h, false), bb = (int)aev_smem_bytes(h, true);
+  cudaError_t e[4];
+  e[0] = cudaFuncSetAttribute(aev_forward_kernel<4, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, fb);
+  e[1] = cudaFuncSetAttribute(aev_forward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>,
+                              cudaFuncAttributeMaxDynamicSharedMemorySize, fb);
+  e[2] = cudaFuncSetAttribute(aev_backward_kernel<4, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, bb);
+  e[3] = cudaFuncSetAttribute(aev_backward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>,
+                              cudaFuncAttributeMaxDynamicSharedMemorySize, bb);
+  for (cudaError_t x : e)
+    if (x != cudaSuccess) return -1;
+  return 0;
 }
