@@ -174,7 +174,8 @@ struct UmmaParams {
   int stage_bytes;     // A_BOX_BYTES + b_box_bytes (raw and lo stages have the same layout)
   int n_raw;           // raw ring depth
   int slot_cols;       // TMEM columns per accumulator slot (= n_pad_max); cross accumulator at column 0
-  int gslots;          // slots (k-steps) per group = commit / drain granularity
+  int kps;             // k-steps (8 contraction elements each) accumulated in TMEM per slot: 1 or 4
+  int gslots;          // slots per group = commit / drain granularity
   int n_groups;        // slot-group ring depth
 };
 
@@ -197,7 +198,7 @@ __device__ __forceinline__ void drain_item(const UmmaItem& t, const UmmaParams& 
 #pragma unroll
     for (int j = 0; j < CT; ++j) part[j] = 0.0f;
   }
-  int ks_left = (t.kb1 - t.kb0) * 4;
+  int ks_left = ((t.kb1 - t.kb0) * 4 + P.kps - 1) / P.kps;  // slots of this item
   const uint32_t lane_base = tmem + ((uint32_t)(quarter * 32) << 16) + (uint32_t)col0;
   int in_part = 0;
   while (ks_left > 0) {
@@ -332,7 +333,7 @@ __global__ void __launch_bounds__(U_THREADS, 1) gemm_umma_kernel(const __grid_co
         const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)a_mn << 15) |
                                ((uint32_t)(t.n_pad >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
         mbar_wait(cross_empty, (item_ctr & 1u) ^ 1u);
-        int in_group = 0, ks_left = nb * 4;
+        int in_group = 0, in_slot = 0, ks_left = nb * 4;
         for (int b = 0; b < nb; ++b) {
           mbar_wait(&conv[ls], lphase);  // lo parts written (and, transitively, the raw stage has landed)
           tc_fence_after();
@@ -342,7 +343,7 @@ __global__ void __launch_bounds__(U_THREADS, 1) gemm_umma_kernel(const __grid_co
           const uint32_t sbl = sal + A_BOX_BYTES;
 #pragma unroll
           for (int ks = 0; ks < 4; ++ks) {
-            if (in_group == 0) {
+            if (in_group == 0 && in_slot == 0) {
               mbar_wait(&group_empty[grp], gphase ^ 1u);
               tc_fence_after();
             }
@@ -359,12 +360,15 @@ __global__ void __launch_bounds__(U_THREADS, 1) gemm_umma_kernel(const __grid_co
             const uint64_t bl = smem_desc(sbl + ks * 32, 16, 1024, 2);
             mma_tf32(d_x, al, bh, idesc, (b == 0 && ks == 0) ? 0u : 1u);
             mma_tf32(d_x, ah, bl, idesc, 1u);
-            mma_tf32(d_hi, ah, bh, idesc, 0u);
+            mma_tf32(d_hi, ah, bh, idesc, in_slot ? 1u : 0u);
             --ks_left;
-            if (++in_group == P.gslots || ks_left == 0) {
-              tc_commit(&group_full[grp]);
-              in_group = 0;
-              if (++grp == (uint32_t)P.n_groups) { grp = 0; gphase ^= 1u; }
+            if (++in_slot == P.kps || ks_left == 0) {
+              in_slot = 0;
+              if (++in_group == P.gslots || ks_left == 0) {
+                tc_commit(&group_full[grp]);
+                in_group = 0;
+                if (++grp == (uint32_t)P.n_groups) { grp = 0; gphase ^= 1u; }
+              }
             }
           }
           tc_commit(&raw_empty[rs]);  // frees the stages when these MMAs have read them
@@ -545,6 +549,10 @@ int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, cons
   P->n_raw = (int)std::min<size_t>(U_MAX_RAW, (UMMA_SMEM_BUDGET - 1024 - bar_bytes) / P->stage_bytes - U_LO_STAGES);
   L.smem_bytes = (size_t)(P->n_raw + U_LO_STAGES) * P->stage_bytes + bar_bytes + 1024;
   P->slot_cols = np_max;
+  {
+    const char* e = getenv("NNP_UMMA_KPS");  // experiment knob: k-steps accumulated in TMEM per slot
+    P->kps = (e && atoi(e) == 1) ? 1 : 4;
+  }
   P->gslots = std::max(1, std::min(4, 128 / np_max));
   P->n_groups = std::min(U_MAX_GROUPS, (512 - np_max) / (P->gslots * np_max));
   if (cudaMalloc((void**)&L.d_items, std::max<size_t>(1, n) * sizeof(UmmaItem)) != cudaSuccess) return -1;

@@ -84,6 +84,7 @@ extern "C" void nnp_destroy(nnp_handle* h) {
     for (auto& g : *v) umma_free_launch(g);
   for (auto* v : {&h->sfwd, &h->sbwd})
     for (auto& g : *v) small_free_launch(g);
+  small_free_launch(h->smid);
   delete h;
 }
 
@@ -539,7 +540,43 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   }
   if (h->use_small) {
     const float inv_alpha = 1.0f / alpha;
-    for (int l = 1; l < L; ++l) {  // forward
+    // layers 2..L-1, the 1-output layer and the backward pass down to delta_1 as ONE fused launch when the
+    // hidden layers are narrow enough for its register tiles
+    h->use_mid = !(cfg->flags & NNP_FLAG_NO_MID) && mid_init() == 0;
+    for (int e = 0; e < S && h->use_mid; ++e)
+      if (h->grp_off[e + 1] > h->grp_off[e] && !mid_supported(L, &h->dims[e * (L + 1)])) h->use_mid = false;
+    if (h->use_mid) {
+      std::vector<MidItem> items;
+      for (int e = 0; e < S; ++e) {
+        const int ne = h->grp_off[e + 1] - h->grp_off[e];
+        const int* d = &h->dims[e * (L + 1)];
+        for (int a0 = 0; a0 < ne; a0 += 4)
+          for (int m = 0; m < M; ++m) {
+            MidItem it;
+            memset(&it, 0, sizeof(it));
+            for (int l = 2; l <= L - 1; ++l) {
+              it.W[l] = h->d_W + h->w_off[e * L + l - 1] + (size_t)m * d[l] * d[l - 1];
+              it.bias[l] = h->d_b + h->b_off[e * L + l - 1] + (size_t)m * d[l];
+            }
+            for (int l = 1; l <= L - 1; ++l) it.H[l] = d[l];
+            it.w_last = h->d_W + h->w_off[e * L + L - 1] + (size_t)m * d[L - 1];
+            it.b_last = B[h->b_off[e * L + L - 1] + m];
+            it.h1 = h->d_act[1] + h->act_off[1][e] + (size_t)a0 * M * d[1] + (size_t)m * d[1];
+            it.ld1 = M * d[1];
+            it.e_out = h->d_eatom + (size_t)(h->grp_off[e] + a0) * M + m;
+            it.lde = M;
+            it.L = L;
+            it.n_atoms = std::min(4, ne - a0);
+            it.alpha = alpha; it.inv_alpha = inv_alpha;
+            items.push_back(it);
+          }
+      }
+      h->smid.name = "mlp_mid";
+      if (mid_build(h->smid, items)) { small_free_launch(h->smid); return fail(NNP_ERR_CUDA); }
+    }
+    const int l_fwd_end = h->use_mid ? 2 : L;   // forward layers run by the per-layer kernels: [1, l_fwd_end)
+    const int l_bwd_begin = h->use_mid ? 1 : L - 1;
+    for (int l = 1; l < l_fwd_end; ++l) {  // forward
       std::vector<SmallFwdItem> items;
       for (int e = 0; e < S; ++e) {
         const int ne = h->grp_off[e + 1] - h->grp_off[e];
@@ -577,7 +614,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       if (small_build_fwd(sl, items)) { small_free_launch(sl); return fail(NNP_ERR_CUDA); }
       h->sfwd.push_back(sl);
     }
-    for (int l = L - 1; l >= 1; --l) {  // backward
+    for (int l = l_bwd_begin; l >= 1; --l) {  // backward
       std::vector<SmallBwdItem> items;
       for (int e = 0; e < S; ++e) {
         const int ne = h->grp_off[e + 1] - h->grp_off[e];
@@ -608,7 +645,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
                 it.epi = EPI_SCALE;
                 it.scale = 1.0f / (float)M;
               }
-              if (l == L - 1) {
+              if (l == L - 1 && !h->use_mid) {
                 it.w_last = h->d_W + h->w_off[e * L + L - 1] + (size_t)m * nout;
                 it.b_last = B[h->b_off[e * L + L - 1] + m];
                 if (n0 == 0) {
@@ -654,9 +691,15 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   h->work[3] = w1bytes;
 
   h->stage_names = {"nbr", "aev_fwd"};
-  for (auto& g : h->fwd) h->stage_names.push_back(g.name);
-  if (!h->use_small) h->stage_names.push_back("mlp_last");
-  for (auto& g : h->bwd) h->stage_names.push_back(g.name);
+  if (h->use_small) {
+    for (auto& g : h->sfwd) h->stage_names.push_back(g.name);
+    if (h->use_mid) h->stage_names.push_back(h->smid.name);
+    for (auto& g : h->sbwd) h->stage_names.push_back(g.name);
+  } else {
+    for (auto& g : h->fwd) h->stage_names.push_back(g.name);
+    h->stage_names.push_back("mlp_last");
+    for (auto& g : h->bwd) h->stage_names.push_back(g.name);
+  }
   h->stage_names.push_back("aev_bwd");
   h->stage_names.push_back("finish");
   h->n_launches = N > 0 ? (int)h->stage_names.size() : 0;
@@ -681,6 +724,7 @@ static void enqueue_chain(nnp_handle* h, const float* d_pos, int ps, const int* 
   launch_aev_forward(h, s); mark();
   if (h->use_small) {  // per-atom energies and delta_L-1 come out of the first backward launch
     for (auto& g : h->sfwd) { small_launch_fwd(g, s); mark(); }
+    if (h->use_mid) { mid_launch(h->smid, s); mark(); }
     for (auto& g : h->sbwd) { small_launch_bwd(g, s); mark(); }
     launch_aev_backward(h, s); mark();
     launch_finish(h, d_idx, d_energy, d_force, fs, s); mark();

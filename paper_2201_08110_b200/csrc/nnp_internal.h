@@ -167,6 +167,23 @@ void small_launch_fwd(const SmallLaunch& L, cudaStream_t s);
 void small_launch_bwd(const SmallLaunch& L, cudaStream_t s);
 void small_free_launch(SmallLaunch& L);
 
+// ---- ligand-size engine, fused middle of the network (mlp_mid.cu): layers 2..L-1 forward, the final
+// 1-output layer + per-atom energies, and the backward pass down to delta_1, one CTA per item
+struct MidItem {
+  const float* W[NNP_MAX_LAYERS];     // W[l], l = 2..L-1: weights of layer l of this (element, model), [H_l][H_{l-1}]
+  const float* bias[NNP_MAX_LAYERS];  // bias[l] or null
+  const float* w_last;                // [H_{L-1}] weights of the 1-output layer L
+  float* h1;                          // in: h_1 of the item's first atom (model columns applied); out: delta_1
+  double* e_out;                      // e_out[a * lde] = b_L + w_L . h_{L-1}
+  int H[NNP_MAX_LAYERS];              // H[l], l = 1..L-1 (each <= 256, % 4 == 0)
+  int L, n_atoms, ld1, lde;           // n_atoms <= 4
+  float b_last, alpha, inv_alpha;
+};
+int mid_init();
+bool mid_supported(int L, const int* dims_of_element);  // dims: [L+1]
+int mid_build(SmallLaunch& L, std::vector<MidItem>& items);
+void mid_launch(const SmallLaunch& L, cudaStream_t s);
+
 // Final layer (1 output) + start of the backward pass.
 struct LastLayerArgs {
   float* act;          // [n_atoms_sorted][M][H] per element group (arena), overwritten with delta
@@ -215,7 +232,8 @@ struct nnp_handle {
   std::vector<TmaLaunch> tfwd, tbwd; // the same launches on the TMA+FFMA engine (used when use_tma)
   std::vector<UmmaLaunch> ufwd, ubwd; // the same launches on the tcgen05 engine (used when use_umma)
   std::vector<SmallLaunch> sfwd, sbwd; // ligand-size engine (used when use_small); no separate last-layer launch
-  bool use_tma = false, use_umma = false, use_small = false;
+  SmallLaunch smid;                    // fused middle launch of the ligand-size engine (used when use_mid)
+  bool use_tma = false, use_umma = false, use_small = false, use_mid = false;
   int n_parts = 1;                   // dE/dAEV is produced as n_parts partial sums (per model at small N)
   LastLayerArgs last;
   long long *d_last_act_off = nullptr, *d_last_w_off = nullptr, *d_last_b_off = nullptr;

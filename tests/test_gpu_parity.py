@@ -14,11 +14,12 @@ torch = pytest.importorskip("torch")
 
 from oracle.ani_oracle import AniOracle  # noqa: E402
 from paper_2201_08110_b200 import workloads as wl  # noqa: E402
-from paper_2201_08110_b200.binding import (NNP, NNP_FLAG_NO_GRAPH, NNP_FLAG_NO_SMALL, NNP_FLAG_NO_TMA,  # noqa: E402
-                                            NNP_FLAG_NO_UMMA, NNPError)
+from paper_2201_08110_b200.binding import (NNP, NNP_FLAG_NO_GRAPH, NNP_FLAG_NO_MID, NNP_FLAG_NO_SMALL,  # noqa: E402
+                                            NNP_FLAG_NO_TMA, NNP_FLAG_NO_UMMA, NNPError)
 
-# MLP engines: ligand-size weight-streaming FFMA (default at these sizes), tcgen05 3xTF32, TMA+FFMA, plain FFMA
-ENGINES = {"small": 0, "umma": NNP_FLAG_NO_SMALL, "tma": NNP_FLAG_NO_SMALL | NNP_FLAG_NO_UMMA,
+# MLP engines: ligand-size weight-streaming FFMA (default at these sizes; with the fused middle launch or
+# one launch per layer), tcgen05 3xTF32, TMA+FFMA, plain FFMA
+ENGINES = {"small": 0, "small_layers": NNP_FLAG_NO_MID, "umma": NNP_FLAG_NO_SMALL, "tma": NNP_FLAG_NO_SMALL | NNP_FLAG_NO_UMMA,
            "ffma": NNP_FLAG_NO_SMALL | NNP_FLAG_NO_UMMA | NNP_FLAG_NO_TMA}
 
 E_TOL_PER_ATOM = 1e-5  # kcal/mol
@@ -106,7 +107,7 @@ def test_config1_stagewise(engine):
     nnp.destroy()
 
 
-@pytest.mark.parametrize("engine", ["small", "umma"])
+@pytest.mark.parametrize("engine", ["small", "small_layers", "umma"])
 def test_config2_trajectory_steps(engine):
     """configs[1]: 50 atoms, 8 models, perturbed steps 0,1,10,100,999 of the 1000-step trajectory."""
     w = wl.config2()
@@ -223,7 +224,7 @@ def test_biases_self_energy_scales_and_embedding():
 
 @pytest.mark.parametrize("n_species,hidden,n,seed", [(3, (16, 12, 8), 37, 1), (2, (32, 20, 4), 70, 2),
                                                       (5, (64, 32, 16), 150, 3)])
-@pytest.mark.parametrize("engine", ["small", "umma"])
+@pytest.mark.parametrize("engine", ["small", "small_layers", "umma"])
 def test_small_parameter_sets(n_species, hidden, n, seed, engine):
     """Generic nnp_config (other species counts / layer widths): ragged tiles in every GEMM."""
     p = wl.small_params(n_species, hidden)
