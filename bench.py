@@ -162,7 +162,7 @@ def run_gpu(args):
     # collective, weak scaling); rank r starts at a different frame of the trajectory
     w = wl.get_config(args.config)
     W, B = w.weights()
-    nnp = NNP(w.params, W, B, w.species, w.mol_offsets)
+    nnp = NNP(w.params, W, B, w.species, w.mol_offsets, flags=args.flags)
     K, Wu = args.steps, args.warmup
     n_frames = min(K + Wu, 1000)
     traj_h = w.trajectory(n_frames)
@@ -331,6 +331,7 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cpu-steps", type=int, default=200)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--flags", type=int, default=0, help="NNP_FLAG_* bits (include/nnp.h) for A/B runs of the engines")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -19,6 +19,7 @@ NNP_FLAG_NO_TMA = 2
 NNP_FLAG_NO_UMMA = 4
 NNP_FLAG_NO_SMALL = 8
 NNP_FLAG_NO_MID = 16
+NNP_FLAG_NO_PDL = 32
 ERRORS = {
     -1: "NNP_ERR_INVALID_ARG",
     -2: "NNP_ERR_CUDA",

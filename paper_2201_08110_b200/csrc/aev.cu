@@ -25,6 +25,8 @@ __global__ void __launch_bounds__(128) nbr_allpairs_kernel(
     int* __restrict__ cnt_r, int* __restrict__ cnt_a, int* __restrict__ status) {
   const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
+  pdl_trigger();
+  pdl_wait();  // the previous step's kernels still read the lists this kernel rewrites
   if (i >= N) return;
   const int m = mol_id[i];
   const int lo = mol_off[m], hi = mol_off[m + 1];
@@ -269,6 +271,8 @@ __global__ void __launch_bounds__(AEV_THREADS) aev_forward_kernel(
   float* row = t.rest;                 // [n_ang]
   float* bF1 = row + n_ang;            // [n_shf_z][CH]
   float* bF2 = bF1 + c.n_shf_z * CH;   // [n_shf_a][CH]
+  pdl_trigger();
+  pdl_wait();
   const float4 pi = pos4[i];
   const int nr = cnt_r[i], na = cnt_a[i];
   for (int f = threadIdx.x; f < n_ang; f += blockDim.x) row[f] = 0.0f;
@@ -372,6 +376,8 @@ __global__ void __launch_bounds__(AEV_THREADS) aev_backward_kernel(
   float* phr = gang + n_pairs * bpad;   // radial part   [capR][3]
   float* pha = phr + 3 * capR;          // angular part  [capR][3]
   float* buf = pha + 3 * capR;          // [6][CH] pair gradients of the triplets of a pass
+  pdl_trigger();
+  pdl_wait();
   const float4 pi = pos4[i];
   const int nr = cnt_r[i], na = cnt_a[i];
   const float* gin = daev + (size_t)sortpos[i] * c.n_feat;
@@ -530,6 +536,8 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(
     const double* __restrict__ self_energy, double escale, double* __restrict__ energy) {
   const int lane = threadIdx.x & 31;
   const int wib = threadIdx.x >> 5;
+  pdl_trigger();
+  pdl_wait();
   if ((int)blockIdx.x < n_force_blocks) {
     const int a = blockIdx.x * FIN_WARPS + wib;
     if (a >= N || force == nullptr) return;
@@ -603,13 +611,13 @@ void launch_aev_forward(nnp_handle* h, cudaStream_t s) {
   const int blocks = h->N;
   const size_t smem = aev_smem_bytes(h, false);
   if (aev_small_shape(h))
-    aev_forward_kernel<4, 8><<<blocks, AEV_THREADS, smem, s>>>(h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a,
-                                                               h->d_sortpos, h->N, h->aev, h->capR, h->capA,
-                                                               trip_chunk(h), h->d_aev);
+    launch_kernel(h->pdl_now, aev_forward_kernel<4, 8>, dim3(blocks), dim3(AEV_THREADS), smem, s, h->d_pos4, h->d_nbr_r,
+                  h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA, trip_chunk(h),
+                  h->d_aev);
   else
-    aev_forward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A><<<blocks, AEV_THREADS, smem, s>>>(
-        h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA,
-        trip_chunk(h), h->d_aev);
+    launch_kernel(h->pdl_now, aev_forward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>, dim3(blocks), dim3(AEV_THREADS), smem, s,
+                  h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR,
+                  h->capA, trip_chunk(h), h->d_aev);
 }
 
 void launch_aev_backward(nnp_handle* h, cudaStream_t s) {
@@ -617,13 +625,13 @@ void launch_aev_backward(nnp_handle* h, cudaStream_t s) {
   const int blocks = h->N;
   const size_t smem = aev_smem_bytes(h, true);
   if (aev_small_shape(h))
-    aev_backward_kernel<4, 8><<<blocks, AEV_THREADS, smem, s>>>(
-        h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA,
-        trip_chunk(h), h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
+    launch_kernel(h->pdl_now, aev_backward_kernel<4, 8>, dim3(blocks), dim3(AEV_THREADS), smem, s, h->d_pos4,
+                  h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA,
+                  trip_chunk(h), (const float*)h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
   else
-    aev_backward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A><<<blocks, AEV_THREADS, smem, s>>>(
-        h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA,
-        trip_chunk(h), h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
+    launch_kernel(h->pdl_now, aev_backward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>, dim3(blocks), dim3(AEV_THREADS), smem, s,
+                  h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR,
+                  h->capA, trip_chunk(h), (const float*)h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
 }
 
 void launch_finish(nnp_handle* h, const int* d_atom_index, double* d_energy, float* d_force, int force_stride,
@@ -632,10 +640,9 @@ void launch_finish(nnp_handle* h, const int* d_atom_index, double* d_energy, flo
   const int nfb = (h->N + FIN_WARPS - 1) / FIN_WARPS;
   const int neb = h->n_mol;
   const float fscale = (float)(h->energy_scale * h->length_scale);
-  finish_kernel<<<nfb + neb, FIN_THREADS, 0, s>>>(h->d_nbr_r, h->d_cnt_r, h->d_phi, h->N, h->capR, d_atom_index, d_force,
-                                          force_stride, fscale, nfb, h->d_eatom, h->d_sortpos, h->d_species,
-                                          h->d_mol_off, h->n_mol, h->M, h->d_self_energy, h->energy_scale,
-                                          d_energy);
+  launch_kernel(h->pdl_now, finish_kernel, dim3(nfb + neb), dim3(FIN_THREADS), 0, s, h->d_nbr_r, h->d_cnt_r, h->d_phi,
+                h->N, h->capR, d_atom_index, d_force, force_stride, fscale, nfb, h->d_eatom, h->d_sortpos, h->d_species,
+                h->d_mol_off, h->n_mol, h->M, h->d_self_energy, h->energy_scale, d_energy);
 }
 
 int aev_set_smem_attributes(nnp_handle* h) {

@@ -8,13 +8,13 @@
 // <= 4 atoms) and walks h_1 -> h_2 -> ... -> h_{L-1} -> e, delta_{L-1} -> ... -> delta_1 with every
 // activation in shared memory / registers.  The weights do not depend on the data, so a producer warp
 // streams them (forward layers, then the same matrices again for the backward pass) as 1-D bulk async
-// copies of <= 32 row tiles through a deep shared-memory ring: the copy of tile t+5 is in flight while
+// copies of <= 32 row tiles through a deep shared-memory ring: the copies of the next few tiles are in flight while
 // tile t is consumed, across layer boundaries, so the only exposed latency is that of the first tile.
 //
-//   forward tile (rows = output features):  a warp owns 4 rows; lanes split the contraction (x of the 4
-//       atoms in registers), 16 partial sums are reduced by a 16-shuffle transposing butterfly (fixed order);
-//   backward tile (rows = contraction index o): a warp owns 4 rows, lanes own 4 consecutive input columns,
-//       accumulators stay in registers over all tiles of the layer; the 8 warps are summed in a fixed order
+//   forward tile (rows = output features):  a warp owns 2 rows; lanes split the contraction (x of the 4
+//       atoms in registers), 8 partial sums are reduced by a 9-shuffle transposing butterfly (fixed order);
+//   backward tile (rows = contraction index o): a warp owns 2 rows, lanes own 4 consecutive input columns,
+//       accumulators stay in registers over all tiles of the layer; the 16 warps are summed in a fixed order
 //       through shared memory, multiplied by CELU'(h) and become the next delta.
 #include <algorithm>
 
@@ -22,10 +22,11 @@
 
 namespace {
 
-constexpr int MID_CONSUMERS = 256;               // 8 consumer warps
+constexpr int MID_CONSUMERS = 512;               // 16 consumer warps
 constexpr int MID_THREADS = MID_CONSUMERS + 32;  // + 1 producer warp
 constexpr int MID_WARPS = MID_CONSUMERS / 32;
-constexpr int MID_TILE_ROWS = 32;                // 4 rows per consumer warp
+constexpr int MID_TILE_ROWS = 32;                // 2 rows per consumer warp
+constexpr int MID_RW = 2;
 constexpr int MID_AC = 4;                        // atoms per CTA
 constexpr int MID_NJ = 2;                        // float4 per lane along a row: rows of <= 256 floats
 constexpr int MID_HMAX = 128 * MID_NJ;
@@ -71,7 +72,16 @@ __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t b
 }
 __device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, %0;" ::"n"(MID_CONSUMERS) : "memory"); }
 
+#ifdef NNP_MID_TRACE
+__device__ long long g_mid_trace[256];
+#define TR(k) do { if (blockIdx.x == 0 && threadIdx.x == 0 && (k) < 256) g_mid_trace[(k)] = clock64(); } while (0)
+#else
+#define TR(k)
+#endif
 }  // namespace
+#ifdef NNP_MID_TRACE
+extern "C" int nnp_debug_mid_trace(long long* out) { return (int)cudaMemcpyFromSymbol(out, g_mid_trace, sizeof(long long) * 256); }
+#endif
 
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem* __restrict__ items, int n_stages) {
@@ -81,6 +91,7 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
   __shared__ MidItem it;
   constexpr int TILE_FLOATS = MID_TILE_ROWS * MID_HMAX;
   constexpr int AH = MID_AC * MID_HMAX;  // floats of one activation / delta buffer
+  TR(0);
   {
     const int* src = reinterpret_cast<const int*>(items + blockIdx.x);
     int* dst = reinterpret_cast<int*>(&it);
@@ -94,6 +105,7 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
+  pdl_trigger();
   float* ring = reinterpret_cast<float*>(mid_smem);
   const int L = it.L;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -132,6 +144,7 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
       for (int r = tid; r < it.H[l]; r += MID_CONSUMERS) bs[l * MID_HMAX + r] = it.bias[l] ? __ldg(it.bias[l] + r) : 0.0f;
     for (int o = tid; o < it.H[L - 1]; o += MID_CONSUMERS) bs[L * MID_HMAX + o] = __ldg(it.w_last + o);
   }
+  pdl_wait();  // h_1 comes from the layer-1 kernel; the weight ring (constant data) is already filling
   {  // h_1 of the chunk (rows of padding atoms are zero)
     const int K4 = it.H[1] >> 2;
     for (int idx = tid; idx < MID_AC * K4; idx += MID_CONSUMERS) {
@@ -141,7 +154,10 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
       reinterpret_cast<float4*>(hs + a * MID_HMAX)[k4] = v;
     }
   }
+  TR(1);
   consumer_sync();
+  TR(2);
+  int trk = 3;
 
   // ---- forward, layers 2..L-1
   for (int l = 2; l <= L - 1; ++l) {
@@ -158,14 +174,16 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
         x[a][j] = k4 < K4 ? reinterpret_cast<const float4*>(hin + a * MID_HMAX)[k4] : make_float4(0.f, 0.f, 0.f, 0.f);
       }
     for (int r0 = 0; r0 < R; r0 += MID_TILE_ROWS) {
+      TR(trk); ++trk;
       mb_wait(&full[slot], phase);
+      TR(trk); ++trk;
       const float4* tile = reinterpret_cast<const float4*>(ring + (size_t)slot * TILE_FLOATS);
-      float s[16];
+      float s[8];
 #pragma unroll
-      for (int q = 0; q < 16; ++q) s[q] = 0.0f;
+      for (int q = 0; q < 8; ++q) s[q] = 0.0f;
 #pragma unroll
-      for (int rr = 0; rr < 4; ++rr) {
-        const int r = warp * 4 + rr;
+      for (int rr = 0; rr < MID_RW; ++rr) {
+        const int r = warp * MID_RW + rr;
         if (r0 + r < R) {
 #pragma unroll
           for (int j = 0; j < MID_NJ; ++j) {
@@ -181,45 +199,40 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
       __syncwarp();
       if (lane == 0) mb_arrive(&empty[slot]);
       if (++slot == (uint32_t)n_stages) { slot = 0; phase ^= 1u; }
-      // transposing butterfly: 16 sums over 32 lanes, 16 shuffles, fixed order
+      // transposing butterfly: 8 sums over 32 lanes, 9 shuffles, fixed order
 #pragma unroll
-      for (int q = 0; q < 8; ++q) {
+      for (int q = 0; q < 4; ++q) {
         const bool up = lane & 16;
-        const float send = up ? s[q] : s[q + 8];
-        const float keep = up ? s[q + 8] : s[q];
+        const float send = up ? s[q] : s[q + 4];
+        const float keep = up ? s[q + 4] : s[q];
         s[q] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
       }
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const bool up = lane & 8;
-        const float send = up ? s[q] : s[q + 4];
-        const float keep = up ? s[q + 4] : s[q];
-        s[q] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-      }
-#pragma unroll
       for (int q = 0; q < 2; ++q) {
-        const bool up = lane & 4;
+        const bool up = lane & 8;
         const float send = up ? s[q] : s[q + 2];
         const float keep = up ? s[q + 2] : s[q];
-        s[q] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+        s[q] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
       }
       {
-        const bool up = lane & 2;
+        const bool up = lane & 4;
         const float send = up ? s[0] : s[1];
         const float keep = up ? s[1] : s[0];
-        s[0] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
+        s[0] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
       }
+      s[0] += __shfl_xor_sync(0xffffffffu, s[0], 2);
       s[0] += __shfl_xor_sync(0xffffffffu, s[0], 1);
-      if ((lane & 1) == 0) {
-        const int q = ((lane >> 4) & 1) * 8 + ((lane >> 3) & 1) * 4 + ((lane >> 2) & 1) * 2 + ((lane >> 1) & 1);
+      if ((lane & 3) == 0) {
+        const int q = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
         const int rr = q >> 2, a = q & 3;
-        const int r = r0 + warp * 4 + rr;
+        const int r = r0 + warp * MID_RW + rr;
         if (r < R) hout[a * MID_HMAX + r] = celu_m(s[0] + bias[r], it.alpha, it.inv_alpha);
       }
     }
     consumer_sync();
   }
 
+  TR(trk); ++trk;
   // ---- layer L (1 output): per-atom energies (FP64) and delta_{L-1} = w_L (.) CELU'(h_{L-1})
   float* dcur = dbuf;
   float* dnext = dbuf + AH;
@@ -240,6 +253,7 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
   }
   consumer_sync();
 
+  TR(trk); ++trk;
   // ---- backward through layers L-1..2: delta_{l-1} = (delta_l W_l) (.) CELU'(h_{l-1})
   for (int l = L - 1; l >= 2; --l) {
     const int R = it.H[l], N4 = it.H[l - 1] >> 2;
@@ -249,26 +263,25 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
 #pragma unroll
       for (int j = 0; j < MID_NJ; ++j) acc[a][j] = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int o0 = 0; o0 < R; o0 += MID_TILE_ROWS) {
+      TR(trk); ++trk;
       mb_wait(&full[slot], phase);
+      TR(trk); ++trk;
       const float4* tile = reinterpret_cast<const float4*>(ring + (size_t)slot * TILE_FLOATS);
-      const int ow = o0 + warp * 4;  // R % 4 == 0: the warp's four rows are valid together
+      const int ow = o0 + warp * MID_RW;  // R % 4 == 0: the warp's two rows are valid together
       if (ow < R) {
-        float4 d[MID_AC];
+        float2 d[MID_AC];
 #pragma unroll
-        for (int a = 0; a < MID_AC; ++a) d[a] = *reinterpret_cast<const float4*>(dcur + a * MID_HMAX + ow);
+        for (int a = 0; a < MID_AC; ++a) d[a] = *reinterpret_cast<const float2*>(dcur + a * MID_HMAX + ow);
 #pragma unroll
         for (int j = 0; j < MID_NJ; ++j) {
           const int n4 = lane + 32 * j;
           if (n4 < N4) {
-            const float4 w0 = tile[(warp * 4 + 0) * N4 + n4], w1 = tile[(warp * 4 + 1) * N4 + n4];
-            const float4 w2 = tile[(warp * 4 + 2) * N4 + n4], w3 = tile[(warp * 4 + 3) * N4 + n4];
+            const float4 w0 = tile[(warp * MID_RW + 0) * N4 + n4], w1 = tile[(warp * MID_RW + 1) * N4 + n4];
 #pragma unroll
             for (int a = 0; a < MID_AC; ++a) {
               float4 v = acc[a][j];
               v.x = fmaf(d[a].x, w0.x, v.x); v.y = fmaf(d[a].x, w0.y, v.y); v.z = fmaf(d[a].x, w0.z, v.z); v.w = fmaf(d[a].x, w0.w, v.w);
               v.x = fmaf(d[a].y, w1.x, v.x); v.y = fmaf(d[a].y, w1.y, v.y); v.z = fmaf(d[a].y, w1.z, v.z); v.w = fmaf(d[a].y, w1.w, v.w);
-              v.x = fmaf(d[a].z, w2.x, v.x); v.y = fmaf(d[a].z, w2.y, v.y); v.z = fmaf(d[a].z, w2.z, v.z); v.w = fmaf(d[a].z, w2.w, v.w);
-              v.x = fmaf(d[a].w, w3.x, v.x); v.y = fmaf(d[a].w, w3.y, v.y); v.z = fmaf(d[a].w, w3.z, v.z); v.w = fmaf(d[a].w, w3.w, v.w);
               acc[a][j] = v;
             }
           }
@@ -307,7 +320,10 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
     }
     consumer_sync();
     float* tmp = dcur; dcur = dnext; dnext = tmp;
+    TR(trk); ++trk;
   }
+  TR(trk); ++trk;
+  TR(255);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -354,7 +370,8 @@ int mid_build(SmallLaunch& L, std::vector<MidItem>& items) {
   return 0;
 }
 
-void mid_launch(const SmallLaunch& L, cudaStream_t s) {
+void mid_launch(const SmallLaunch& L, cudaStream_t s, bool pdl) {
   if (L.n_items == 0) return;
-  small_mid_kernel<<<L.n_items, MID_THREADS, L.smem_bytes, s>>>(reinterpret_cast<const MidItem*>(L.d_items), L.variant);
+  launch_kernel(pdl, small_mid_kernel, dim3(L.n_items), dim3(MID_THREADS), L.smem_bytes, s,
+                reinterpret_cast<const MidItem*>(L.d_items), L.variant);
 }

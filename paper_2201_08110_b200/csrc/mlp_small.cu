@@ -113,7 +113,8 @@ __global__ void __launch_bounds__(SM_THREADS, 2) small_fwd_kernel(const SmallFwd
     }
   };
   int r = 2 * warp;
-  if (r < it.n_rows) load_rows(r);
+  pdl_trigger();
+  if (r < it.n_rows) load_rows(r);  // weights: constant data, in flight before the producer of X has finished
   // X rows (contiguous K floats per atom) arrive by bulk async copies, all in flight at once
   if (threadIdx.x == 0) {
     sbar_init(&xbar, 1);
@@ -121,6 +122,7 @@ __global__ void __launch_bounds__(SM_THREADS, 2) small_fwd_kernel(const SmallFwd
     sbar_expect_tx(&xbar, (uint32_t)(it.n_atoms * it.K * 4));
   }
   __syncthreads();
+  pdl_wait();
   if (threadIdx.x < it.n_atoms)
     bulk_g2s(smem_f + (size_t)threadIdx.x * it.K, it.X + (size_t)threadIdx.x * it.ldx, (uint32_t)(it.K * 4), &xbar);
   sbar_wait(&xbar, 0);
@@ -191,8 +193,10 @@ __device__ __forceinline__ void small_bwd_body(const SmallBwdItem& it, float* sm
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
+  pdl_trigger();
   for (int o = threadIdx.x; o < it.n_out; o += SM_THREADS)
     bulk_g2s(ws + (size_t)o * 128, it.W + (size_t)o * it.ldw, (uint32_t)(it.n_cols * 4), &bars[o / rpg]);
+  pdl_wait();  // delta / activations come from the previous kernel
   if (!it.w_last) {
     if (threadIdx.x < it.n_atoms)
       bulk_g2s(ds + (size_t)threadIdx.x * it.n_out, it.D + (size_t)threadIdx.x * it.ldd, (uint32_t)(it.n_out * 4), dbar);
@@ -375,20 +379,22 @@ int small_build_bwd(SmallLaunch& L, std::vector<SmallBwdItem>& items) {
   return 0;
 }
 
-void small_launch_fwd(const SmallLaunch& L, cudaStream_t s) {
+void small_launch_fwd(const SmallLaunch& L, cudaStream_t s, bool pdl) {
   if (L.n_items == 0) return;
   const SmallFwdItem* it = reinterpret_cast<const SmallFwdItem*>(L.d_items);
+  const dim3 g(L.n_items), b(SM_THREADS);
   switch (L.variant) {
-    case 1: small_fwd_kernel<1><<<L.n_items, SM_THREADS, L.smem_bytes, s>>>(it); break;
-    case 2: small_fwd_kernel<2><<<L.n_items, SM_THREADS, L.smem_bytes, s>>>(it); break;
-    case 4: small_fwd_kernel<4><<<L.n_items, SM_THREADS, L.smem_bytes, s>>>(it); break;
-    default: small_fwd_kernel<8><<<L.n_items, SM_THREADS, L.smem_bytes, s>>>(it); break;
+    case 1: launch_kernel(pdl, small_fwd_kernel<1>, g, b, L.smem_bytes, s, it); break;
+    case 2: launch_kernel(pdl, small_fwd_kernel<2>, g, b, L.smem_bytes, s, it); break;
+    case 4: launch_kernel(pdl, small_fwd_kernel<4>, g, b, L.smem_bytes, s, it); break;
+    default: launch_kernel(pdl, small_fwd_kernel<8>, g, b, L.smem_bytes, s, it); break;
   }
 }
 
-void small_launch_bwd(const SmallLaunch& L, cudaStream_t s) {
+void small_launch_bwd(const SmallLaunch& L, cudaStream_t s, bool pdl) {
   if (L.n_items == 0) return;
-  small_bwd_kernel<<<L.n_items, SM_THREADS, L.smem_bytes, s>>>(reinterpret_cast<const SmallBwdItem*>(L.d_items));
+  launch_kernel(pdl, small_bwd_kernel, dim3(L.n_items), dim3(SM_THREADS), L.smem_bytes, s,
+                reinterpret_cast<const SmallBwdItem*>(L.d_items));
 }
 
 void small_free_launch(SmallLaunch& L) {

@@ -137,6 +137,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   h->device = dev;
   h->N = n_atoms; h->n_mol = n_molecules; h->S = S; h->M = M; h->L = L; h->n_feat = n_feat;
   h->flags = cfg->flags;
+  h->use_pdl = !(cfg->flags & NNP_FLAG_NO_PDL);
   h->energy_scale = cfg->energy_scale;
   h->length_scale = cfg->length_scale;
   h->dims.assign(cfg->layer_dims, cfg->layer_dims + (size_t)S * (L + 1));
@@ -719,13 +720,15 @@ static void enqueue_chain(nnp_handle* h, const float* d_pos, int ps, const int* 
     if (ev) cudaEventRecord(h->events[k], s);
     ++k;
   };
+  h->pdl_now = h->use_pdl && !ev;  // event records between the kernels would break the programmatic edges
+  const bool pdl = h->pdl_now;
   mark();
   launch_neighbors(h, d_pos, ps, d_idx, s); mark();
   launch_aev_forward(h, s); mark();
   if (h->use_small) {  // per-atom energies and delta_L-1 come out of the first backward launch
-    for (auto& g : h->sfwd) { small_launch_fwd(g, s); mark(); }
-    if (h->use_mid) { mid_launch(h->smid, s); mark(); }
-    for (auto& g : h->sbwd) { small_launch_bwd(g, s); mark(); }
+    for (auto& g : h->sfwd) { small_launch_fwd(g, s, pdl); mark(); }
+    if (h->use_mid) { mid_launch(h->smid, s, pdl); mark(); }
+    for (auto& g : h->sbwd) { small_launch_bwd(g, s, pdl); mark(); }
     launch_aev_backward(h, s); mark();
     launch_finish(h, d_idx, d_energy, d_force, fs, s); mark();
     return;

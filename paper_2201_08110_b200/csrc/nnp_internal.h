@@ -20,6 +20,32 @@
 #define NNP_ST_CAPACITY 1
 #define NNP_ST_NONFINITE 2
 
+// ---- programmatic dependent launch (PDL): a kernel launched with the attribute may start while its
+// predecessor in the stream is still running; everything it does before pdl_wait() must touch only data that is
+// constant after nnp_create (items, weights, topology).  pdl_wait() returns when the predecessor grid has
+// completed and its writes are visible; pdl_trigger() lets the successor start launching.  Both are no-ops for
+// plain launches.  Every CTA of every kernel in the chain calls pdl_wait() (completion is then transitive).
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_kernel(bool pdl, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s,
+                                 Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+#endif
+
 // AEV constants, passed by value to kernels.
 struct AevConst {
   int S, n_shf_r, n_shf_a, n_shf_z, n_sub, n_radial, n_feat;
@@ -163,8 +189,8 @@ int small_init();
 void small_bwd_shape(int n_atoms, int* AW, int* G);
 int small_build_fwd(SmallLaunch& L, std::vector<SmallFwdItem>& items);
 int small_build_bwd(SmallLaunch& L, std::vector<SmallBwdItem>& items);
-void small_launch_fwd(const SmallLaunch& L, cudaStream_t s);
-void small_launch_bwd(const SmallLaunch& L, cudaStream_t s);
+void small_launch_fwd(const SmallLaunch& L, cudaStream_t s, bool pdl);
+void small_launch_bwd(const SmallLaunch& L, cudaStream_t s, bool pdl);
 void small_free_launch(SmallLaunch& L);
 
 // ---- ligand-size engine, fused middle of the network (mlp_mid.cu): layers 2..L-1 forward, the final
@@ -182,7 +208,7 @@ struct MidItem {
 int mid_init();
 bool mid_supported(int L, const int* dims_of_element);  // dims: [L+1]
 int mid_build(SmallLaunch& L, std::vector<MidItem>& items);
-void mid_launch(const SmallLaunch& L, cudaStream_t s);
+void mid_launch(const SmallLaunch& L, cudaStream_t s, bool pdl);
 
 // Final layer (1 output) + start of the backward pass.
 struct LastLayerArgs {
@@ -234,6 +260,7 @@ struct nnp_handle {
   std::vector<SmallLaunch> sfwd, sbwd; // ligand-size engine (used when use_small); no separate last-layer launch
   SmallLaunch smid;                    // fused middle launch of the ligand-size engine (used when use_mid)
   bool use_tma = false, use_umma = false, use_small = false, use_mid = false;
+  bool use_pdl = false, pdl_now = false;  // programmatic dependent launches along the chain (pdl_now: this enqueue)
   int n_parts = 1;                   // dE/dAEV is produced as n_parts partial sums (per model at small N)
   LastLayerArgs last;
   long long *d_last_act_off = nullptr, *d_last_w_off = nullptr, *d_last_b_off = nullptr;
