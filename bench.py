@@ -24,6 +24,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+from paper_2201_08110_b200 import multi  # noqa: E402
 from paper_2201_08110_b200 import workloads as wl  # noqa: E402
 
 METRIC = "ANI-2x energy+force atom-evals/sec (50-atom, 8-model ligand; us/step and % of roofline in extra keys)"
@@ -42,12 +43,12 @@ def workload_config(w, extra=None):
     return cfg
 
 
-def ncu_traffic_bytes(config: int):
-    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed
-    `ncu --set full` summary (profiles/top_kernel_traffic.txt, lines `config<C>_dram_bytes=<n>`); None if absent."""
+def ncu_traffic_bytes(config: int, stage: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of a kernel, per launch, from the committed `ncu --set full`
+    summaries (profiles/top_kernel_traffic.txt, lines `config<C>_<stage>_dram_bytes=<n>`); None if absent."""
     try:
         for line in open(os.path.join(ROOT, "profiles", "top_kernel_traffic.txt")):
-            if line.startswith(f"config{config}_dram_bytes="):
+            if line.startswith(f"config{config}_{stage}_dram_bytes="):
                 return float(line.split("=", 1)[1])
     except OSError:
         pass
@@ -70,7 +71,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100", "-i",
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "20", "-i",
                  str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -79,9 +80,16 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.lines.append(line.strip())
+            self.lines.append((time.perf_counter(), line.strip()))
 
-    def stop(self):
+    def wait_first_sample(self, timeout=10.0):
+        t0 = time.perf_counter()
+        while self.proc is not None and not self.lines and time.perf_counter() - t0 < timeout:
+            time.sleep(0.01)
+
+    def stop(self, t_begin=None, t_end=None):
+        """Summary of the samples taken in [t_begin, t_end] (perf_counter times); if the window is shorter than
+        the sampling period, the samples of the whole loaded run are used and `window` says so."""
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
@@ -89,9 +97,14 @@ class ClockSampler:
             self.proc.wait(timeout=5)
         except Exception:
             self.proc.kill()
+        window = "timed region"
+        lines = [ln for t, ln in self.lines if (t_begin is None or t >= t_begin) and (t_end is None or t <= t_end)]
+        if not lines:
+            window = "whole run under load (timed region shorter than the sampling period)"
+            lines = [ln for _, ln in self.lines]
         sm, mx, reasons = [], [], set()
         names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
-        for ln in self.lines:
+        for ln in lines:
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 7:
                 continue
@@ -104,7 +117,84 @@ class ClockSampler:
                 if v.lower().startswith("active"):
                     reasons.add(n)
         return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "samples": len(sm), "reasons": sorted(reasons)}
+                "samples": len(sm), "window": window, "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+KERNEL_OF_STAGE = {  # ligand-size engine / tensor-core engine
+    "ligand": {"mlp_fwd_l1": "small_fwd_kernel", "mlp_mid": "small_mid_kernel", "mlp_bwd_l1": "small_bwd1_kernel"},
+    "tensor": {"mlp_fwd_l1": "gemm_umma_kernel", "mlp_fwd_l2": "gemm_umma_kernel", "mlp_fwd_l3": "gemm_umma_kernel",
+               "mlp_bwd_l3": "gemm_umma_kernel", "mlp_bwd_l2": "gemm_umma_kernel", "mlp_bwd_l1": "gemm_umma_kernel"},
+}
+
+
+def stage_rooflines(w, nnp, stages, config):
+    """Roofline of the dominant MLP kernel (and, under "kernels", of every MLP launch) from the live CUDA-event
+    stage times.  Algorithmic work per launch: a layer GEMM does 2 flop per weight per
+    atom-model; the ligand-size layer-1 forward must stream the layer-1 weights of the ensemble once (HBM-bound
+    when L2 was flushed); FP32 peak = SMs x 128 lanes x 2 flop x max SM clock; TF32 tensor peak = measured bf16
+    peak x 0.5 (nominal ratio), against which 3xTF32 can reach at most 1/3."""
+    import torch
+
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        peaks = {}
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    hbm_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+    bf16 = float(peaks.get("bf16_tflops", 1650.0))
+    sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    n_sm = torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count
+    fp32_peak = n_sm * 128 * 2 * sm_mhz * 1e6 / 1e12  # TFLOP/s
+    p = w.params
+    dims = np.asarray(p.layer_dims, dtype=np.int64)  # [S][L+1]
+    L = dims.shape[1] - 1
+    counts = np.bincount(w.species, minlength=dims.shape[0]).astype(np.int64)
+    M = w.n_models
+    mac = {l: int((counts * dims[:, l - 1] * dims[:, l]).sum()) * M for l in range(1, L + 1)}  # per pass
+    w1_bytes = int(((counts > 0) * dims[:, 0] * dims[:, 1]).sum()) * M * 4
+    engine = "ligand" if "mlp_mid" in stages or "mlp_last" not in stages else "tensor"
+    out = []
+
+    def add(stage, bound, work, unit, peak, src, note=None):
+        if stage not in stages or stages[stage] <= 0:
+            return
+        achieved = work / (stages[stage] * 1e-6) / (1e9 if unit == "GB/s" else 1e12)
+        d = {"stage": stage, "kernel": KERNEL_OF_STAGE[engine].get(stage, stage), "bound": bound,
+             "achieved": achieved, "peak": peak, "unit": unit, "frac": achieved / peak, "kernel_us": stages[stage],
+             "algorithmic_work": work, "peak_source": src}
+        if note:
+            d["note"] = note
+        out.append(d)
+
+    alu_src = f"derived: {n_sm} SMs x 128 FP32 lanes x 2 flop x {sm_mhz:.0f} MHz"
+    if engine == "ligand":
+        add("mlp_fwd_l1", "hbm", w1_bytes + w.n_atoms * nnp.n_features * 4, "GB/s", hbm_peak, hbm_src,
+            "layer-1 weights of the ensemble streamed once + AEV rows; L2 flushed before the step")
+        add("mlp_bwd_l1", "alu", 2.0 * mac[1], "TFLOP/s", fp32_peak, alu_src,
+            "weights re-read from L2 (resident after the forward pass); FFMA2 on the CUDA cores")
+        add("mlp_mid", "alu", 4.0 * sum(mac[l] for l in range(2, L)) + 4.0 * mac[L], "TFLOP/s", fp32_peak, alu_src,
+            "layers 2..L-1 forward+backward and the 1-output layer, one CTA per (element, model, 4 atoms)")
+    else:
+        tf32_peak = 0.5 * bf16
+        tsrc = "measured bf16 (MEASURED_PEAKS.json bf16_tflops) x 0.5 nominal TF32:BF16 ratio" if "bf16_tflops" in peaks \
+            else "fallback 1650 TFLOP/s bf16 x 0.5"
+        for l in range(1, L):
+            for st in (f"mlp_fwd_l{l}", f"mlp_bwd_l{l}"):
+                add(st, "tensor", 2.0 * mac[l], "TFLOP/s", tf32_peak, tsrc,
+                    "useful flops; 3xTF32 issues 3 MMAs per useful MAC, so the ceiling of frac is 1/3")
+    if not out:
+        return None
+    top = max(out, key=lambda d: d["kernel_us"])
+    roof = {k: top[k] for k in ("bound", "achieved", "peak", "unit", "frac")}
+    roof["kernel"] = f'{top["kernel"]} ({top["stage"]})'
+    roof["traffic"] = ncu_traffic_bytes(config, top["stage"])
+    roof.update({k: top[k] for k in ("kernel_us", "algorithmic_work", "peak_source")})
+    roof["timing"] = "CUDA events around the launch on the launch stream (profiling mode: plain launches, so the " \
+                     "event-to-event time includes launch latency; conservative)"
+    roof["top_stage_overall"] = max(stages, key=stages.get)
+    roof["kernels"] = out
+    return roof
 
 
 # ------------------------------------------------------------------------------------------------
@@ -174,7 +264,7 @@ def run_gpu(args):
     stream = torch.cuda.current_stream()
 
     def frame(t):
-        return (t + 17 * rank) % n_frames
+        return multi.rank_frame(t, rank, n_frames)
 
     def barrier():
         if dist is not None:
@@ -190,28 +280,27 @@ def run_gpu(args):
         if timed_events is not None:
             timed_events[1].record(stream)
 
-    for t in range(Wu):
-        step(t)
-    nnp.check()
-    barrier()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
+    for t in range(Wu):
+        step(t)
+    nnp.check()
+    if rank == 0:
+        sampler.wait_first_sample()
+    barrier()
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
     t_wall0 = time.perf_counter()
     for t in range(K):
         step(Wu + t, evs[t])
     barrier()
-    t_wall = time.perf_counter() - t_wall0
-    clocks = sampler.stop() if rank == 0 else None
+    t_wall1 = time.perf_counter()
+    t_wall = t_wall1 - t_wall0
     nnp.check()
     dev_ms = sum(a.elapsed_time(b) for a, b in evs)
     per_step_ms = sorted(a.elapsed_time(b) for a, b in evs)
-    tmax = torch.tensor([dev_ms], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    dev_ms_max = float(tmax.item())
-    value = world * w.n_atoms * K / (dev_ms_max * 1e-3)
+    dev_ms_max = multi.max_over_ranks(dev_ms, dist, dev)
+    value = multi.aggregate_throughput(w.n_atoms, K, world, dev_ms_max)
 
     # ---- warm-L2 variant (weights stay L2-resident between steps, as in a tight MD loop)
     warm_ms = None
@@ -239,24 +328,7 @@ def run_gpu(args):
                 acc[k] = acc.get(k, 0.0) + v
         nnp.set_profiling(False)
         stages = {k: 1e3 * v / n_prof for k, v in acc.items()}  # us
-        top = max(stages, key=stages.get)
-        work = nnp.work()
-        peaks = {}
-        try:
-            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-        except Exception:
-            pass
-        hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
-        peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s"
-        # dominant kernel of this workload: the layer-1 GEMMs stream the layer-1 weights once per launch
-        l1 = "mlp_fwd_l1"
-        l1_bytes = work["layer1_weight_bytes"] + w.n_atoms * nnp.n_features * 4
-        achieved = l1_bytes / (stages[l1] * 1e-6) / 1e9
-        roofline = {"bound": "hbm", "kernel": "gemm_tma_kernel (" + l1 + ")", "achieved": achieved,
-                    "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
-                    "traffic": ncu_traffic_bytes(args.config),
-                    "peak_source": peak_src, "algorithmic_bytes": l1_bytes, "kernel_us": stages[l1],
-                    "top_stage": top}
+        roofline = stage_rooflines(w, nnp, stages, args.config)
 
     # ---- end-to-end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
@@ -275,12 +347,11 @@ def run_gpu(args):
             t0 = time.perf_counter()
             nnp.compute_host_into(hp[frame(Wu + t)].data_ptr(), hE.data_ptr(), hF.data_ptr(), sraw)  # syncs
             tot += time.perf_counter() - t0
-        tt = torch.tensor([tot], dtype=torch.float64, device=dev)
-        if dist is not None:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * w.n_atoms * K / float(tt.item()), "unit": UNIT,
+        tot_max = multi.max_over_ranks(tot, dist, dev)
+        e2e = {"value": multi.aggregate_throughput(w.n_atoms, K, world, 1e3 * tot_max), "unit": UNIT,
                "h2d_bytes_per_step": w.n_atoms * 12, "d2h_bytes_per_step": w.n_atoms * 12 + w.n_molecules * 8,
-               "us_per_step": 1e6 * float(tt.item()) / K}
+               "us_per_step": 1e6 * tot_max / K}
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
 
     # ---- CPU baseline: the oracle as it stands, bounded sample, rank 0 at N=1 only
     cpu = None
@@ -325,11 +396,11 @@ def run_gpu(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=1000)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config, 1-based (2 = the metric's)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--cpu-steps", type=int, default=200)
+    ap.add_argument("--cpu-steps", type=int, default=1000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--flags", type=int, default=0, help="NNP_FLAG_* bits (include/nnp.h) for A/B runs of the engines")
     args = ap.parse_args()

@@ -72,16 +72,7 @@ __device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t b
 }
 __device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, %0;" ::"n"(MID_CONSUMERS) : "memory"); }
 
-#ifdef NNP_MID_TRACE
-__device__ long long g_mid_trace[256];
-#define TR(k) do { if (blockIdx.x == 0 && threadIdx.x == 0 && (k) < 256) g_mid_trace[(k)] = clock64(); } while (0)
-#else
-#define TR(k)
-#endif
 }  // namespace
-#ifdef NNP_MID_TRACE
-extern "C" int nnp_debug_mid_trace(long long* out) { return (int)cudaMemcpyFromSymbol(out, g_mid_trace, sizeof(long long) * 256); }
-#endif
 
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem* __restrict__ items, int n_stages) {
@@ -91,7 +82,6 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
   __shared__ MidItem it;
   constexpr int TILE_FLOATS = MID_TILE_ROWS * MID_HMAX;
   constexpr int AH = MID_AC * MID_HMAX;  // floats of one activation / delta buffer
-  TR(0);
   {
     const int* src = reinterpret_cast<const int*>(items + blockIdx.x);
     int* dst = reinterpret_cast<int*>(&it);
@@ -154,10 +144,7 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
       reinterpret_cast<float4*>(hs + a * MID_HMAX)[k4] = v;
     }
   }
-  TR(1);
   consumer_sync();
-  TR(2);
-  int trk = 3;
 
   // ---- forward, layers 2..L-1
   for (int l = 2; l <= L - 1; ++l) {
@@ -174,9 +161,7 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
         x[a][j] = k4 < K4 ? reinterpret_cast<const float4*>(hin + a * MID_HMAX)[k4] : make_float4(0.f, 0.f, 0.f, 0.f);
       }
     for (int r0 = 0; r0 < R; r0 += MID_TILE_ROWS) {
-      TR(trk); ++trk;
       mb_wait(&full[slot], phase);
-      TR(trk); ++trk;
       const float4* tile = reinterpret_cast<const float4*>(ring + (size_t)slot * TILE_FLOATS);
       float s[8];
 #pragma unroll
@@ -231,8 +216,6 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
     }
     consumer_sync();
   }
-
-  TR(trk); ++trk;
   // ---- layer L (1 output): per-atom energies (FP64) and delta_{L-1} = w_L (.) CELU'(h_{L-1})
   float* dcur = dbuf;
   float* dnext = dbuf + AH;
@@ -252,8 +235,6 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
     }
   }
   consumer_sync();
-
-  TR(trk); ++trk;
   // ---- backward through layers L-1..2: delta_{l-1} = (delta_l W_l) (.) CELU'(h_{l-1})
   for (int l = L - 1; l >= 2; --l) {
     const int R = it.H[l], N4 = it.H[l - 1] >> 2;
@@ -263,9 +244,7 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
 #pragma unroll
       for (int j = 0; j < MID_NJ; ++j) acc[a][j] = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int o0 = 0; o0 < R; o0 += MID_TILE_ROWS) {
-      TR(trk); ++trk;
       mb_wait(&full[slot], phase);
-      TR(trk); ++trk;
       const float4* tile = reinterpret_cast<const float4*>(ring + (size_t)slot * TILE_FLOATS);
       const int ow = o0 + warp * MID_RW;  // R % 4 == 0: the warp's two rows are valid together
       if (ow < R) {
@@ -320,10 +299,7 @@ __global__ void __launch_bounds__(MID_THREADS, 1) small_mid_kernel(const MidItem
     }
     consumer_sync();
     float* tmp = dcur; dcur = dnext; dnext = tmp;
-    TR(trk); ++trk;
   }
-  TR(trk); ++trk;
-  TR(255);
 }
 
 // ------------------------------------------------------------------------------------------------

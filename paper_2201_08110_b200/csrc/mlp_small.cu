@@ -314,6 +314,121 @@ __global__ void __launch_bounds__(SM_THREADS) small_bwd_kernel(const SmallBwdIte
 }
 
 // ------------------------------------------------------------------------------------------------
+// backward through layer 1 (the 43 MB layer): out[a][n] = scale * sum_o D[a][o] W[o][n]
+// ------------------------------------------------------------------------------------------------
+// Every weight of the item's [n_out][128-column] chunk is read from shared memory exactly ONCE and applied to
+// all atoms of the item from registers: a warp owns a slice of the rows o, a lane owns 4 consecutive columns and
+// NA x 4 accumulators, held as packed pairs of atoms and updated with FFMA2 (fma.rn.f32x2: two atoms per
+// instruction); the delta tile is stored transposed ([o][atom]) so that one broadcast 128-bit load yields the
+// operands of two packed pairs.  The 8 row slices are summed in a fixed order through shared memory (the
+// weight buffer is reused).  Weight rows arrive as bulk async copies, one mbarrier per row slice, all issued
+// before griddepcontrol.wait.
+constexpr int B1_SLICES = SM_WARPS;
+
+__device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsigned long long b, unsigned long long c) {
+  unsigned long long d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ unsigned long long pack2(float x, float y) {
+  unsigned long long d;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(x), "f"(y));
+  return d;
+}
+__device__ __forceinline__ float2 unpack2(unsigned long long v) {
+  float2 r;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+  return r;
+}
+
+template <int NA>
+__device__ __forceinline__ void small_bwd1_body(const SmallBwdItem& it, float* smem_f, uint64_t* bars) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int rps = (it.n_out + B1_SLICES - 1) / B1_SLICES;  // rows per slice
+  const size_t ws_floats = max((size_t)it.n_out * 128, (size_t)B1_SLICES * NA * 128);
+  float* ws = smem_f;                 // [n_out][128]; later red [B1_SLICES][NA][128]
+  float* dsT = smem_f + ws_floats;    // [n_out][NA]
+  if (threadIdx.x == 0) {
+    for (int g = 0; g < B1_SLICES; ++g) {
+      const int rows = max(0, min(it.n_out, (g + 1) * rps) - g * rps);
+      sbar_init(&bars[g], 1);
+      if (rows) sbar_expect_tx(&bars[g], (uint32_t)(rows * it.n_cols * 4));
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  pdl_trigger();
+  for (int o = threadIdx.x; o < it.n_out; o += SM_THREADS)
+    bulk_g2s(ws + (size_t)o * 128, it.W + (size_t)o * it.ldw, (uint32_t)(it.n_cols * 4), &bars[o / rps]);
+  pdl_wait();  // delta comes from the previous kernel
+  for (int idx = threadIdx.x; idx < NA * it.n_out; idx += SM_THREADS) {
+    const int a = idx / it.n_out, o = idx - a * it.n_out;
+    dsT[o * NA + a] = a < it.n_atoms ? it.D[(size_t)a * it.ldd + o] : 0.0f;
+  }
+  __syncthreads();
+
+  unsigned long long acc[NA / 2][4];
+#pragma unroll
+  for (int q = 0; q < NA / 2; ++q)
+#pragma unroll
+    for (int c = 0; c < 4; ++c) acc[q][c] = 0ull;
+  const bool col_ok = 4 * lane < it.n_cols;
+  const int o0 = warp * rps, o1 = min(it.n_out, o0 + rps);
+  if (o0 < o1) sbar_wait(&bars[warp], 0);
+  if (col_ok) {
+    const float4* wp = reinterpret_cast<const float4*>(ws) + lane;
+#pragma unroll 2
+    for (int o = o0; o < o1; ++o) {
+      const float4 w = wp[(size_t)o * 32];
+      const unsigned long long wx = pack2(w.x, w.x), wy = pack2(w.y, w.y), wz = pack2(w.z, w.z), ww = pack2(w.w, w.w);
+      const float4* dp = reinterpret_cast<const float4*>(dsT + (size_t)o * NA);
+#pragma unroll
+      for (int q = 0; q < NA / 4; ++q) {
+        const float4 d = dp[q];
+        const unsigned long long d01 = pack2(d.x, d.y), d23 = pack2(d.z, d.w);
+        acc[2 * q][0] = ffma2(d01, wx, acc[2 * q][0]); acc[2 * q][1] = ffma2(d01, wy, acc[2 * q][1]);
+        acc[2 * q][2] = ffma2(d01, wz, acc[2 * q][2]); acc[2 * q][3] = ffma2(d01, ww, acc[2 * q][3]);
+        acc[2 * q + 1][0] = ffma2(d23, wx, acc[2 * q + 1][0]); acc[2 * q + 1][1] = ffma2(d23, wy, acc[2 * q + 1][1]);
+        acc[2 * q + 1][2] = ffma2(d23, wz, acc[2 * q + 1][2]); acc[2 * q + 1][3] = ffma2(d23, ww, acc[2 * q + 1][3]);
+      }
+    }
+  }
+  __syncthreads();  // every warp is done with the weight buffer: reuse it for the slice sums
+  float4* red = reinterpret_cast<float4*>(ws);
+  if (col_ok) {
+#pragma unroll
+    for (int q = 0; q < NA / 2; ++q) {
+      const float2 c0 = unpack2(acc[q][0]), c1 = unpack2(acc[q][1]), c2 = unpack2(acc[q][2]), c3 = unpack2(acc[q][3]);
+      red[((size_t)warp * NA + 2 * q) * 32 + lane] = make_float4(c0.x, c1.x, c2.x, c3.x);
+      red[((size_t)warp * NA + 2 * q + 1) * 32 + lane] = make_float4(c0.y, c1.y, c2.y, c3.y);
+    }
+  }
+  __syncthreads();
+  for (int idx = threadIdx.x; idx < it.n_atoms * 32; idx += SM_THREADS) {
+    const int a = idx >> 5, l = idx & 31;
+    if (4 * l >= it.n_cols) continue;
+    float4 v = red[(size_t)a * 32 + l];
+#pragma unroll
+    for (int s = 1; s < B1_SLICES; ++s) {  // fixed order
+      const float4 u = red[((size_t)s * NA + a) * 32 + l];
+      v.x += u.x; v.y += u.y; v.z += u.z; v.w += u.w;
+    }
+    v.x *= it.scale; v.y *= it.scale; v.z *= it.scale; v.w *= it.scale;
+    *reinterpret_cast<float4*>(it.out + (size_t)a * it.ldo + 4 * l) = v;
+  }
+}
+
+__global__ void __launch_bounds__(SM_THREADS, 1) small_bwd1_kernel(const SmallBwdItem* __restrict__ items) {
+  extern __shared__ __align__(16) float smem_f[];
+  __shared__ __align__(8) uint64_t bars[B1_SLICES];
+  const SmallBwdItem it = items[blockIdx.x];
+  if (it.n_atoms <= 4) small_bwd1_body<4>(it, smem_f, bars);
+  else if (it.n_atoms <= 8) small_bwd1_body<8>(it, smem_f, bars);
+  else if (it.n_atoms <= 16) small_bwd1_body<16>(it, smem_f, bars);
+  else small_bwd1_body<24>(it, smem_f, bars);
+}
+
+// ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
 static const size_t SMALL_SMEM_MAX = 200 * 1024;
@@ -331,6 +446,7 @@ int small_init() {
   rc |= set_smem(small_fwd_kernel<4>, SMALL_SMEM_MAX);
   rc |= set_smem(small_fwd_kernel<8>, SMALL_SMEM_MAX);
   rc |= set_smem(small_bwd_kernel, SMALL_SMEM_MAX);
+  rc |= set_smem(small_bwd1_kernel, SMALL_SMEM_MAX);
   return rc;
 }
 
@@ -379,6 +495,29 @@ int small_build_bwd(SmallLaunch& L, std::vector<SmallBwdItem>& items) {
   return 0;
 }
 
+static int bwd1_pad(int n_atoms) { return n_atoms <= 4 ? 4 : n_atoms <= 8 ? 8 : n_atoms <= 16 ? 16 : 24; }
+
+// layer-1 backward items: n_atoms <= 24, n_cols <= 128, epilogue EPI_SCALE
+int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items) {
+  std::stable_sort(items.begin(), items.end(), [](const SmallBwdItem& a, const SmallBwdItem& b) {
+    return (long long)a.n_out * a.n_cols * (a.n_atoms + 4) > (long long)b.n_out * b.n_cols * (b.n_atoms + 4);
+  });
+  L.n_items = (int)items.size();
+  L.variant = 100;
+  L.smem_bytes = 0;
+  for (const auto& it : items) {
+    if (it.n_atoms < 1 || it.n_atoms > 24 || it.n_cols > 128 || it.epi != EPI_SCALE) return -1;
+    const int NA = bwd1_pad(it.n_atoms);
+    const size_t b = (std::max((size_t)it.n_out * 128, (size_t)B1_SLICES * NA * 128) + (size_t)it.n_out * NA) * 4;
+    L.smem_bytes = std::max(L.smem_bytes, b);
+  }
+  if (L.smem_bytes > SMALL_SMEM_MAX) return -1;
+  if (cudaMalloc(&L.d_items, std::max<size_t>(1, items.size()) * sizeof(SmallBwdItem)) != cudaSuccess) return -1;
+  if (!items.empty())
+    cudaMemcpy(L.d_items, items.data(), items.size() * sizeof(SmallBwdItem), cudaMemcpyHostToDevice);
+  return 0;
+}
+
 void small_launch_fwd(const SmallLaunch& L, cudaStream_t s, bool pdl) {
   if (L.n_items == 0) return;
   const SmallFwdItem* it = reinterpret_cast<const SmallFwdItem*>(L.d_items);
@@ -393,6 +532,11 @@ void small_launch_fwd(const SmallLaunch& L, cudaStream_t s, bool pdl) {
 
 void small_launch_bwd(const SmallLaunch& L, cudaStream_t s, bool pdl) {
   if (L.n_items == 0) return;
+  if (L.variant == 100) {
+    launch_kernel(pdl, small_bwd1_kernel, dim3(L.n_items), dim3(SM_THREADS), L.smem_bytes, s,
+                  reinterpret_cast<const SmallBwdItem*>(L.d_items));
+    return;
+  }
   launch_kernel(pdl, small_bwd_kernel, dim3(L.n_items), dim3(SM_THREADS), L.smem_bytes, s,
                 reinterpret_cast<const SmallBwdItem*>(L.d_items));
 }

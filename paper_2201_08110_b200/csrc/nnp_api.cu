@@ -617,13 +617,15 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     }
     for (int l = l_bwd_begin; l >= 1; --l) {  // backward
       std::vector<SmallBwdItem> items;
+      const bool bwd1 = l == 1 && (h->use_mid || L - 1 > 1);  // plain delta_1 -> dE/dAEV (no fused last layer)
       for (int e = 0; e < S; ++e) {
         const int ne = h->grp_off[e + 1] - h->grp_off[e];
         if (ne == 0) continue;
         const int nin = h->dims[e * (L + 1) + l - 1], nout = h->dims[e * (L + 1) + l];
         const float* Wl = h->d_W + h->w_off[e * L + l - 1];
-        for (int a0 = 0; a0 < ne; a0 += 32) {
-          const int na = std::min(32, ne - a0);
+        const int achunk = bwd1 ? 24 : 32;  // layer 1 runs on the weights-read-once kernel (<= 24 atoms per item)
+        for (int a0 = 0; a0 < ne; a0 += achunk) {
+          const int na = std::min(achunk, ne - a0);
           for (int m = 0; m < M; ++m)
             for (int n0 = 0; n0 < nin; n0 += 128) {
               SmallBwdItem it;
@@ -660,7 +662,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       }
       SmallLaunch sl;
       sl.name = "mlp_bwd_l" + std::to_string(l);
-      if (small_build_bwd(sl, items)) { small_free_launch(sl); return fail(NNP_ERR_CUDA); }
+      if (bwd1 ? small_build_bwd1(sl, items) : small_build_bwd(sl, items)) { small_free_launch(sl); return fail(NNP_ERR_CUDA); }
       h->sbwd.push_back(sl);
     }
   }

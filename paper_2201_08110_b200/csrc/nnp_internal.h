@@ -189,6 +189,7 @@ int small_init();
 void small_bwd_shape(int n_atoms, int* AW, int* G);
 int small_build_fwd(SmallLaunch& L, std::vector<SmallFwdItem>& items);
 int small_build_bwd(SmallLaunch& L, std::vector<SmallBwdItem>& items);
+int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items);  // layer 1: weights read once, FFMA2
 void small_launch_fwd(const SmallLaunch& L, cudaStream_t s, bool pdl);
 void small_launch_bwd(const SmallLaunch& L, cudaStream_t s, bool pdl);
 void small_free_launch(SmallLaunch& L);
