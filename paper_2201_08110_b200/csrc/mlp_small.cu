@@ -318,9 +318,9 @@ __global__ void __launch_bounds__(SM_THREADS) small_bwd_kernel(const SmallBwdIte
 // ------------------------------------------------------------------------------------------------
 // Every weight of the item's [n_out][128-column] chunk is read from shared memory exactly ONCE and applied to
 // all atoms of the item from registers: a warp owns a slice of the rows o, a lane owns 4 consecutive columns and
-// NA x 4 accumulators, held as packed pairs of atoms and updated with FFMA2 (fma.rn.f32x2: two atoms per
-// instruction); the delta tile is stored transposed ([o][atom]) so that one broadcast 128-bit load yields the
-// operands of two packed pairs.  The 8 row slices are summed in a fixed order through shared memory (the
+// NA x 4 accumulators, held as packed pairs of columns and updated with FFMA2 (fma.rn.f32x2: two columns per
+// instruction; the weight pairs come straight out of the 128-bit shared-memory load, the delta operand is a
+// broadcast pair); one broadcast 128-bit load of the delta tile serves four rows of one atom.  The 8 row slices are summed in a fixed order through shared memory (the
 // weight buffer is reused).  Weight rows arrive as bulk async copies, one mbarrier per row slice, all issued
 // before griddepcontrol.wait.
 constexpr int B1_SLICES = SM_WARPS;
@@ -344,52 +344,57 @@ __device__ __forceinline__ float2 unpack2(unsigned long long v) {
 template <int NA>
 __device__ __forceinline__ void small_bwd1_body(const SmallBwdItem& it, float* smem_f, uint64_t* bars) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int rps = (it.n_out + B1_SLICES - 1) / B1_SLICES;  // rows per slice
+  const int rps = (((it.n_out + B1_SLICES - 1) / B1_SLICES) + 3) & ~3;  // rows per slice, a multiple of 4
   const size_t ws_floats = max((size_t)it.n_out * 128, (size_t)B1_SLICES * NA * 128);
-  float* ws = smem_f;                 // [n_out][128]; later red [B1_SLICES][NA][128]
-  float* dsT = smem_f + ws_floats;    // [n_out][NA]
+  float* ws = smem_f;               // [n_out][128]; later red [B1_SLICES][NA][128]
+  float* ds = smem_f + ws_floats;   // [NA][n_out]
+  uint64_t* dbar = bars + B1_SLICES;
   if (threadIdx.x == 0) {
     for (int g = 0; g < B1_SLICES; ++g) {
       const int rows = max(0, min(it.n_out, (g + 1) * rps) - g * rps);
       sbar_init(&bars[g], 1);
       if (rows) sbar_expect_tx(&bars[g], (uint32_t)(rows * it.n_cols * 4));
     }
+    sbar_init(dbar, 1);
+    sbar_expect_tx(dbar, (uint32_t)(it.n_atoms * it.n_out * 4));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
   pdl_trigger();
   for (int o = threadIdx.x; o < it.n_out; o += SM_THREADS)
     bulk_g2s(ws + (size_t)o * 128, it.W + (size_t)o * it.ldw, (uint32_t)(it.n_cols * 4), &bars[o / rps]);
+  for (int idx = it.n_atoms * it.n_out + threadIdx.x; idx < NA * it.n_out; idx += SM_THREADS) ds[idx] = 0.0f;
   pdl_wait();  // delta comes from the previous kernel
-  for (int idx = threadIdx.x; idx < NA * it.n_out; idx += SM_THREADS) {
-    const int a = idx / it.n_out, o = idx - a * it.n_out;
-    dsT[o * NA + a] = a < it.n_atoms ? it.D[(size_t)a * it.ldd + o] : 0.0f;
-  }
-  __syncthreads();
+  if (threadIdx.x < it.n_atoms)
+    bulk_g2s(ds + (size_t)threadIdx.x * it.n_out, it.D + (size_t)threadIdx.x * it.ldd, (uint32_t)(it.n_out * 4), dbar);
+  __syncthreads();  // zero rows of the padding atoms visible
+  sbar_wait(dbar, 0);
 
-  unsigned long long acc[NA / 2][4];
+  // acc[a][0] = columns (4 lane, 4 lane + 1), acc[a][1] = columns (4 lane + 2, 4 lane + 3) of atom a
+  unsigned long long acc[NA][2];
 #pragma unroll
-  for (int q = 0; q < NA / 2; ++q)
-#pragma unroll
-    for (int c = 0; c < 4; ++c) acc[q][c] = 0ull;
+  for (int a = 0; a < NA; ++a) acc[a][0] = acc[a][1] = 0ull;
   const bool col_ok = 4 * lane < it.n_cols;
   const int o0 = warp * rps, o1 = min(it.n_out, o0 + rps);
   if (o0 < o1) sbar_wait(&bars[warp], 0);
   if (col_ok) {
     const float4* wp = reinterpret_cast<const float4*>(ws) + lane;
-#pragma unroll 2
-    for (int o = o0; o < o1; ++o) {
-      const float4 w = wp[(size_t)o * 32];
-      const unsigned long long wx = pack2(w.x, w.x), wy = pack2(w.y, w.y), wz = pack2(w.z, w.z), ww = pack2(w.w, w.w);
-      const float4* dp = reinterpret_cast<const float4*>(dsT + (size_t)o * NA);
+    for (int o = o0; o < o1; o += 4) {
+      unsigned long long wlo[4], whi[4];
 #pragma unroll
-      for (int q = 0; q < NA / 4; ++q) {
-        const float4 d = dp[q];
-        const unsigned long long d01 = pack2(d.x, d.y), d23 = pack2(d.z, d.w);
-        acc[2 * q][0] = ffma2(d01, wx, acc[2 * q][0]); acc[2 * q][1] = ffma2(d01, wy, acc[2 * q][1]);
-        acc[2 * q][2] = ffma2(d01, wz, acc[2 * q][2]); acc[2 * q][3] = ffma2(d01, ww, acc[2 * q][3]);
-        acc[2 * q + 1][0] = ffma2(d23, wx, acc[2 * q + 1][0]); acc[2 * q + 1][1] = ffma2(d23, wy, acc[2 * q + 1][1]);
-        acc[2 * q + 1][2] = ffma2(d23, wz, acc[2 * q + 1][2]); acc[2 * q + 1][3] = ffma2(d23, ww, acc[2 * q + 1][3]);
+      for (int i = 0; i < 4; ++i) {
+        const float4 w = wp[(size_t)(o + i) * 32];
+        wlo[i] = pack2(w.x, w.y);
+        whi[i] = pack2(w.z, w.w);
+      }
+#pragma unroll
+      for (int a = 0; a < NA; ++a) {
+        const float4 d = *reinterpret_cast<const float4*>(ds + (size_t)a * it.n_out + o);
+        const unsigned long long d0 = pack2(d.x, d.x), d1 = pack2(d.y, d.y), d2 = pack2(d.z, d.z), d3 = pack2(d.w, d.w);
+        acc[a][0] = ffma2(d0, wlo[0], acc[a][0]); acc[a][1] = ffma2(d0, whi[0], acc[a][1]);
+        acc[a][0] = ffma2(d1, wlo[1], acc[a][0]); acc[a][1] = ffma2(d1, whi[1], acc[a][1]);
+        acc[a][0] = ffma2(d2, wlo[2], acc[a][0]); acc[a][1] = ffma2(d2, whi[2], acc[a][1]);
+        acc[a][0] = ffma2(d3, wlo[3], acc[a][0]); acc[a][1] = ffma2(d3, whi[3], acc[a][1]);
       }
     }
   }
@@ -397,10 +402,9 @@ __device__ __forceinline__ void small_bwd1_body(const SmallBwdItem& it, float* s
   float4* red = reinterpret_cast<float4*>(ws);
   if (col_ok) {
 #pragma unroll
-    for (int q = 0; q < NA / 2; ++q) {
-      const float2 c0 = unpack2(acc[q][0]), c1 = unpack2(acc[q][1]), c2 = unpack2(acc[q][2]), c3 = unpack2(acc[q][3]);
-      red[((size_t)warp * NA + 2 * q) * 32 + lane] = make_float4(c0.x, c1.x, c2.x, c3.x);
-      red[((size_t)warp * NA + 2 * q + 1) * 32 + lane] = make_float4(c0.y, c1.y, c2.y, c3.y);
+    for (int a = 0; a < NA; ++a) {
+      const float2 lo = unpack2(acc[a][0]), hi = unpack2(acc[a][1]);
+      red[((size_t)warp * NA + a) * 32 + lane] = make_float4(lo.x, lo.y, hi.x, hi.y);
     }
   }
   __syncthreads();
@@ -420,7 +424,7 @@ __device__ __forceinline__ void small_bwd1_body(const SmallBwdItem& it, float* s
 
 __global__ void __launch_bounds__(SM_THREADS, 1) small_bwd1_kernel(const SmallBwdItem* __restrict__ items) {
   extern __shared__ __align__(16) float smem_f[];
-  __shared__ __align__(8) uint64_t bars[B1_SLICES];
+  __shared__ __align__(8) uint64_t bars[B1_SLICES + 1];
   const SmallBwdItem it = items[blockIdx.x];
   if (it.n_atoms <= 4) small_bwd1_body<4>(it, smem_f, bars);
   else if (it.n_atoms <= 8) small_bwd1_body<8>(it, smem_f, bars);
