@@ -20,6 +20,8 @@ NNP_FLAG_NO_UMMA = 4
 NNP_FLAG_NO_SMALL = 8
 NNP_FLAG_NO_MID = 16
 NNP_FLAG_NO_PDL = 32
+NNP_FLAG_NO_CELLS = 64
+NNP_FLAG_FORCE_CELLS = 128
 ERRORS = {
     -1: "NNP_ERR_INVALID_ARG",
     -2: "NNP_ERR_CUDA",

@@ -598,6 +598,10 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(
 // ------------------------------------------------------------------------------------------------
 void launch_neighbors(nnp_handle* h, const float* d_pos, int pos_stride, const int* d_atom_index, cudaStream_t s) {
   if (h->N == 0) return;
+  if (h->use_cells) {
+    launch_neighbors_cells(h, d_pos, pos_stride, d_atom_index, s);
+    return;
+  }
   const int blocks = (h->N + 3) / 4;
   nbr_allpairs_kernel<<<blocks, 128, 0, s>>>(d_pos, pos_stride, d_atom_index, h->d_species, h->d_mol_id,
                                              h->d_mol_off, h->N, h->aev, h->capR, h->capA, h->d_pos4, h->d_nbr_r,

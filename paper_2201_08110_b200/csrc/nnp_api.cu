@@ -85,6 +85,7 @@ extern "C" void nnp_destroy(nnp_handle* h) {
   for (auto* v : {&h->sfwd, &h->sbwd})
     for (auto& g : *v) small_free_launch(g);
   small_free_launch(h->smid);
+  cells_free(h);
   delete h;
 }
 
@@ -192,6 +193,8 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   h->capR = cfg->max_radial_neighbors > 0 ? cfg->max_radial_neighbors : std::min(std::max(max_mol - 1, 1), 256);
   h->capA = cfg->max_angular_neighbors > 0 ? cfg->max_angular_neighbors : std::min(std::max(max_mol - 1, 1), 128);
   if (h->capA > h->capR) h->capA = h->capR;
+  // A1 engine: all pairs inside a molecule at ligand sizes, cell binning for large molecules
+  h->use_cells = N > 0 && !(cfg->flags & NNP_FLAG_NO_CELLS) && (max_mol >= 1024 || (cfg->flags & NNP_FLAG_FORCE_CELLS));
 
   auto fail = [&](int code) {
     nnp_destroy(h);
@@ -269,6 +272,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       dev_alloc(&h->d_eatom, (size_t)N * M) || dev_alloc(&h->d_status, 1) || dev_alloc(&h->d_hpos, (size_t)N * 3) ||
       dev_alloc(&h->d_hforce, (size_t)N * 3) || dev_alloc(&h->d_henergy, (size_t)n_molecules))
     return fail(NNP_ERR_ALLOC);
+  if (h->use_cells && cells_alloc(h) != 0) return fail(NNP_ERR_ALLOC);
   cudaMemset(h->d_status, 0, sizeof(int));
   cudaMemset(h->d_nbr_r, 0, sizeof(int) * std::max<size_t>((size_t)N * h->capR, 1));
   cudaMemset(h->d_nbr_a, 0, sizeof(int) * std::max<size_t>((size_t)N * h->capA, 1));
@@ -705,7 +709,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   }
   h->stage_names.push_back("aev_bwd");
   h->stage_names.push_back("finish");
-  h->n_launches = N > 0 ? (int)h->stage_names.size() : 0;
+  h->n_launches = N > 0 ? (int)h->stage_names.size() + (h->use_cells ? 4 : 0) : 0;  // cell path: 5 kernels in "nbr"
   h->events.resize(h->stage_names.size() + 1);
   for (auto& e : h->events)
     if (cudaEventCreate(&e) != cudaSuccess) return fail(NNP_ERR_CUDA);

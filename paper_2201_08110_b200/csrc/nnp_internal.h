@@ -246,6 +246,11 @@ struct nnp_handle {
   float* d_daev = nullptr;  // [n_parts][N sorted][n_feat]
   float* d_phi = nullptr;   // [N][capR][3]
   double* d_eatom = nullptr;  // [N sorted][M]
+  // cell-binned neighbour search (nbr_cells.cu), used for large molecules
+  bool use_cells = false;
+  void* d_cell_grid = nullptr;
+  int *d_cell_count = nullptr, *d_cell_start = nullptr, *d_cell_of = nullptr, *d_cell_rank = nullptr,
+      *d_cell_atoms = nullptr;
   int* d_status = nullptr;
   // weights
   float *d_W = nullptr, *d_b = nullptr;
@@ -286,6 +291,9 @@ struct nnp_handle {
 
 // kernels (launch wrappers)
 void launch_neighbors(nnp_handle* h, const float* d_pos, int pos_stride, const int* d_atom_index, cudaStream_t s);
+int cells_alloc(nnp_handle* h);
+void cells_free(nnp_handle* h);
+void launch_neighbors_cells(nnp_handle* h, const float* d_pos, int pos_stride, const int* d_atom_index, cudaStream_t s);
 void launch_aev_forward(nnp_handle* h, cudaStream_t s);
 void launch_aev_backward(nnp_handle* h, cudaStream_t s);
 void launch_gemm(const GemmLaunch& g, cudaStream_t s);

@@ -14,8 +14,9 @@ torch = pytest.importorskip("torch")
 
 from oracle.ani_oracle import AniOracle  # noqa: E402
 from paper_2201_08110_b200 import workloads as wl  # noqa: E402
-from paper_2201_08110_b200.binding import (NNP, NNP_FLAG_NO_GRAPH, NNP_FLAG_NO_MID, NNP_FLAG_NO_SMALL,  # noqa: E402
-                                            NNP_FLAG_NO_TMA, NNP_FLAG_NO_UMMA, NNPError)
+from paper_2201_08110_b200.binding import (NNP, NNP_FLAG_FORCE_CELLS, NNP_FLAG_NO_CELLS, NNP_FLAG_NO_GRAPH,  # noqa: E402
+                                            NNP_FLAG_NO_MID, NNP_FLAG_NO_PDL, NNP_FLAG_NO_SMALL, NNP_FLAG_NO_TMA,
+                                            NNP_FLAG_NO_UMMA, NNPError)
 
 # MLP engines: ligand-size weight-streaming FFMA (default at these sizes; with the fused middle launch or
 # one launch per layer), tcgen05 3xTF32, TMA+FFMA, plain FFMA
@@ -177,6 +178,58 @@ def test_config5_water_cluster():
     F = gpu["F"]
     assert np.abs(F.sum(axis=0)).max() <= 1e-2
     nnp.destroy()
+
+
+def test_cell_binned_neighbour_search():
+    """A1 with cell binning (default for molecules >= 1024 atoms) against the all-pairs kernel and the oracle:
+    forced on at ligand size (stage-wise parity), on a batch of molecules (cells shared by several molecules) and
+    switched off at 9999 atoms; the rows are identical, so energies and forces are bit-identical."""
+    w = wl.config2()
+    W, B = w.weights()
+    orc = AniOracle(w.params, W, B)
+    ref = orc.energy_forces(w.positions, w.species, want_intermediates=True)
+    nnp = NNP(w.params, W, B, w.species, flags=NNP_FLAG_FORCE_CELLS)
+    gpu = gpu_eval(nnp, w.positions, stages=True)
+    check_stages(gpu, ref, orc, w.positions, w.mol_offsets)
+    check_energy_forces(gpu, ref, w.mol_offsets)
+    plain = NNP(w.params, W, B, w.species)
+    r0 = gpu_eval(plain, w.positions)
+    assert np.array_equal(r0["E"], gpu["E"]) and np.array_equal(r0["F"], gpu["F"])
+    nnp.destroy(); plain.destroy()
+
+    w = wl.config3(n_mol=24)
+    W, B = w.weights()
+    orc = AniOracle(w.params, W, B)
+    a = NNP(w.params, W, B, w.species, w.mol_offsets, flags=NNP_FLAG_FORCE_CELLS)
+    b = NNP(w.params, W, B, w.species, w.mol_offsets)
+    ra = gpu_eval(a, w.positions, n_mol=w.n_molecules, stages=True)
+    rb = gpu_eval(b, w.positions, n_mol=w.n_molecules)
+    for which, key in (("radial", "pairs_r"), ("angular", "pairs_a")):
+        assert set(map(tuple, ra[key].tolist())) == directed(orc.pairs(w.positions, which, w.mol_offsets))
+    assert np.array_equal(ra["E"], rb["E"]) and np.array_equal(ra["F"], rb["F"])
+    a.destroy(); b.destroy()
+
+    w = wl.config5()
+    W, B = w.weights()
+    a = NNP(w.params, W, B, w.species)  # cells
+    b = NNP(w.params, W, B, w.species, flags=NNP_FLAG_NO_CELLS)
+    ra, rb = gpu_eval(a, w.positions), gpu_eval(b, w.positions)
+    assert a.launches_per_compute == b.launches_per_compute + 4
+    assert np.array_equal(ra["E"], rb["E"]) and np.array_equal(ra["F"], rb["F"])
+    a.destroy(); b.destroy()
+
+
+def test_pdl_and_plain_launch_chains_agree():
+    """Programmatic dependent launches only change WHEN a kernel starts: same bits as plain launches."""
+    w = wl.config2()
+    W, B = w.weights()
+    a = NNP(w.params, W, B, w.species)
+    b = NNP(w.params, W, B, w.species, flags=NNP_FLAG_NO_PDL)
+    traj = w.trajectory(8)
+    for t in range(8):
+        ra, rb = gpu_eval(a, traj[t]), gpu_eval(b, traj[t])
+        assert np.array_equal(ra["E"], rb["E"]) and np.array_equal(ra["F"], rb["F"])
+    a.destroy(); b.destroy()
 
 
 # ------------------------------------------------------------------------------------------------
