@@ -97,10 +97,10 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo, uint
   return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)((lbo >> 4) & 0x3FFF) << 16) |
          ((uint64_t)((sbo >> 4) & 0x3FFF) << 32) | (1ull << 46) | ((uint64_t)layout << 61);
 }
+// round to TF32 (10 explicit mantissa bits), nearest, ties away from zero == cvt.rna.tf32.f32 for finite inputs,
+// done on the integer ALU (the conversion instruction runs at a fraction of the ALU rate and paced the converters)
 __device__ __forceinline__ float tf32_rna(float x) {
-  uint32_t r;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
-  return __uint_as_float(r);
+  return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xFFFFE000u);
 }
 // weights: hi = trunc_tf32(w) is implicit (the tensor core truncates the raw value); lo = rna(w - hi)
 __device__ __forceinline__ float w_lo(float w) {
@@ -244,10 +244,19 @@ __device__ __forceinline__ void drain_item(const UmmaItem& t, const UmmaParams& 
       for (int j = 0; j < CT; ++j)
         if (j < nv) C[(size_t)j * t.ldc] = celu_f(tot[j] + b, t.alpha, t.inv_alpha);
     } else if (t.epi == EPI_MUL_DCELU) {
+      // aux may alias C (delta overwrites the activation in place): read every activation of this thread first, so
+      // the loads are independent and in flight together instead of being ordered behind the stores
       const float* aux = t.aux + (size_t)col0 * t.ldaux + f;
+      constexpr int HB = CT < 16 ? CT : 16;  // batch size: enough loads in flight, no register spills
 #pragma unroll
-      for (int j = 0; j < CT; ++j)
-        if (j < nv) C[(size_t)j * t.ldc] = tot[j] * dcelu_from_h(aux[(size_t)j * t.ldaux], t.inv_alpha);
+      for (int j0 = 0; j0 < CT; j0 += HB) {
+        float hv[HB];
+#pragma unroll
+        for (int j = 0; j < HB; ++j) hv[j] = j0 + j < nv ? aux[(size_t)(j0 + j) * t.ldaux] : 0.0f;
+#pragma unroll
+        for (int j = 0; j < HB; ++j)
+          if (j0 + j < nv) C[(size_t)(j0 + j) * t.ldc] = tot[j0 + j] * dcelu_from_h(hv[j], t.inv_alpha);
+      }
     } else {
 #pragma unroll
       for (int j = 0; j < CT; ++j)
@@ -324,56 +333,59 @@ __global__ void __launch_bounds__(U_THREADS, 1) gemm_umma_kernel(const __grid_co
     }
   } else if (warp == 1) {
     // ------------------------------------------------------------ MMA issuer
+    // One thread; its instruction stream is the critical path of the CTA (every instruction of a single thread
+    // costs its full latency), so everything loop-invariant lives in registers and the four shared-memory
+    // descriptors of a box are formed once and advanced by an integer add per k-step.
     if (lane == 0) {
       uint32_t rs = 0, ls = 0, lphase = 0, grp = 0, gphase = 0, item_ctr = 0;
       const uint32_t d_x = tmem;
+      const uint32_t n_raw = (uint32_t)P.n_raw, n_groups = (uint32_t)P.n_groups, gslots = (uint32_t)P.gslots,
+                     kps = (uint32_t)P.kps, slot_cols = (uint32_t)P.slot_cols, stage_bytes = (uint32_t)P.stage_bytes;
+      const uint32_t raw0 = smem_u32(raw), lo0 = smem_u32(los);
+      // descriptor templates (address field zero): K-major 128B swizzle / MN-major 128B swizzle with 32B atoms
+      const uint64_t desc_k = smem_desc(0, 16, 1024, 2), desc_mn = smem_desc(0, 4096, 512, 1);
+      uint32_t d_hi = tmem + slot_cols;  // slot (grp 0, in_group 0)
       for (int it = it0; it < it1; ++it) {
         const UmmaItem& t = P.items[it];
         const int a_mn = t.a_mn, nb = t.kb1 - t.kb0;
         const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)a_mn << 15) |
                                ((uint32_t)(t.n_pad >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+        const uint64_t desc_a = a_mn ? desc_mn : desc_k;
+        const uint32_t a_step = a_mn ? (1024u >> 4) : (32u >> 4);  // descriptor address units (16 B) per k-step
         mbar_wait(cross_empty, (item_ctr & 1u) ^ 1u);
-        int in_group = 0, in_slot = 0, ks_left = nb * 4;
+        uint32_t in_group = 0, in_slot = 0, ks_left = (uint32_t)nb * 4u, first = 1u;
         for (int b = 0; b < nb; ++b) {
           mbar_wait(&conv[ls], lphase);  // lo parts written (and, transitively, the raw stage has landed)
           tc_fence_after();
-          const uint32_t sa = smem_u32(raw + (size_t)rs * P.stage_bytes);
-          const uint32_t sb = sa + A_BOX_BYTES;
-          const uint32_t sal = smem_u32(los + (size_t)ls * P.stage_bytes);
-          const uint32_t sbl = sal + A_BOX_BYTES;
+          const uint32_t sa = (raw0 + rs * stage_bytes) >> 4, sal = (lo0 + ls * stage_bytes) >> 4;
+          uint64_t ah = desc_a | sa, al = desc_a | sal;
+          uint64_t bh = desc_k | (sa + (A_BOX_BYTES >> 4)), bl = desc_k | (sal + (A_BOX_BYTES >> 4));
 #pragma unroll
           for (int ks = 0; ks < 4; ++ks) {
-            if (in_group == 0 && in_slot == 0) {
+            if ((in_group | in_slot) == 0) {
               mbar_wait(&group_empty[grp], gphase ^ 1u);
               tc_fence_after();
             }
-            const uint32_t d_hi = tmem + (uint32_t)P.slot_cols * (1u + grp * (uint32_t)P.gslots + (uint32_t)in_group);
-            uint64_t ah, al;
-            if (!a_mn) {
-              ah = smem_desc(sa + ks * 32, 16, 1024, 2);
-              al = smem_desc(sal + ks * 32, 16, 1024, 2);
-            } else {
-              ah = smem_desc(sa + ks * 1024, 4096, 512, 1);
-              al = smem_desc(sal + ks * 1024, 4096, 512, 1);
-            }
-            const uint64_t bh = smem_desc(sb + ks * 32, 16, 1024, 2);
-            const uint64_t bl = smem_desc(sbl + ks * 32, 16, 1024, 2);
-            mma_tf32(d_x, al, bh, idesc, (b == 0 && ks == 0) ? 0u : 1u);
+            mma_tf32(d_x, al, bh, idesc, first ^ 1u);
             mma_tf32(d_x, ah, bl, idesc, 1u);
-            mma_tf32(d_hi, ah, bh, idesc, in_slot ? 1u : 0u);
+            mma_tf32(d_hi, ah, bh, idesc, in_slot);
+            first = 0u;
+            ah += a_step; al += a_step; bh += 2; bl += 2;
             --ks_left;
-            if (++in_slot == P.kps || ks_left == 0) {
+            if (++in_slot == kps || ks_left == 0) {
               in_slot = 0;
-              if (++in_group == P.gslots || ks_left == 0) {
+              d_hi += slot_cols;
+              if (++in_group == gslots || ks_left == 0) {
                 tc_commit(&group_full[grp]);
                 in_group = 0;
-                if (++grp == (uint32_t)P.n_groups) { grp = 0; gphase ^= 1u; }
+                if (++grp == n_groups) { grp = 0; gphase ^= 1u; }
+                d_hi = tmem + slot_cols * (1u + grp * gslots);
               }
             }
           }
           tc_commit(&raw_empty[rs]);  // frees the stages when these MMAs have read them
           tc_commit(&lo_empty[ls]);
-          if (++rs == (uint32_t)P.n_raw) rs = 0;
+          if (++rs == n_raw) rs = 0;
           if (++ls == U_LO_STAGES) { ls = 0; lphase ^= 1u; }
         }
         ++item_ctr;
