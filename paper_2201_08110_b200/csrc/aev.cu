@@ -124,14 +124,18 @@ __device__ __forceinline__ float gauss(float d, float khi, float klo) {
 
 constexpr int AEV_THREADS = 256;  // one CTA per centre atom
 constexpr int TAB_FIELDS = 10;    // per radial slot: ux uy uz rhi rlo fcr dfcr fca dfca spec
-constexpr int TRIP_CHUNK_MAX = 1024;  // triplets of a centre processed per pass through shared memory
+// triplets of a centre processed per pass through shared memory: small enough that 6-8 CTAs share an SM (the
+// phases of a centre are latency-bound, other centres fill the gaps), measured on configs[2] and configs[4]
+constexpr int TRIP_CHUNK_FWD = 256;
+constexpr int TRIP_CHUNK_BWD = 512;
 
 // triplets per pass: enough for every centre of this handle, a multiple of 32, bounded
-static int trip_chunk(const nnp_handle* h) {
+static int trip_chunk(const nnp_handle* h, bool backward) {
   const long long t = (long long)h->capA * (h->capA - 1) / 2;
   long long c = (t + 31) / 32 * 32;
   if (c < 32) c = 32;
-  if (c > TRIP_CHUNK_MAX) c = TRIP_CHUNK_MAX;
+  const int cap = backward ? TRIP_CHUNK_BWD : TRIP_CHUNK_FWD;
+  if (c > cap) c = cap;
   return (int)c;
 }
 static int ang_row_pad(const nnp_handle* h) {  // floats per padded angular block of the staged dE/dAEV row
@@ -146,7 +150,7 @@ static size_t aev_common_floats(const nnp_handle* h) {
 size_t aev_smem_bytes(const nnp_handle* h, bool backward) {
   size_t fl = aev_common_floats(h);
   const int n_pairs = h->S * (h->S + 1) / 2;
-  const int CH = trip_chunk(h);
+  const int CH = trip_chunk(h, backward);
   if (!backward) {
     fl += (size_t)(h->n_feat - h->aev.n_radial);                       // angular part of the row
     fl += (size_t)(h->aev.n_shf_z + h->aev.n_shf_a) * CH;              // F1 / F2 factors of a pass
@@ -616,12 +620,12 @@ void launch_aev_forward(nnp_handle* h, cudaStream_t s) {
   const size_t smem = aev_smem_bytes(h, false);
   if (aev_small_shape(h))
     launch_kernel(h->pdl_now, aev_forward_kernel<4, 8>, dim3(blocks), dim3(AEV_THREADS), smem, s, h->d_pos4, h->d_nbr_r,
-                  h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA, trip_chunk(h),
+                  h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA, trip_chunk(h, false),
                   h->d_aev);
   else
     launch_kernel(h->pdl_now, aev_forward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>, dim3(blocks), dim3(AEV_THREADS), smem, s,
                   h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR,
-                  h->capA, trip_chunk(h), h->d_aev);
+                  h->capA, trip_chunk(h, false), h->d_aev);
 }
 
 void launch_aev_backward(nnp_handle* h, cudaStream_t s) {
@@ -631,11 +635,11 @@ void launch_aev_backward(nnp_handle* h, cudaStream_t s) {
   if (aev_small_shape(h))
     launch_kernel(h->pdl_now, aev_backward_kernel<4, 8>, dim3(blocks), dim3(AEV_THREADS), smem, s, h->d_pos4,
                   h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA,
-                  trip_chunk(h), (const float*)h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
+                  trip_chunk(h, true), (const float*)h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
   else
     launch_kernel(h->pdl_now, aev_backward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>, dim3(blocks), dim3(AEV_THREADS), smem, s,
                   h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR,
-                  h->capA, trip_chunk(h), (const float*)h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
+                  h->capA, trip_chunk(h, true), (const float*)h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
 }
 
 void launch_finish(nnp_handle* h, const int* d_atom_index, double* d_energy, float* d_force, int force_stride,
