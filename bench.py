@@ -122,7 +122,7 @@ class ClockSampler:
 
 # ------------------------------------------------------------------------------------------------
 KERNEL_OF_STAGE = {  # ligand-size engine / tensor-core engine
-    "ligand": {"mlp_fwd_l1": "small_fwd_kernel", "mlp_mid": "small_mid_kernel", "mlp_bwd_l1": "small_bwd1_kernel"},
+    "ligand": {"mlp_fwd_l1": "small_fwd1_kernel", "mlp_mid": "small_mid_kernel", "mlp_bwd_l1": "small_bwd1_kernel"},
     "tensor": {"mlp_fwd_l1": "gemm_umma_kernel", "mlp_fwd_l2": "gemm_umma_kernel", "mlp_fwd_l3": "gemm_umma_kernel",
                "mlp_bwd_l3": "gemm_umma_kernel", "mlp_bwd_l2": "gemm_umma_kernel", "mlp_bwd_l1": "gemm_umma_kernel"},
 }

@@ -22,6 +22,7 @@ NNP_FLAG_NO_MID = 16
 NNP_FLAG_NO_PDL = 32
 NNP_FLAG_NO_CELLS = 64
 NNP_FLAG_FORCE_CELLS = 128
+NNP_FLAG_NO_FWD1 = 256
 ERRORS = {
     -1: "NNP_ERR_INVALID_ARG",
     -2: "NNP_ERR_CUDA",

@@ -433,6 +433,179 @@ __global__ void __launch_bounds__(SM_THREADS, 1) small_bwd1_kernel(const SmallBw
 }
 
 // ------------------------------------------------------------------------------------------------
+// forward through layer 1 (the 43 MB layer): out[a][r] = CELU(b[r] + sum_k W[r][k] X[a][k]),  K = 1008
+// ------------------------------------------------------------------------------------------------
+// Persistent: one CTA per SM-sized share of ONE element's weight rows (the rows of all models of an (element,
+// layer 1) block are contiguous).  The element's AEV rows (<= 24 atoms) are staged in shared memory once; a
+// producer warp streams the weight rows as 12-row tiles (bulk async copies, one per row, padded pitch) through a
+// ring and runs ahead of the 8 consumer warps, starting before griddepcontrol.wait (weights are constant data),
+// so the weight fetch is continuous: the launch is bound by HBM when the step starts with a cold L2.
+// Consumers: a register-tiled contraction.  A thread owns 3 rows x AG atoms and one of 16 interleaved slices
+// of K; per 4-wide k-step it loads 3 weight + AG activation float4 (conflict-free, mostly broadcast) and issues
+// 3 x AG x 2 FFMA2 (the two halves of a float4 dot product run as a packed pair).  The 16 slice partials of an
+// output are summed in a fixed order: one shuffle (the two slices of a warp), then the 8 warps through shared
+// memory; bias + CELU fused.
+constexpr int F1_ROWS = 12;               // rows per tile: 4 row groups x 3
+constexpr int F1_CONSUMERS = 256;
+constexpr int F1_THREADS = F1_CONSUMERS + 32;
+constexpr int F1_MAX_STAGES = 6;
+static const size_t F1_SMEM = 200 * 1024;
+
+__host__ __device__ __forceinline__ int f1_pitch(int K) { return (K & 7) == 0 ? K + 4 : K; }  // == 4 (mod 8) words
+__host__ __device__ __forceinline__ int f1_pad_atoms(int n) { return n <= 4 ? 4 : n <= 8 ? 8 : n <= 16 ? 16 : 24; }
+__host__ __device__ __forceinline__ int f1_stages(int n_atoms, int K) {
+  const size_t P = (size_t)f1_pitch(K) * 4;
+  const int NAT = f1_pad_atoms(n_atoms);
+  const size_t fixed = (size_t)NAT * P + (size_t)(F1_CONSUMERS / 32) * F1_ROWS * NAT * 4;
+  const long long st = ((long long)F1_SMEM - (long long)fixed) / (long long)(F1_ROWS * P);
+  return st > F1_MAX_STAGES ? F1_MAX_STAGES : (int)st;
+}
+__device__ __forceinline__ void sbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(s_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void f1_consumer_sync() { asm volatile("bar.sync 1, %0;" ::"n"(F1_CONSUMERS) : "memory"); }
+// packed pair of floats <-> 64-bit register (FFMA2 operands)
+__device__ __forceinline__ unsigned long long f1_pack(float x, float y) {
+  unsigned long long d;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(x), "f"(y));
+  return d;
+}
+__device__ __forceinline__ unsigned long long f1_ffma2(unsigned long long a, unsigned long long b, unsigned long long c) {
+  unsigned long long d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ float f1_sum2(unsigned long long v) {
+  float x, y;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(v));
+  return x + y;
+}
+
+template <int AG>
+__device__ __forceinline__ void small_fwd1_body(const Fwd1Item& it, float* smem_f, uint64_t* full, uint64_t* empty,
+                                                uint64_t* xbar) {
+  constexpr int NAT = 4 * AG;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int K4 = it.K >> 2, P = f1_pitch(it.K);
+  const int n_stages = f1_stages(it.n_atoms, it.K);
+  const int n_tiles = (it.n_rows + F1_ROWS - 1) / F1_ROWS;
+  float* Xs = smem_f;                                  // [NAT][P]
+  float* Ws = Xs + (size_t)NAT * P;                    // [n_stages][F1_ROWS][P]
+  float* red = Ws + (size_t)n_stages * F1_ROWS * P;    // [warps][F1_ROWS][NAT]
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < n_stages; ++s) {
+      sbar_init(&full[s], 1);
+      sbar_init(&empty[s], F1_CONSUMERS / 32);
+    }
+    sbar_init(xbar, 1);
+    sbar_expect_tx(xbar, (uint32_t)(it.n_atoms * it.K * 4));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  pdl_trigger();
+
+  if (warp == F1_CONSUMERS / 32) {
+    // ------------------------------------------------------------ producer warp: weight tiles, lane r = row r
+    uint32_t slot = 0, phase = 0;
+    for (int t = 0; t < n_tiles; ++t) {
+      const int rows = min(F1_ROWS, it.n_rows - t * F1_ROWS);
+      if (lane == 0) {
+        sbar_wait(&empty[slot], phase ^ 1u);
+        sbar_expect_tx(&full[slot], (uint32_t)(rows * it.K * 4));
+      }
+      __syncwarp();
+      if (lane < rows)
+        bulk_g2s(Ws + ((size_t)slot * F1_ROWS + lane) * P, it.W + ((size_t)t * F1_ROWS + lane) * it.K,
+                 (uint32_t)(it.K * 4), &full[slot]);
+      if (++slot == (uint32_t)n_stages) { slot = 0; phase ^= 1u; }
+    }
+    pdl_wait();
+    return;
+  }
+  // -------------------------------------------------------------- consumers
+  const int tid = threadIdx.x;
+  for (int idx = it.n_atoms * P + tid; idx < NAT * P; idx += F1_CONSUMERS) Xs[idx] = 0.0f;  // rows of padding atoms
+  pdl_wait();  // the AEV rows come from the previous kernel
+  if (tid < it.n_atoms) bulk_g2s(Xs + (size_t)tid * P, it.X + (size_t)tid * it.ldx, (uint32_t)(it.K * 4), xbar);
+  f1_consumer_sync();
+  sbar_wait(xbar, 0);
+
+  // lane = (k-slice pair, atom group, row group); the two slices of a warp are 4 float4 apart, which together with
+  // the pitch == 20 (mod 32) words keeps the 8 distinct 16-byte addresses of a weight load on different banks
+  const int rg = lane & 3, ag = (lane >> 2) & 3, ks2 = lane >> 4;
+  const int slice = (warp & 3) + 8 * (warp >> 2) + 4 * ks2;
+  const float4* xs4 = reinterpret_cast<const float4*>(Xs);
+  const int P4 = P >> 2;
+  uint32_t slot = 0, phase = 0;
+  for (int t = 0; t < n_tiles; ++t) {
+    sbar_wait(&full[slot], phase);
+    const float4* ws4 = reinterpret_cast<const float4*>(Ws + (size_t)slot * F1_ROWS * P);
+    unsigned long long acc[3][AG];
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+      for (int j = 0; j < AG; ++j) acc[i][j] = 0ull;
+#pragma unroll 2
+    for (int k4 = slice; k4 < K4; k4 += F1_CONSUMERS / 16) {
+      unsigned long long wlo[3], whi[3];
+#pragma unroll
+      for (int i = 0; i < 3; ++i) {
+        const float4 w = ws4[(rg + 4 * i) * P4 + k4];
+        wlo[i] = f1_pack(w.x, w.y);
+        whi[i] = f1_pack(w.z, w.w);
+      }
+#pragma unroll
+      for (int j = 0; j < AG; ++j) {
+        const float4 x = xs4[(ag + 4 * j) * P4 + k4];
+        const unsigned long long xlo = f1_pack(x.x, x.y), xhi = f1_pack(x.z, x.w);
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+          acc[i][j] = f1_ffma2(wlo[i], xlo, acc[i][j]);
+          acc[i][j] = f1_ffma2(whi[i], xhi, acc[i][j]);
+        }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) sbar_arrive(&empty[slot]);  // the tile has been read: the producer may refill the stage
+    if (++slot == (uint32_t)n_stages) { slot = 0; phase ^= 1u; }
+    // slice partials: the warp's two slices by one shuffle, then the warps through shared memory (fixed order)
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+      for (int j = 0; j < AG; ++j) {
+        float v = f1_sum2(acc[i][j]);
+        v += __shfl_xor_sync(0xffffffffu, v, 16);
+        if (ks2 == 0) red[((size_t)warp * F1_ROWS + rg + 4 * i) * NAT + ag + 4 * j] = v;
+      }
+    f1_consumer_sync();
+    const int r0 = t * F1_ROWS;
+    for (int idx = tid; idx < F1_ROWS * NAT; idx += F1_CONSUMERS) {
+      const int a = idx / F1_ROWS, r = idx - a * F1_ROWS;  // consecutive threads -> consecutive rows (coalesced stores)
+      if (a < it.n_atoms && r0 + r < it.n_rows) {
+        float v = red[(size_t)r * NAT + a];
+#pragma unroll
+        for (int w = 1; w < F1_CONSUMERS / 32; ++w) v += red[((size_t)w * F1_ROWS + r) * NAT + a];
+        const float b = it.bias ? it.bias[r0 + r] : 0.0f;
+        it.out[(size_t)a * it.ldc + r0 + r] = celu_s(v + b, it.alpha, it.inv_alpha);
+      }
+    }
+    f1_consumer_sync();  // red is reused by the next tile
+  }
+}
+
+__global__ void __launch_bounds__(F1_THREADS, 1) small_fwd1_kernel(const Fwd1Item* __restrict__ items) {
+  extern __shared__ __align__(16) float smem_f[];
+  __shared__ __align__(8) uint64_t full[F1_MAX_STAGES];
+  __shared__ __align__(8) uint64_t empty[F1_MAX_STAGES];
+  __shared__ __align__(8) uint64_t xbar;
+  const Fwd1Item it = items[blockIdx.x];
+  if (it.n_atoms <= 4) small_fwd1_body<1>(it, smem_f, full, empty, &xbar);
+  else if (it.n_atoms <= 8) small_fwd1_body<2>(it, smem_f, full, empty, &xbar);
+  else if (it.n_atoms <= 16) small_fwd1_body<4>(it, smem_f, full, empty, &xbar);
+  else small_fwd1_body<6>(it, smem_f, full, empty, &xbar);
+}
+
+// ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
 static const size_t SMALL_SMEM_MAX = 200 * 1024;
@@ -451,6 +624,7 @@ int small_init() {
   rc |= set_smem(small_fwd_kernel<8>, SMALL_SMEM_MAX);
   rc |= set_smem(small_bwd_kernel, SMALL_SMEM_MAX);
   rc |= set_smem(small_bwd1_kernel, SMALL_SMEM_MAX);
+  rc |= set_smem(small_fwd1_kernel, F1_SMEM);
   return rc;
 }
 
@@ -522,8 +696,29 @@ int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items) {
   return 0;
 }
 
+// persistent layer-1 forward items (one CTA each, heavy first)
+int small_build_fwd1(SmallLaunch& L, std::vector<Fwd1Item>& items) {
+  std::stable_sort(items.begin(), items.end(), [](const Fwd1Item& a, const Fwd1Item& b) {
+    return (long long)a.n_rows * (16 + a.n_atoms) > (long long)b.n_rows * (16 + b.n_atoms);
+  });
+  L.n_items = (int)items.size();
+  L.variant = 101;
+  L.smem_bytes = F1_SMEM;
+  for (const auto& it : items)
+    if (it.n_atoms < 1 || it.n_atoms > 24 || (it.K & 3) || f1_stages(it.n_atoms, it.K) < 2) return -1;
+  if (cudaMalloc(&L.d_items, std::max<size_t>(1, items.size()) * sizeof(Fwd1Item)) != cudaSuccess) return -1;
+  if (!items.empty()) cudaMemcpy(L.d_items, items.data(), items.size() * sizeof(Fwd1Item), cudaMemcpyHostToDevice);
+  return 0;
+}
+int small_fwd1_tile_rows() { return F1_ROWS; }
+
 void small_launch_fwd(const SmallLaunch& L, cudaStream_t s, bool pdl) {
   if (L.n_items == 0) return;
+  if (L.variant == 101) {
+    launch_kernel(pdl, small_fwd1_kernel, dim3(L.n_items), dim3(F1_THREADS), L.smem_bytes, s,
+                  reinterpret_cast<const Fwd1Item*>(L.d_items));
+    return;
+  }
   const SmallFwdItem* it = reinterpret_cast<const SmallFwdItem*>(L.d_items);
   const dim3 g(L.n_items), b(SM_THREADS);
   switch (L.variant) {

@@ -581,7 +581,66 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     }
     const int l_fwd_end = h->use_mid ? 2 : L;   // forward layers run by the per-layer kernels: [1, l_fwd_end)
     const int l_bwd_begin = h->use_mid ? 1 : L - 1;
-    for (int l = 1; l < l_fwd_end; ++l) {  // forward
+    bool fwd1_done = false;
+    if (!(cfg->flags & NNP_FLAG_NO_FWD1)) {
+      // layer 1 forward: persistent CTAs, each streams a share of ONE element's weight rows (all models of the
+      // element are contiguous); shares are proportional to (row tiles) x (streaming + compute cost per tile)
+      struct Work { int e, a0, na; long long tiles; double cost; int n_cta; };
+      std::vector<Work> work;
+      const int TR = small_fwd1_tile_rows();
+      double total = 0;
+      for (int e = 0; e < S; ++e) {
+        const int ne = h->grp_off[e + 1] - h->grp_off[e];
+        const long long rows = (long long)M * h->dims[e * (L + 1) + 1];
+        for (int a0 = 0; a0 < ne; a0 += 24) {
+          Work wk{e, a0, std::min(24, ne - a0), (rows + TR - 1) / TR, 0.0, 1};
+          wk.cost = (double)wk.tiles * (16 + wk.na);
+          total += wk.cost;
+          work.push_back(wk);
+        }
+      }
+      const int budget = std::max(prop.multiProcessorCount, (int)work.size());
+      int used = 0;
+      for (auto& wk : work) {
+        wk.n_cta = (int)std::max<long long>(1, std::min<long long>(wk.tiles, (long long)(wk.cost / total * budget)));
+        used += wk.n_cta;
+      }
+      for (bool grew = true; grew && used < budget;) {  // hand the remaining CTAs to the most loaded shares
+        grew = false;
+        Work* best = nullptr;
+        for (auto& wk : work)
+          if (wk.n_cta < wk.tiles && (!best || wk.cost / wk.n_cta > best->cost / best->n_cta)) best = &wk;
+        if (best) { ++best->n_cta; ++used; grew = true; }
+      }
+      std::vector<Fwd1Item> items;
+      for (const auto& wk : work) {
+        const int e = wk.e, nout = h->dims[e * (L + 1) + 1];
+        const long long rows = (long long)M * nout;
+        const long long tiles_per = (wk.tiles + wk.n_cta - 1) / wk.n_cta;
+        for (long long t0 = 0; t0 < wk.tiles; t0 += tiles_per) {
+          const long long r0 = t0 * TR, r1 = std::min(rows, (t0 + tiles_per) * TR);
+          Fwd1Item it;
+          memset(&it, 0, sizeof(it));
+          it.W = h->d_W + h->w_off[e * L + 0] + (size_t)r0 * n_feat;
+          it.X = h->d_aev + (size_t)(h->grp_off[e] + wk.a0) * n_feat;
+          it.bias = h->d_b + h->b_off[e * L + 0] + r0;
+          it.out = h->d_act[1] + h->act_off[1][e] + (size_t)wk.a0 * M * nout + r0;
+          it.ldx = n_feat; it.ldc = M * nout;
+          it.n_atoms = wk.na; it.K = n_feat; it.n_rows = (int)(r1 - r0);
+          it.alpha = alpha; it.inv_alpha = inv_alpha;
+          items.push_back(it);
+        }
+      }
+      SmallLaunch sl;
+      sl.name = "mlp_fwd_l1";
+      if (small_build_fwd1(sl, items) == 0) {
+        h->sfwd.push_back(sl);
+        fwd1_done = true;
+      } else {
+        small_free_launch(sl);  // shapes the persistent kernel does not take: per-layer kernel below
+      }
+    }
+    for (int l = fwd1_done ? 2 : 1; l < l_fwd_end; ++l) {  // forward
       std::vector<SmallFwdItem> items;
       for (int e = 0; e < S; ++e) {
         const int ne = h->grp_off[e + 1] - h->grp_off[e];

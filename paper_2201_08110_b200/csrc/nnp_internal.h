@@ -179,6 +179,14 @@ struct SmallBwdItem {       // out[a*ldo + n] = epi(sum_o D[a*ldd + o] W[o*ldw +
   int epi, AW, G;           // atoms per warp (1..4), atom groups (1,2,4,8): G*AW >= n_atoms
   float scale, inv_alpha, b_last;
 };
+struct Fwd1Item {            // persistent layer-1 forward item: one CTA, a run of weight rows of one element
+  const float* W;            // first weight row of the run (row-major, pitch K); rows of all models are contiguous
+  const float* X;            // AEV row of the item's first atom (pitch ldx)
+  const float* bias;         // bias of the first row, or null
+  float* out;                // out[a*ldc + r] at (first atom, first row)
+  int ldx, ldc, n_atoms, K, n_rows;  // n_atoms <= 24, K % 4 == 0
+  float alpha, inv_alpha;
+};
 struct SmallLaunch {
   void* d_items = nullptr;
   int n_items = 0, variant = 1;
@@ -189,7 +197,9 @@ int small_init();
 void small_bwd_shape(int n_atoms, int* AW, int* G);
 int small_build_fwd(SmallLaunch& L, std::vector<SmallFwdItem>& items);
 int small_build_bwd(SmallLaunch& L, std::vector<SmallBwdItem>& items);
-int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items);  // layer 1: weights read once, FFMA2
+int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items);
+int small_build_fwd1(SmallLaunch& L, std::vector<Fwd1Item>& items);
+int small_fwd1_tile_rows();  // layer 1: persistent, weights streamed through a ring  // layer 1: weights read once, FFMA2
 void small_launch_fwd(const SmallLaunch& L, cudaStream_t s, bool pdl);
 void small_launch_bwd(const SmallLaunch& L, cudaStream_t s, bool pdl);
 void small_free_launch(SmallLaunch& L);
