@@ -142,10 +142,10 @@ static int ang_row_pad(const nnp_handle* h) {  // floats per padded angular bloc
   return h->aev.n_sub + 4;
 }
 
-// shared memory (floats): table | asl[capA] | sp_off[S+1] | pair_st[n_pairs] | kernel-specific part
+// shared memory (floats): table | asl[capA] | sp_off[S+1] | pair_st[n_pairs] | tmp[2 capA] | pres[n_pairs+1] | kernel part
 static size_t aev_common_floats(const nnp_handle* h) {
   const int S = h->S;
-  return (size_t)TAB_FIELDS * h->capR + h->capA + (S + 1) + (size_t)S * (S + 1) / 2;
+  return (size_t)TAB_FIELDS * h->capR + 3 * (size_t)h->capA + (S + 1) + (size_t)S * (S + 1) + 1;
 }
 size_t aev_smem_bytes(const nnp_handle* h, bool backward) {
   size_t fl = aev_common_floats(h);
@@ -168,6 +168,8 @@ struct CentreTab {
   int* asl;      // angular neighbours: radial slots, sorted by species (stable)
   int* sp_off;   // [S+1] first position in asl of every species
   int* pair_st;  // [n_pairs] (s << 8) | t of every species-pair block, s <= t
+  int* tmp;      // [2 capA] scratch of build_tab: angular slots and their species in list order
+  int* pres;     // [n_pairs + 1] species-pair blocks that have at least one triplet (ascending), count at [n_pairs]
   float* rest;   // kernel-specific part (16-byte aligned)
 };
 
@@ -179,7 +181,9 @@ __device__ __forceinline__ CentreTab carve_tab(float* smem, int capR, int capA, 
   t.asl = t.spec + capR;
   t.sp_off = t.asl + capA;
   t.pair_st = t.sp_off + (S + 1);
-  const int used = TAB_FIELDS * capR + capA + (S + 1) + S * (S + 1) / 2;
+  t.tmp = t.pair_st + S * (S + 1) / 2;
+  t.pres = t.tmp + 2 * capA;
+  const int used = TAB_FIELDS * capR + 3 * capA + (S + 1) + S * (S + 1) + 1;
   t.rest = smem + ((used + 3) & ~3);
   return t;
 }
@@ -189,15 +193,20 @@ __device__ __forceinline__ CentreTab carve_tab(float* smem, int capR, int capA, 
 // species-pair block are index ranges), the species offsets and the block -> species-pair table.
 __device__ __forceinline__ void build_tab(const CentreTab& t, int i, int nr, int na, const float4 pi,
                                           const float4* __restrict__ pos4, const int* __restrict__ nbr_r,
-                                          const int* __restrict__ nbr_a, int capR, int capA, const AevConst& c) {
+                                          const int* __restrict__ nbr_a, int capR, int capA, const AevConst& c,
+                                          bool want_pres) {
   for (int q = threadIdx.x; q < nr; q += blockDim.x) {
     const int j = nbr_r[(size_t)i * capR + q];
     const float4 pj = pos4[j];
     const double dx = (double)pj.x - (double)pi.x;
     const double dy = (double)pj.y - (double)pi.y;
     const double dz = (double)pj.z - (double)pi.z;
-    const double r = sqrt(dx * dx + dy * dy + dz * dz);
-    const double inv = 1.0 / r;
+    // 1/r by two Newton steps on the FP32 rsqrt seed (relative error 1e-7 -> 1e-14 -> rounding), r = r2 / r
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    double inv = (double)rsqrtf((float)r2);
+    inv = inv * (1.5 - 0.5 * r2 * inv * inv);
+    inv = inv * (1.5 - 0.5 * r2 * inv * inv);
+    const double r = r2 * inv;
     t.ux[q] = (float)(dx * inv);
     t.uy[q] = (float)(dy * inv);
     t.uz[q] = (float)(dz * inv);
@@ -220,21 +229,49 @@ __device__ __forceinline__ void build_tab(const CentreTab& t, int i, int nr, int
     for (int u = s; u < c.S; ++u) t.pair_st[p++] = (s << 8) | u;
   }
   __syncthreads();
-  // stable counting sort of the angular list by species: rank = #(smaller species) + #(same, earlier)
+  // the angular slots and their species, staged once (the sort below reads them na times)
   for (int q = threadIdx.x; q < na; q += blockDim.x) {
     const int slot = nbr_a[(size_t)i * capA + q];
-    const int sp = t.spec[slot];
+    t.tmp[q] = slot;
+    t.tmp[capA + q] = t.spec[slot];
+  }
+  __syncthreads();
+  // stable counting sort of the angular list by species: rank = #(smaller species) + #(same, earlier)
+  for (int q = threadIdx.x; q < na; q += blockDim.x) {
+    const int sp = t.tmp[capA + q];
     int rank = 0;
+#pragma unroll 4
     for (int q2 = 0; q2 < na; ++q2) {
-      const int s2 = t.spec[nbr_a[(size_t)i * capA + q2]];
+      const int s2 = t.tmp[capA + q2];
       rank += (s2 < sp) || (s2 == sp && q2 < q);
     }
-    t.asl[rank] = slot;
+    t.asl[rank] = t.tmp[q];
   }
   for (int s = threadIdx.x; s <= c.S; s += blockDim.x) {
     int cnt = 0;
-    for (int q2 = 0; q2 < na; ++q2) cnt += t.spec[nbr_a[(size_t)i * capA + q2]] < s;
+#pragma unroll 4
+    for (int q2 = 0; q2 < na; ++q2) cnt += t.tmp[capA + q2] < s;
     t.sp_off[s] = cnt;
+  }
+  __syncthreads();
+  if (!want_pres) return;  // CTA-uniform
+  // species-pair blocks with at least one triplet, in ascending order (ballot compaction by the first warp)
+  if (threadIdx.x < 32) {
+    const int n_pairs = (c.S * (c.S + 1)) >> 1;
+    int count = 0;
+    for (int base = 0; base < n_pairs; base += 32) {
+      const int p = base + (int)threadIdx.x;
+      bool has = false;
+      if (p < n_pairs) {
+        const int st = t.pair_st[p], s = st >> 8, u = st & 255;
+        const int ns = t.sp_off[s + 1] - t.sp_off[s], nu = t.sp_off[u + 1] - t.sp_off[u];
+        has = s == u ? ns >= 2 : (ns > 0 && nu > 0);
+      }
+      const unsigned b = __ballot_sync(FULL, has);
+      if (has) t.pres[count + __popc(b & ((1u << threadIdx.x) - 1u))] = p;
+      count += __popc(b);
+    }
+    if (threadIdx.x == 0) t.pres[n_pairs] = count;
   }
   __syncthreads();
 }
@@ -280,7 +317,7 @@ __global__ void __launch_bounds__(AEV_THREADS) aev_forward_kernel(
   const float4 pi = pos4[i];
   const int nr = cnt_r[i], na = cnt_a[i];
   for (int f = threadIdx.x; f < n_ang; f += blockDim.x) row[f] = 0.0f;
-  build_tab(t, i, nr, na, pi, pos4, nbr_r, nbr_a, capR, capA, c);
+  build_tab(t, i, nr, na, pi, pos4, nbr_r, nbr_a, capR, capA, c, true);
   float* out = aev + (size_t)sortpos[i] * c.n_feat;
 
   // ---- radial (O3)
@@ -288,10 +325,11 @@ __global__ void __launch_bounds__(AEV_THREADS) aev_forward_kernel(
     const int s = col / c.n_shf_r, k = col % c.n_shf_r;
     const float shf = c.shf_r[k];
     float acc = 0.0f;
-    for (int q = 0; q < nr; ++q) {
-      if (t.spec[q] != s) continue;
+#pragma unroll 4
+    for (int q = 0; q < nr; ++q) {  // predicated (no branch): the exponentials of consecutive neighbours overlap
       const float d = (t.rhi[q] - shf) + t.rlo[q];
-      acc += 0.25f * gauss(d, c.kr_hi, c.kr_lo) * t.fcr[q];
+      const float v = 0.25f * gauss(d, c.kr_hi, c.kr_lo) * t.fcr[q];
+      acc += t.spec[q] == s ? v : 0.0f;
     }
     out[col] = acc;
   }
@@ -326,13 +364,14 @@ __global__ void __launch_bounds__(AEV_THREADS) aev_forward_kernel(
       }
     }
     __syncthreads();
-    for (int f = threadIdx.x; f < n_ang; f += blockDim.x) {
-      const int p = f / c.n_sub, sub = f - p * c.n_sub;
+    const int n_out = t.pres[(c.S * (c.S + 1)) >> 1] * c.n_sub;  // columns of the blocks that have triplets
+    for (int fo = threadIdx.x; fo < n_out; fo += blockDim.x) {
+      const int pp = fo / c.n_sub, sub = fo - pp * c.n_sub;
+      const int p = t.pres[pp], f = p * c.n_sub + sub;
       const int ia = sub / c.n_shf_z, iz = sub - ia * c.n_shf_z;
       const int st = t.pair_st[p];
       const int s = st >> 8, u = st & 255;
       const int a0 = t.sp_off[s], a1 = t.sp_off[s + 1], b0 = t.sp_off[u], b1 = t.sp_off[u + 1];
-      if (a0 == a1 || b0 == b1) continue;
       const float* f1 = bF1 + iz * CH;
       const float* f2 = bF2 + ia * CH;
       float acc = 0.0f;
@@ -365,7 +404,7 @@ __device__ __forceinline__ float warp_sum(float v) {
 }
 
 template <int NZ, int NA>
-__global__ void __launch_bounds__(AEV_THREADS) aev_backward_kernel(
+__global__ void __launch_bounds__(AEV_THREADS, 6) aev_backward_kernel(
     const float4* __restrict__ pos4, const int* __restrict__ nbr_r, const int* __restrict__ nbr_a,
     const int* __restrict__ cnt_r, const int* __restrict__ cnt_a, const int* __restrict__ sortpos, int N,
     const __grid_constant__ AevConst c, int capR, int capA, int CH, const float* __restrict__ daev, int n_parts,
@@ -385,24 +424,55 @@ __global__ void __launch_bounds__(AEV_THREADS) aev_backward_kernel(
   const float4 pi = pos4[i];
   const int nr = cnt_r[i], na = cnt_a[i];
   const float* gin = daev + (size_t)sortpos[i] * c.n_feat;
-  // dE/dAEV row = fixed-order sum of the partial rows; the loads of a column are independent
-  for (int f = threadIdx.x; f < c.n_feat; f += blockDim.x) {
-    float v = gin[f];
-    int p = 1;
-    for (; p + 4 <= n_parts; p += 4) {
-      const float v0 = gin[(size_t)p * part_stride + f], v1 = gin[(size_t)(p + 1) * part_stride + f];
-      const float v2 = gin[(size_t)(p + 2) * part_stride + f], v3 = gin[(size_t)(p + 3) * part_stride + f];
-      v += v0; v += v1; v += v2; v += v3;
+  // dE/dAEV row = fixed-order sum of the partial rows.  All loads of a pass (2 columns x 8 partial rows per thread)
+  // are issued before the first add: one memory latency per pass instead of one per partial row
+  if (n_parts == 1) {  // large systems: one row, keep as many columns in flight as possible
+    for (int fb = 0; fb < c.n_feat; fb += 8 * AEV_THREADS) {
+      float x[8];
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const int f = fb + k * AEV_THREADS + threadIdx.x;
+        x[k] = f < c.n_feat ? gin[f] : 0.0f;
+      }
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const int f = fb + k * AEV_THREADS + threadIdx.x;
+        if (f < c.n_radial) g[f] = x[k];
+        else if (f < c.n_feat) {
+          const int fa = f - c.n_radial, blk = fa / c.n_sub;
+          gang[blk * bpad + (fa - blk * c.n_sub)] = x[k];
+        }
+      }
     }
-    for (; p < n_parts; ++p) v += gin[(size_t)p * part_stride + f];
-    if (f < c.n_radial) g[f] = v;
-    else {
-      const int fa = f - c.n_radial, blk = fa / c.n_sub;
-      gang[blk * bpad + (fa - blk * c.n_sub)] = v;
+  }
+  for (int fb = 0; n_parts > 1 && fb < c.n_feat; fb += 2 * AEV_THREADS) {
+    float acc[2] = {0.0f, 0.0f};
+    for (int p0 = 0; p0 < n_parts; p0 += 8) {
+      float x[2][8];
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        const int f = fb + k * AEV_THREADS + threadIdx.x;
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+          x[k][u] = (f < c.n_feat && p0 + u < n_parts) ? gin[(size_t)(p0 + u) * part_stride + f] : 0.0f;
+      }
+#pragma unroll
+      for (int k = 0; k < 2; ++k)
+#pragma unroll
+        for (int u = 0; u < 8; ++u) acc[k] += x[k][u];
+    }
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const int f = fb + k * AEV_THREADS + threadIdx.x;
+      if (f < c.n_radial) g[f] = acc[k];
+      else if (f < c.n_feat) {
+        const int fa = f - c.n_radial, blk = fa / c.n_sub;
+        gang[blk * bpad + (fa - blk * c.n_sub)] = acc[k];
+      }
     }
   }
   for (int f = threadIdx.x; f < 3 * nr; f += blockDim.x) pha[f] = 0.0f;
-  build_tab(t, i, nr, na, pi, pos4, nbr_r, nbr_a, capR, capA, c);
+  build_tab(t, i, nr, na, pi, pos4, nbr_r, nbr_a, capR, capA, c, false);
 
   // ---- radial: dT/dr = 0.25 e (f_C' - 2 eta (r - Shf) f_C); a group of lanes per neighbour
   {
