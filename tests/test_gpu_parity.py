@@ -292,6 +292,46 @@ def test_small_parameter_sets(n_species, hidden, n, seed, engine):
     nnp.destroy()
 
 
+@pytest.mark.parametrize("hidden", [(24,), (32, 16), (32, 24, 16, 8)])
+@pytest.mark.parametrize("engine", ["small", "small_layers", "umma"])
+def test_network_depths(hidden, engine):
+    """n_layers = 2, 3 and 5 (the ANI-2x networks have 4): the fused middle launch handles any number of hidden
+    layers, and with a single hidden layer it is not used at all."""
+    p = wl.small_params(3, hidden)
+    w = wl.random_molecule(41, 3, seed=300 + len(hidden), params=p, n_models=2)
+    W, B = wl.make_weights(p, 2, seed=7, random_biases=True)
+    orc = AniOracle(p, W, B)
+    ref = orc.energy_forces(w.positions, w.species, want_intermediates=True)
+    nnp = NNP(p, W, B, w.species, flags=ENGINES[engine])
+    gpu = gpu_eval(nnp, w.positions, stages=True)
+    check_stages(gpu, ref, orc, w.positions, w.mol_offsets)
+    check_energy_forces(gpu, ref, w.mol_offsets, propagated_energy_tol(ref, w.mol_offsets, p.energy_scale))
+    nnp.destroy()
+
+
+def test_other_aev_hyperparameters():
+    """An ANI-1x-like AEV shape (8 angular sections, 4 angular shifts, integer zeta = 32, other etas and cutoffs):
+    the generic instantiation of the AEV kernels (register arrays sized for up to 8 x 16 sub-terms)."""
+    import dataclasses
+
+    base = wl.small_params(3, (32, 16, 8))
+    p = dataclasses.replace(
+        base, rc_radial=np.float32(5.2), rc_angular=np.float32(3.5), eta_r=np.float32(16.0), eta_a=np.float32(8.0),
+        zeta=np.float32(32.0), shf_r=(0.9 + 0.26875 * np.arange(16)).astype(np.float32),
+        shf_a=(0.9 + 0.65 * np.arange(4)).astype(np.float32),
+        shf_z=((2 * np.arange(8) + 1) * np.pi / 16).astype(np.float32))
+    assert p.n_features == base.n_features  # 4 x 8 = 8 x 4 sub-terms: same row length, different layout
+    w = wl.random_molecule(33, 3, seed=321, params=p, n_models=2)
+    W, B = wl.make_weights(p, 2, seed=8, random_biases=True)
+    orc = AniOracle(p, W, B)
+    ref = orc.energy_forces(w.positions, w.species, want_intermediates=True)
+    nnp = NNP(p, W, B, w.species)
+    gpu = gpu_eval(nnp, w.positions, stages=True)
+    check_stages(gpu, ref, orc, w.positions, w.mol_offsets)
+    check_energy_forces(gpu, ref, w.mol_offsets, propagated_energy_tol(ref, w.mol_offsets, p.energy_scale))
+    nnp.destroy()
+
+
 def test_degenerate_inputs():
     """Edge cases: a lone atom (zero AEV, energy = network at 0), a dimer, an empty molecule inside a
     batch, and an empty handle."""
