@@ -83,6 +83,7 @@ typedef struct {
 #define NNP_FLAG_NO_CELLS 64     /* neighbour search: all pairs inside a molecule even for large molecules */
 #define NNP_FLAG_FORCE_CELLS 128 /* neighbour search: cell binning even for small molecules (default: molecules >= 1024 atoms) */
 #define NNP_FLAG_NO_FWD1 256     /* ligand-size engine: row-pair layer-1 forward kernel instead of the persistent ring-fed one */
+#define NNP_FLAG_NO_NBR_FUSION 1024 /* small molecules: separate neighbour launch instead of building the rows inside the AEV forward kernel */
 #define NNP_FLAG_NO_PDL 32  /* plain stream-ordered launches instead of programmatic dependent launches along the chain */
 #define NNP_FLAG_NO_MID 16  /* ligand-size engine: one launch per layer instead of the fused middle-of-the-network launch */
 

@@ -18,38 +18,47 @@
 // D2 <= Rc^2.  Evaluated in FP64 for every candidate, so the pair sets are bit-exact by construction.
 // Rows come out sorted by j.  nbr_a stores the SLOT of the neighbour in the radial row.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) nbr_allpairs_kernel(
-    const float* __restrict__ pos, int pos_stride, const int* __restrict__ atom_index,
-    const int* __restrict__ species, const int* __restrict__ mol_id, const int* __restrict__ mol_off, int N,
-    AevConst c, int capR, int capA, float4* __restrict__ pos4, int* __restrict__ nbr_r, int* __restrict__ nbr_a,
-    int* __restrict__ cnt_r, int* __restrict__ cnt_a, int* __restrict__ status) {
-  const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int lane = threadIdx.x & 31;
-  pdl_trigger();
-  pdl_wait();  // the previous step's kernels still read the lists this kernel rewrites
-  if (i >= N) return;
-  const int m = mol_id[i];
-  const int lo = mol_off[m], hi = mol_off[m + 1];
-  const int rowi = atom_index ? atom_index[i] : i;
-  const float xi = pos[(size_t)rowi * pos_stride + 0] * c.length_scale;
-  const float yi = pos[(size_t)rowi * pos_stride + 1] * c.length_scale;
-  const float zi = pos[(size_t)rowi * pos_stride + 2] * c.length_scale;
+// raw inputs of the neighbour search (the caller's position buffer and the molecule topology)
+struct NbrArgs {
+  const float* pos;
+  const int* atom_index;
+  const int* species;
+  const int* mol_id;
+  const int* mol_off;
+  int* status;
+  int pos_stride;
+  float length_scale;
+};
+
+__device__ __forceinline__ float4 raw_pos4(const NbrArgs& a, int j) {
+  const int row = a.atom_index ? a.atom_index[j] : j;
+  const float* p = a.pos + (size_t)row * a.pos_stride;
+  return make_float4(p[0] * a.length_scale, p[1] * a.length_scale, p[2] * a.length_scale, __int_as_float(a.species[j]));
+}
+
+// one warp builds the radial and angular rows of centre i
+__device__ __forceinline__ void nbr_row_warp(const NbrArgs& a, int i, int lane, double rc_r2, double rc_a2, int capR,
+                                             int capA, float4* __restrict__ pos4, int* __restrict__ nbr_r,
+                                             int* __restrict__ nbr_a, int* __restrict__ cnt_r, int* __restrict__ cnt_a) {
+  const int m = a.mol_id[i];
+  const int lo = a.mol_off[m], hi = a.mol_off[m + 1];
+  const float4 pi = raw_pos4(a, i);
   if (lane == 0) {
-    pos4[i] = make_float4(xi, yi, zi, __int_as_float(species[i]));
-    if (!(isfinite(xi) && isfinite(yi) && isfinite(zi))) atomicOr(status, NNP_ST_NONFINITE);
+    pos4[i] = pi;
+    if (!(isfinite(pi.x) && isfinite(pi.y) && isfinite(pi.z))) atomicOr(a.status, NNP_ST_NONFINITE);
   }
   int nr = 0, na = 0;
   for (int base = lo; base < hi; base += 32) {
     const int j = base + lane;
     bool in_r = false, in_a = false;
     if (j < hi && j != i) {
-      const int rowj = atom_index ? atom_index[j] : j;
-      const double dx = (double)(pos[(size_t)rowj * pos_stride + 0] * c.length_scale) - (double)xi;
-      const double dy = (double)(pos[(size_t)rowj * pos_stride + 1] * c.length_scale) - (double)yi;
-      const double dz = (double)(pos[(size_t)rowj * pos_stride + 2] * c.length_scale) - (double)zi;
+      const float4 pj = raw_pos4(a, j);
+      const double dx = (double)pj.x - (double)pi.x;
+      const double dy = (double)pj.y - (double)pi.y;
+      const double dz = (double)pj.z - (double)pi.z;
       const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-      in_r = d2 <= c.rc_r2;
-      in_a = d2 <= c.rc_a2;
+      in_r = d2 <= rc_r2;
+      in_a = d2 <= rc_a2;
     }
     const unsigned br = __ballot_sync(FULL, in_r);
     const unsigned ba = __ballot_sync(FULL, in_a);
@@ -64,10 +73,22 @@ __global__ void __launch_bounds__(128) nbr_allpairs_kernel(
     na += __popc(ba);
   }
   if (lane == 0) {
-    if (nr > capR || na > capA) atomicOr(status, NNP_ST_CAPACITY);
+    if (nr > capR || na > capA) atomicOr(a.status, NNP_ST_CAPACITY);
     cnt_r[i] = min(nr, capR);
     cnt_a[i] = min(na, capA);
   }
+}
+
+__global__ void __launch_bounds__(128) nbr_allpairs_kernel(const __grid_constant__ NbrArgs a, int N, double rc_r2,
+                                                           double rc_a2, int capR, int capA, float4* __restrict__ pos4,
+                                                           int* __restrict__ nbr_r, int* __restrict__ nbr_a,
+                                                           int* __restrict__ cnt_r, int* __restrict__ cnt_a) {
+  const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  pdl_trigger();
+  pdl_wait();  // the previous step's kernels still read the lists this kernel rewrites
+  if (i >= N) return;
+  nbr_row_warp(a, i, lane, rc_r2, rc_a2, capR, capA, pos4, nbr_r, nbr_a, cnt_r, cnt_a);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -194,10 +215,10 @@ __device__ __forceinline__ CentreTab carve_tab(float* smem, int capR, int capA, 
 __device__ __forceinline__ void build_tab(const CentreTab& t, int i, int nr, int na, const float4 pi,
                                           const float4* __restrict__ pos4, const int* __restrict__ nbr_r,
                                           const int* __restrict__ nbr_a, int capR, int capA, const AevConst& c,
-                                          bool want_pres) {
+                                          bool want_pres, const NbrArgs* raw = nullptr) {
   for (int q = threadIdx.x; q < nr; q += blockDim.x) {
     const int j = nbr_r[(size_t)i * capR + q];
-    const float4 pj = pos4[j];
+    const float4 pj = raw ? raw_pos4(*raw, j) : pos4[j];  // fused neighbour search: pos4[j] is another CTA's job
     const double dx = (double)pj.x - (double)pi.x;
     const double dy = (double)pj.y - (double)pi.y;
     const double dz = (double)pj.z - (double)pi.z;
@@ -304,7 +325,9 @@ template <int NZ, int NA>
 __global__ void __launch_bounds__(AEV_THREADS) aev_forward_kernel(
     const float4* __restrict__ pos4, const int* __restrict__ nbr_r, const int* __restrict__ nbr_a,
     const int* __restrict__ cnt_r, const int* __restrict__ cnt_a, const int* __restrict__ sortpos, int N,
-    const __grid_constant__ AevConst c, int capR, int capA, int CH, float* __restrict__ aev) {
+    const __grid_constant__ AevConst c, int capR, int capA, int CH, float* __restrict__ aev,
+    const __grid_constant__ NbrArgs nb, int fused, float4* __restrict__ pos4_w, int* __restrict__ nbr_r_w,
+    int* __restrict__ nbr_a_w, int* __restrict__ cnt_r_w, int* __restrict__ cnt_a_w) {
   extern __shared__ __align__(16) float smem[];
   const int i = blockIdx.x;
   const CentreTab t = carve_tab(smem, capR, capA, c.S);
@@ -314,10 +337,18 @@ __global__ void __launch_bounds__(AEV_THREADS) aev_forward_kernel(
   float* bF2 = bF1 + c.n_shf_z * CH;   // [n_shf_a][CH]
   pdl_trigger();
   pdl_wait();
-  const float4 pi = pos4[i];
-  const int nr = cnt_r[i], na = cnt_a[i];
+  if (fused) {
+    // small molecules: the centre's CTA builds its own neighbour rows (first warp) instead of a separate launch;
+    // the rows also go to global memory for the backward and gather kernels
+    if (threadIdx.x < 32)
+      nbr_row_warp(nb, i, threadIdx.x, c.rc_r2, c.rc_a2, capR, capA, pos4_w, nbr_r_w, nbr_a_w, cnt_r_w, cnt_a_w);
+    __syncthreads();  // the CTA's own global writes are visible to the CTA
+  }
+  const float4 pi = fused ? raw_pos4(nb, i) : pos4[i];
+  const int nr = fused ? cnt_r_w[i] : cnt_r[i], na = fused ? cnt_a_w[i] : cnt_a[i];
   for (int f = threadIdx.x; f < n_ang; f += blockDim.x) row[f] = 0.0f;
-  build_tab(t, i, nr, na, pi, pos4, nbr_r, nbr_a, capR, capA, c, true);
+  build_tab(t, i, nr, na, pi, pos4, fused ? nbr_r_w : nbr_r, fused ? nbr_a_w : nbr_a, capR, capA, c, true,
+            fused ? &nb : nullptr);
   float* out = aev + (size_t)sortpos[i] * c.n_feat;
 
   // ---- radial (O3)
@@ -670,32 +701,44 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(
 // ------------------------------------------------------------------------------------------------
 // launch wrappers
 // ------------------------------------------------------------------------------------------------
+static NbrArgs nbr_args(nnp_handle* h, const float* d_pos, int pos_stride, const int* d_atom_index) {
+  NbrArgs a;
+  a.pos = d_pos; a.atom_index = d_atom_index; a.species = h->d_species; a.mol_id = h->d_mol_id; a.mol_off = h->d_mol_off;
+  a.status = h->d_status; a.pos_stride = pos_stride; a.length_scale = h->aev.length_scale;
+  return a;
+}
+
 void launch_neighbors(nnp_handle* h, const float* d_pos, int pos_stride, const int* d_atom_index, cudaStream_t s) {
-  if (h->N == 0) return;
+  if (h->N == 0 || h->fuse_nbr) return;  // fused: the AEV forward kernel builds the rows
   if (h->use_cells) {
     launch_neighbors_cells(h, d_pos, pos_stride, d_atom_index, s);
     return;
   }
   const int blocks = (h->N + 3) / 4;
-  nbr_allpairs_kernel<<<blocks, 128, 0, s>>>(d_pos, pos_stride, d_atom_index, h->d_species, h->d_mol_id,
-                                             h->d_mol_off, h->N, h->aev, h->capR, h->capA, h->d_pos4, h->d_nbr_r,
-                                             h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_status);
+  nbr_allpairs_kernel<<<blocks, 128, 0, s>>>(nbr_args(h, d_pos, pos_stride, d_atom_index), h->N, h->aev.rc_r2,
+                                             h->aev.rc_a2, h->capR, h->capA, h->d_pos4, h->d_nbr_r, h->d_nbr_a,
+                                             h->d_cnt_r, h->d_cnt_a);
 }
 
 static bool aev_small_shape(const nnp_handle* h) { return h->aev.n_shf_z <= 4 && h->aev.n_shf_a <= 8; }
 
-void launch_aev_forward(nnp_handle* h, cudaStream_t s) {
+void launch_aev_forward(nnp_handle* h, const float* d_pos, int pos_stride, const int* d_atom_index, cudaStream_t s) {
   if (h->N == 0) return;
   const int blocks = h->N;
   const size_t smem = aev_smem_bytes(h, false);
+  const NbrArgs nb = nbr_args(h, d_pos, pos_stride, d_atom_index);
+  const int fused = h->fuse_nbr ? 1 : 0;
+  const bool pdl = h->pdl_now && !fused;  // fused: first kernel of the step, must not overtake the previous step
   if (aev_small_shape(h))
-    launch_kernel(h->pdl_now, aev_forward_kernel<4, 8>, dim3(blocks), dim3(AEV_THREADS), smem, s, h->d_pos4, h->d_nbr_r,
-                  h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA, trip_chunk(h, false),
-                  h->d_aev);
+    launch_kernel(pdl, aev_forward_kernel<4, 8>, dim3(blocks), dim3(AEV_THREADS), smem, s, (const float4*)h->d_pos4,
+                  (const int*)h->d_nbr_r, (const int*)h->d_nbr_a, (const int*)h->d_cnt_r, (const int*)h->d_cnt_a,
+                  (const int*)h->d_sortpos, h->N, h->aev, h->capR, h->capA, trip_chunk(h, false), h->d_aev, nb, fused,
+                  h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a);
   else
-    launch_kernel(h->pdl_now, aev_forward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>, dim3(blocks), dim3(AEV_THREADS), smem, s,
-                  h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR,
-                  h->capA, trip_chunk(h, false), h->d_aev);
+    launch_kernel(pdl, aev_forward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>, dim3(blocks), dim3(AEV_THREADS), smem, s,
+                  (const float4*)h->d_pos4, (const int*)h->d_nbr_r, (const int*)h->d_nbr_a, (const int*)h->d_cnt_r,
+                  (const int*)h->d_cnt_a, (const int*)h->d_sortpos, h->N, h->aev, h->capR, h->capA,
+                  trip_chunk(h, false), h->d_aev, nb, fused, h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a);
 }
 
 void launch_aev_backward(nnp_handle* h, cudaStream_t s) {

@@ -272,6 +272,9 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       dev_alloc(&h->d_eatom, (size_t)N * M) || dev_alloc(&h->d_status, 1) || dev_alloc(&h->d_hpos, (size_t)N * 3) ||
       dev_alloc(&h->d_hforce, (size_t)N * 3) || dev_alloc(&h->d_henergy, (size_t)n_molecules))
     return fail(NNP_ERR_ALLOC);
+  // latency-bound sizes only: in a large batch the serial row build inside every centre's CTA costs more than the
+  // launch it saves (configs[2]: +36 us in the AEV forward against a 12 us neighbour kernel)
+  h->fuse_nbr = N > 0 && N <= 512 && !h->use_cells && max_mol <= 256 && !(cfg->flags & NNP_FLAG_NO_NBR_FUSION);
   if (h->use_cells && cells_alloc(h) != 0) return fail(NNP_ERR_ALLOC);
   cudaMemset(h->d_status, 0, sizeof(int));
   cudaMemset(h->d_nbr_r, 0, sizeof(int) * std::max<size_t>((size_t)N * h->capR, 1));
@@ -756,7 +759,8 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   h->work[2] = 2.0 * 4.0 * (double)N * n_feat;
   h->work[3] = w1bytes;
 
-  h->stage_names = {"nbr", "aev_fwd"};
+  if (h->fuse_nbr) h->stage_names = {"aev_fwd"};  // the AEV forward kernel builds the neighbour rows itself
+  else h->stage_names = {"nbr", "aev_fwd"};
   if (h->use_small) {
     for (auto& g : h->sfwd) h->stage_names.push_back(g.name);
     if (h->use_mid) h->stage_names.push_back(h->smid.name);
@@ -788,8 +792,8 @@ static void enqueue_chain(nnp_handle* h, const float* d_pos, int ps, const int* 
   h->pdl_now = h->use_pdl && !ev;  // event records between the kernels would break the programmatic edges
   const bool pdl = h->pdl_now;
   mark();
-  launch_neighbors(h, d_pos, ps, d_idx, s); mark();
-  launch_aev_forward(h, s); mark();
+  if (!h->fuse_nbr) { launch_neighbors(h, d_pos, ps, d_idx, s); mark(); }
+  launch_aev_forward(h, d_pos, ps, d_idx, s); mark();
   if (h->use_small) {  // per-atom energies and delta_L-1 come out of the first backward launch
     for (auto& g : h->sfwd) { small_launch_fwd(g, s, pdl); mark(); }
     if (h->use_mid) { mid_launch(h->smid, s, pdl); mark(); }

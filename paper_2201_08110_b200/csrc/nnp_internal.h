@@ -258,6 +258,7 @@ struct nnp_handle {
   double* d_eatom = nullptr;  // [N sorted][M]
   // cell-binned neighbour search (nbr_cells.cu), used for large molecules
   bool use_cells = false;
+  bool fuse_nbr = false;  // small molecules: the AEV forward kernel builds the neighbour rows itself
   void* d_cell_grid = nullptr;
   int *d_cell_count = nullptr, *d_cell_start = nullptr, *d_cell_of = nullptr, *d_cell_rank = nullptr,
       *d_cell_atoms = nullptr;
@@ -304,7 +305,7 @@ void launch_neighbors(nnp_handle* h, const float* d_pos, int pos_stride, const i
 int cells_alloc(nnp_handle* h);
 void cells_free(nnp_handle* h);
 void launch_neighbors_cells(nnp_handle* h, const float* d_pos, int pos_stride, const int* d_atom_index, cudaStream_t s);
-void launch_aev_forward(nnp_handle* h, cudaStream_t s);
+void launch_aev_forward(nnp_handle* h, const float* d_pos, int pos_stride, const int* d_atom_index, cudaStream_t s);
 void launch_aev_backward(nnp_handle* h, cudaStream_t s);
 void launch_gemm(const GemmLaunch& g, cudaStream_t s);
 void launch_last_layer(nnp_handle* h, cudaStream_t s);

@@ -15,12 +15,12 @@ torch = pytest.importorskip("torch")
 from oracle.ani_oracle import AniOracle  # noqa: E402
 from paper_2201_08110_b200 import workloads as wl  # noqa: E402
 from paper_2201_08110_b200.binding import (NNP, NNP_FLAG_FORCE_CELLS, NNP_FLAG_NO_CELLS, NNP_FLAG_NO_GRAPH,  # noqa: E402
-                                            NNP_FLAG_NO_FWD1, NNP_FLAG_NO_MID, NNP_FLAG_NO_PDL, NNP_FLAG_NO_SMALL, NNP_FLAG_NO_TMA,
+                                            NNP_FLAG_NO_FWD1, NNP_FLAG_NO_MID, NNP_FLAG_NO_NBR_FUSION, NNP_FLAG_NO_PDL, NNP_FLAG_NO_SMALL, NNP_FLAG_NO_TMA,
                                             NNP_FLAG_NO_UMMA, NNPError)
 
 # MLP engines: ligand-size weight-streaming FFMA (default at these sizes; with the fused middle launch or
 # one launch per layer), tcgen05 3xTF32, TMA+FFMA, plain FFMA
-ENGINES = {"small": 0, "small_layers": NNP_FLAG_NO_MID | NNP_FLAG_NO_FWD1, "umma": NNP_FLAG_NO_SMALL, "tma": NNP_FLAG_NO_SMALL | NNP_FLAG_NO_UMMA,
+ENGINES = {"small": 0, "small_layers": NNP_FLAG_NO_MID | NNP_FLAG_NO_FWD1 | NNP_FLAG_NO_NBR_FUSION, "umma": NNP_FLAG_NO_SMALL, "tma": NNP_FLAG_NO_SMALL | NNP_FLAG_NO_UMMA,
            "ffma": NNP_FLAG_NO_SMALL | NNP_FLAG_NO_UMMA | NNP_FLAG_NO_TMA}
 
 E_TOL_PER_ATOM = 1e-5  # kcal/mol
