@@ -322,7 +322,7 @@ __device__ __forceinline__ void trip_decode(int t, int na, int& a, int& b) {
 // NZ / NA are the register-array bounds (n_shf_z <= NZ, n_shf_a <= NA).
 // ------------------------------------------------------------------------------------------------
 template <int NZ, int NA>
-__global__ void __launch_bounds__(AEV_THREADS) aev_forward_kernel(
+__global__ void __launch_bounds__(AEV_THREADS, 6) aev_forward_kernel(
     const float4* __restrict__ pos4, const int* __restrict__ nbr_r, const int* __restrict__ nbr_a,
     const int* __restrict__ cnt_r, const int* __restrict__ cnt_a, const int* __restrict__ sortpos, int N,
     const __grid_constant__ AevConst c, int capR, int capA, int CH, float* __restrict__ aev,
