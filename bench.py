@@ -179,10 +179,31 @@ def stage_rooflines(w, nnp, stages, config):
         tf32_peak = 0.5 * bf16
         tsrc = "measured bf16 (MEASURED_PEAKS.json bf16_tflops) x 0.5 nominal TF32:BF16 ratio" if "bf16_tflops" in peaks \
             else "fallback 1650 TFLOP/s bf16 x 0.5"
+        # layer 1 skips the 32-wide contraction boxes (forward) / 128-wide output tiles (backward) that hold only AEV
+        # columns of absent species: quote the dense nominal flops AND the share actually issued
+        present = counts > 0
+        n_sub = p.shf_a.size * p.shf_z.size
+        live = np.zeros(int(dims[0, 0]), bool)
+        for s_ in range(dims.shape[0]):
+            live[s_ * p.shf_r.size:(s_ + 1) * p.shf_r.size] = present[s_]
+        pidx = 0
+        for s_ in range(dims.shape[0]):
+            for t_ in range(s_, dims.shape[0]):
+                live[p.n_radial + pidx * n_sub:p.n_radial + (pidx + 1) * n_sub] = present[s_] and present[t_]
+                pidx += 1
+        nb = (live.size + 31) // 32
+        nt = (live.size + 127) // 128
+        frac_f = sum(live[32 * b:32 * b + 32].any() for b in range(nb)) / nb
+        frac_b = sum(live[128 * b:128 * b + 128].any() for b in range(nt)) / nt
         for l in range(1, L):
             for st in (f"mlp_fwd_l{l}", f"mlp_bwd_l{l}"):
+                issued = (frac_f if st.startswith("mlp_fwd") else frac_b) if l == 1 else 1.0
                 add(st, "tensor", 2.0 * mac[l], "TFLOP/s", tf32_peak, tsrc,
-                    "useful flops; 3xTF32 issues 3 MMAs per useful MAC, so the ceiling of frac is 1/3")
+                    "dense nominal useful flops; 3xTF32 issues 3 MMAs per useful MAC (ceiling of frac 1/3); "
+                    f"share of the dense flops actually issued (structural zeros of absent species skipped): {issued:.3f}")
+                if out and out[-1]["stage"] == st:
+                    out[-1]["issued_fraction"] = issued
+                    out[-1]["achieved_issued"] = out[-1]["achieved"] * issued
     if not out:
         return None
     top = max(out, key=lambda d: d["kernel_us"])

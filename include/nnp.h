@@ -84,6 +84,7 @@ typedef struct {
 #define NNP_FLAG_FORCE_CELLS 128 /* neighbour search: cell binning even for small molecules (default: molecules >= 1024 atoms) */
 #define NNP_FLAG_NO_FWD1 256     /* ligand-size engine: row-pair layer-1 forward kernel instead of the persistent ring-fed one */
 #define NNP_FLAG_NO_NBR_FUSION 1024 /* small molecules: separate neighbour launch instead of building the rows inside the AEV forward kernel */
+#define NNP_FLAG_NO_ZERO_SKIP 2048 /* tensor engine: run layer 1 densely even over AEV columns that are structurally zero */
 #define NNP_FLAG_NO_PDL 32  /* plain stream-ordered launches instead of programmatic dependent launches along the chain */
 #define NNP_FLAG_NO_MID 16  /* ligand-size engine: one launch per layer instead of the fused middle-of-the-network launch */
 
@@ -164,7 +165,9 @@ int nnp_get_work(nnp_handle *h, double *what_host, int32_t n);
  *                     by centre i; *n_pairs receives the total even when it exceeds `capacity` pairs
  *   nnp_debug_aev     f32[N][n_features]
  *   nnp_debug_atomic_energies  f64[M][N], model units (before mean/scale)
- *   nnp_debug_daev    f32[N][n_features] = dE_model_units/dAEV (mean over the ensemble)
+ *   nnp_debug_daev    f32[N][n_features] = dE_model_units/dAEV (mean over the ensemble).  Columns of AEV blocks that
+ *                     are zero for every atom of the system (a species that does not occur) never reach the forces;
+ *                     the tensor engine does not compute whole 128-column tiles of them (exported as 0).
  */
 int nnp_debug_pairs(nnp_handle *h, int32_t which, int64_t *n_pairs, int32_t *ij_host, int64_t capacity);
 int nnp_debug_aev(nnp_handle *h, float *aev_host);

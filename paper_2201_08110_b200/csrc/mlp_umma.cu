@@ -315,7 +315,13 @@ __global__ void __launch_bounds__(U_THREADS, 1) gemm_umma_kernel(const __grid_co
         const CUtensorMap* bm = &P.bmap[t.bmap];
         const int a_mn = t.a_mn, a_c0 = t.a_c0, a_c1 = t.a_c1, b_c0 = t.b_c0, b_c1 = t.b_c1, kb1 = t.kb1;
         const uint32_t tx = A_BOX_BYTES + (uint32_t)t.n_pad * 128u;
-        for (int kb = t.kb0; kb < kb1; ++kb) {
+        unsigned long long live = t.kmask;
+        for (int kbi = t.kb0; kbi < kb1; ++kbi) {
+          int kb = kbi;
+          if (live) {  // skip the contraction boxes that only hold structural zeros
+            kb = __ffsll((long long)live) - 1;
+            live &= live - 1;
+          }
           mbar_wait(&raw_empty[rs], rphase ^ 1);
           unsigned char* sa = raw + (size_t)rs * P.stage_bytes;
           unsigned char* sb = sa + A_BOX_BYTES;
@@ -512,8 +518,12 @@ int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, cons
   for (const UmmaProblem& p : probs) {
     if (p.n_atoms <= 0 || p.F <= 0 || p.K <= 0) continue;
     const int nt = tile_of_bmap[p.bmap];
-    const int nkb = (p.K + BOXF - 1) / BOXF;
-    for (int f0 = 0; f0 < p.F; f0 += 128)
+    const int nkb_all = (p.K + BOXF - 1) / BOXF;
+    unsigned long long kmask = nkb_all <= 64 ? p.kmask : 0ull;
+    if (nkb_all < 64) kmask &= (1ull << nkb_all) - 1ull;
+    const int nkb = kmask ? __builtin_popcountll(kmask) : nkb_all;
+    for (int f0 = 0; f0 < p.F; f0 += 128) {
+      if (p.fmask && f0 / 128 < 64 && !((p.fmask >> (f0 / 128)) & 1ull)) continue;
       for (int a0 = 0; a0 < p.n_atoms; a0 += nt) {
         UmmaItem t;
         memset(&t, 0, sizeof(t));
@@ -522,6 +532,7 @@ int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, cons
         else { t.a_c0 = p.a_c0 + f0; t.a_c1 = p.a_c1; }        // (feature col, contraction row)
         t.b_c0 = p.b_c0; t.b_c1 = p.b_c1 + a0;
         t.kb0 = 0; t.kb1 = nkb;
+        t.kmask = kmask;
         t.n_pad = nt;
         t.n_valid = std::min(nt, p.n_atoms - a0);
         t.f_valid = std::min(128, p.F - f0);
@@ -535,6 +546,7 @@ int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, cons
         items.push_back(t);
         cost.push_back((long long)nkb * (128 + 2 * nt));
       }
+    }
   }
   // heavy items first, dealt to the persistent CTAs in snake order (static => deterministic)
   const size_t n = items.size();

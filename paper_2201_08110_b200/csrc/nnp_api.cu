@@ -283,6 +283,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   cudaMemset(h->d_cnt_a, 0, sizeof(int) * std::max<size_t>(N, 1));
   cudaMemset(h->d_phi, 0, sizeof(float) * std::max<size_t>((size_t)N * h->capR * 3, 1));
   cudaMemset(h->d_eatom, 0, sizeof(double) * std::max<size_t>((size_t)N * M, 1));
+  cudaMemset(h->d_daev, 0, sizeof(float) * std::max<size_t>((size_t)h->n_parts * N * n_feat, 1));  // skipped tiles stay 0
 
   // activations act[l], l = 1..L-1, layout per element group: [atom][model][H_l]
   for (int l = 1; l < L; ++l) {
@@ -456,6 +457,33 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       }
     }
   }
+  // Structural zeros of the AEV: the radial block of species s and the angular blocks of pairs (s, t) are zero for
+  // every atom when s (or t) does not occur in the system.  Layer 1 can skip the 32-wide contraction boxes that hold
+  // only such columns (forward) and the 128-wide tiles of dE/dAEV that hold only such columns (backward: the AEV
+  // backward kernel never reads them).  The result is unchanged; only multiplications by zero are not issued.
+  unsigned long long l1_kmask = 0, l1_fmask = 0;
+  if (!(cfg->flags & NNP_FLAG_NO_ZERO_SKIP) && n_feat <= 64 * 32) {
+    std::vector<char> live(n_feat, 0);
+    std::vector<char> present(S, 0);
+    for (int e = 0; e < S; ++e) present[e] = h->grp_off[e + 1] > h->grp_off[e];
+    for (int sp = 0; sp < S; ++sp)
+      if (present[sp])
+        for (int k = 0; k < cfg->n_shf_r; ++k) live[sp * cfg->n_shf_r + k] = 1;
+    for (int sp = 0, pidx = 0; sp < S; ++sp)
+      for (int tp = sp; tp < S; ++tp, ++pidx)
+        if (present[sp] && present[tp])
+          for (int k = 0; k < n_sub; ++k) live[n_radial + pidx * n_sub + k] = 1;
+    bool any_dead = false;
+    for (int cidx = 0; cidx < n_feat; ++cidx) {
+      if (live[cidx]) {
+        l1_kmask |= 1ull << (cidx / 32);
+        l1_fmask |= 1ull << (cidx / 128);
+      } else {
+        any_dead = true;
+      }
+    }
+    if (!any_dead) l1_kmask = l1_fmask = 0;  // nothing to skip
+  }
   if (h->use_umma) {
     // tcgen05 engine: D[f][a] = sum_k W[f][k] X[a][k].  Layer 1 forward runs all models of an element as ONE
     // problem (their weight rows are contiguous and they share the AEV input): F = M*H1 is a multiple of 128.
@@ -487,6 +515,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
           p.alpha = alpha;
           p.inv_alpha = 1.0f / alpha;
           if (pass == 0 && l == 1) {
+            p.kmask = l1_kmask;
             p.F = M * nout; p.K = nin;
             p.a_c0 = 0; p.a_c1 = 0; p.b_c0 = 0; p.b_c1 = 0;
             p.C = h->d_act[1] + h->act_off[1][e];
@@ -520,6 +549,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
             const int n_prob = h->n_parts == 1 ? 1 : M;
             for (int m = 0; m < n_prob; ++m) {
               UmmaProblem q = p;
+              q.fmask = l1_fmask;
               q.F = nin;
               q.epi = EPI_SCALE;
               q.scale = 1.0f / (float)M;

@@ -126,7 +126,8 @@ struct UmmaItem {            // one tile of one GEMM, as the persistent CTAs con
   int amap, bmap, a_mn;      // tensor-map slots; a_mn = 1: weights read as an MN-major operand (backward)
   int a_c0, a_c1;            // weight box origin: K-major (k col, feature row) / MN-major (feature col, k row)
   int b_c0, b_c1;            // activation box origin (k col, atom row)
-  int kb0, kb1;              // 32-wide contraction boxes [kb0, kb1)
+  int kb0, kb1;              // contraction boxes (32 wide) [kb0, kb1) as the consumers count them
+  unsigned long long kmask;  // non-zero: the boxes actually loaded are the set bits (popcount = kb1 - kb0)
   int n_pad, n_valid, f_valid;  // MMA N (16/32/64/128), atoms and feature rows actually stored
   int epi, ldc, ldaux;
   float* C;                  // C[a * ldc + f]
@@ -135,6 +136,8 @@ struct UmmaItem {            // one tile of one GEMM, as the persistent CTAs con
   float scale, alpha, inv_alpha;
 };
 struct UmmaProblem {
+  unsigned long long kmask;    // non-zero: contraction boxes (32 wide) to run; the others multiply structural zeros
+  unsigned long long fmask;    // non-zero: 128-feature output tiles to run; the others are never read downstream
   int amap, bmap;
   int a_c0, a_c1, b_c0, b_c1;  // origins of feature 0 / atom 0 / contraction element 0
   int F, n_atoms, K;
