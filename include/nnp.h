@@ -85,6 +85,7 @@ typedef struct {
 #define NNP_FLAG_NO_FWD1 256     /* ligand-size engine: row-pair layer-1 forward kernel instead of the persistent ring-fed one */
 #define NNP_FLAG_NO_NBR_FUSION 1024 /* small molecules: separate neighbour launch instead of building the rows inside the AEV forward kernel */
 #define NNP_FLAG_NO_ZERO_SKIP 2048 /* tensor engine: run layer 1 densely even over AEV columns that are structurally zero */
+#define NNP_FLAG_BWD1_PERSISTENT 4096 /* ligand-size engine: persistent ring-fed layer-1 backward kernel (2-D tensor copies) instead of one CTA per item; faster alone, 1.6 us slower inside the PDL chain at 50 atoms */
 #define NNP_FLAG_NO_PDL 32  /* plain stream-ordered launches instead of programmatic dependent launches along the chain */
 #define NNP_FLAG_NO_MID 16  /* ligand-size engine: one launch per layer instead of the fused middle-of-the-network launch */
 

@@ -714,6 +714,14 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     for (int l = l_bwd_begin; l >= 1; --l) {  // backward
       std::vector<SmallBwdItem> items;
       const bool bwd1 = l == 1 && (h->use_mid || L - 1 > 1);  // plain delta_1 -> dE/dAEV (no fused last layer)
+      std::vector<TmaOperand> wops;  // layer-1 weight block per present element (tensor maps of the persistent kernel)
+      std::vector<int> wslot(S, -1);
+      if (bwd1)
+        for (int e = 0; e < S; ++e)
+          if (h->grp_off[e + 1] > h->grp_off[e]) {
+            wslot[e] = (int)wops.size();
+            wops.push_back(TmaOperand{h->d_W + h->w_off[e * L + 0], (long long)M * h->dims[e * (L + 1) + 1], n_feat, n_feat});
+          }
       for (int e = 0; e < S; ++e) {
         const int ne = h->grp_off[e + 1] - h->grp_off[e];
         if (ne == 0) continue;
@@ -731,6 +739,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
               it.D = h->d_act[l] + h->act_off[l][e] + (size_t)a0 * M * nout + (size_t)m * nout;
               it.ldd = M * nout;
               it.n_atoms = na; it.n_out = nout; it.n_cols = std::min(128, nin - n0);
+              it.tmap = wslot[e]; it.t_row0 = m * nout; it.t_col0 = n0;
               small_bwd_shape(na, &it.AW, &it.G);
               it.inv_alpha = inv_alpha;
               if (l > 1) {
@@ -758,7 +767,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       }
       SmallLaunch sl;
       sl.name = "mlp_bwd_l" + std::to_string(l);
-      if (bwd1 ? small_build_bwd1(sl, items) : small_build_bwd(sl, items)) { small_free_launch(sl); return fail(NNP_ERR_CUDA); }
+      if (bwd1 ? small_build_bwd1(sl, items, (cfg->flags & NNP_FLAG_BWD1_PERSISTENT) != 0, wops) : small_build_bwd(sl, items)) { small_free_launch(sl); return fail(NNP_ERR_CUDA); }
       h->sbwd.push_back(sl);
     }
   }

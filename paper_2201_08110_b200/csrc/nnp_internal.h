@@ -180,6 +180,7 @@ struct SmallBwdItem {       // out[a*ldo + n] = epi(sum_o D[a*ldd + o] W[o*ldw +
   int ldw, ldd, ldo, ldaux, lde;
   int n_atoms, n_out, n_cols;  // n_atoms <= 32, n_out % 4 == 0, n_cols % 4 == 0
   int epi, AW, G;           // atoms per warp (1..4), atom groups (1,2,4,8): G*AW >= n_atoms
+  int tmap, t_row0, t_col0; // persistent layer-1 kernel: tensor map of the element's layer-1 block, row / column origin
   float scale, inv_alpha, b_last;
 };
 struct Fwd1Item {            // persistent layer-1 forward item: one CTA, a run of weight rows of one element
@@ -193,6 +194,9 @@ struct Fwd1Item {            // persistent layer-1 forward item: one CTA, a run 
 struct SmallLaunch {
   void* d_items = nullptr;
   int n_items = 0, variant = 1;
+  int grid = 0, stages = 0;  // persistent kernels: CTAs and ring depth
+  void* params = nullptr;    // persistent layer-1 backward: host copy of its __grid_constant__ parameter block
+  void* d_aux = nullptr;     // persistent layer-1 backward: per-CTA item ranges (device)
   size_t smem_bytes = 0;
   std::string name;
 };
@@ -200,7 +204,8 @@ int small_init();
 void small_bwd_shape(int n_atoms, int* AW, int* G);
 int small_build_fwd(SmallLaunch& L, std::vector<SmallFwdItem>& items);
 int small_build_bwd(SmallLaunch& L, std::vector<SmallBwdItem>& items);
-int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items);
+int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool persistent_ok,
+                     const std::vector<TmaOperand>& wops);  // wops[tmap]: the [rows][cols] layer-1 weight block of an element
 int small_build_fwd1(SmallLaunch& L, std::vector<Fwd1Item>& items);
 int small_fwd1_tile_rows();  // layer 1: persistent, weights streamed through a ring  // layer 1: weights read once, FFMA2
 void small_launch_fwd(const SmallLaunch& L, cudaStream_t s, bool pdl);
