@@ -347,19 +347,42 @@ __device__ __forceinline__ float2 unpack2(unsigned long long v) {
   return r;
 }
 
+struct Bwd1pParams {
+  CUtensorMap wmap[NNP_MAX_SPECIES];  // layer-1 weight block of an element: [M * H1 rows][n_feat columns], box 32 x 128
+  const SmallBwdItem* items;  // grouped by CTA: CTA b owns items [cta_off[b], cta_off[b + 1])
+  const int* cta_off;
+  int n_items, n_stages;
+  int use_tma;  // one-CTA-per-item kernel: weight chunk by 2-D tensor copies (else one bulk copy per row)
+};
+
+__device__ __forceinline__ void p1_tma_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+      ::"r"(s_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(s_u32(bar))
+      : "memory");
+}
+
 template <int NA>
-__device__ __forceinline__ void small_bwd1_body(const SmallBwdItem& it, float* smem_f, uint64_t* bars) {
+__device__ __forceinline__ void small_bwd1_body(const SmallBwdItem& it, float* smem_raw, uint64_t* bars,
+                                                const CUtensorMap* wmap) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int rps = (((it.n_out + B1_SLICES - 1) / B1_SLICES) + 3) & ~3;  // rows per slice, a multiple of 4
-  const size_t ws_floats = max((size_t)it.n_out * 128, (size_t)B1_SLICES * NA * 128);
+  const int n_tiles = (it.n_out + 31) >> 5;                              // 32-row tiles of the tensor copies
+  const bool tma = wmap != nullptr && n_tiles <= B1_SLICES;
+  float* smem_f = smem_raw + (((128u - (s_u32(smem_raw) & 127u)) & 127u) >> 2);  // 128-byte aligned (tensor copies)
+  const size_t ws_floats = max((size_t)n_tiles * 32 * 128, (size_t)B1_SLICES * NA * 128);
   float* ws = smem_f;               // [n_out][128]; later red [B1_SLICES][NA][128]
   float* ds = smem_f + ws_floats;   // [NA][n_out]
   uint64_t* dbar = bars + B1_SLICES;
   if (threadIdx.x == 0) {
     for (int g = 0; g < B1_SLICES; ++g) {
-      const int rows = max(0, min(it.n_out, (g + 1) * rps) - g * rps);
       sbar_init(&bars[g], 1);
-      if (rows) sbar_expect_tx(&bars[g], (uint32_t)(rows * it.n_cols * 4));
+      if (tma) {
+        if (g < n_tiles) sbar_expect_tx(&bars[g], 32u * 128u * 4u);  // whole box: columns beyond the matrix arrive as zeros
+      } else {
+        const int rows = max(0, min(it.n_out, (g + 1) * rps) - g * rps);
+        if (rows) sbar_expect_tx(&bars[g], (uint32_t)(rows * it.n_cols * 4));
+      }
     }
     sbar_init(dbar, 1);
     sbar_expect_tx(dbar, (uint32_t)(it.n_atoms * it.n_out * 4));
@@ -367,8 +390,13 @@ __device__ __forceinline__ void small_bwd1_body(const SmallBwdItem& it, float* s
   }
   __syncthreads();
   pdl_trigger();
-  for (int o = threadIdx.x; o < it.n_out; o += SM_THREADS)
-    bulk_g2s(ws + (size_t)o * 128, it.W + (size_t)o * it.ldw, (uint32_t)(it.n_cols * 4), &bars[o / rps]);
+  if (tma) {  // one 2-D tensor copy per 32-row tile (512-byte row segments as separate bulk copies are issue-bound)
+    if ((int)threadIdx.x < n_tiles)
+      p1_tma_2d(ws + (size_t)threadIdx.x * 32 * 128, wmap, it.t_col0, it.t_row0 + 32 * (int)threadIdx.x, &bars[threadIdx.x]);
+  } else {
+    for (int o = threadIdx.x; o < it.n_out; o += SM_THREADS)
+      bulk_g2s(ws + (size_t)o * 128, it.W + (size_t)o * it.ldw, (uint32_t)(it.n_cols * 4), &bars[o / rps]);
+  }
   for (int idx = it.n_atoms * it.n_out + threadIdx.x; idx < NA * it.n_out; idx += SM_THREADS) ds[idx] = 0.0f;
   pdl_wait();  // delta comes from the previous kernel
   if (threadIdx.x < it.n_atoms)
@@ -382,7 +410,13 @@ __device__ __forceinline__ void small_bwd1_body(const SmallBwdItem& it, float* s
   for (int a = 0; a < NA; ++a) acc[a][0] = acc[a][1] = 0ull;
   const bool col_ok = 4 * lane < it.n_cols;
   const int o0 = warp * rps, o1 = min(it.n_out, o0 + rps);
-  if (o0 < o1) sbar_wait(&bars[warp], 0);
+  if (o0 < o1) {
+    if (tma) {
+      for (int t = o0 >> 5; t <= (o1 - 1) >> 5; ++t) sbar_wait(&bars[t], 0);
+    } else {
+      sbar_wait(&bars[warp], 0);
+    }
+  }
   if (col_ok) {
     const float4* wp = reinterpret_cast<const float4*>(ws) + lane;
     for (int o = o0; o < o1; o += 4) {
@@ -428,14 +462,15 @@ __device__ __forceinline__ void small_bwd1_body(const SmallBwdItem& it, float* s
   }
 }
 
-__global__ void __launch_bounds__(SM_THREADS, 1) small_bwd1_kernel(const SmallBwdItem* __restrict__ items) {
+__global__ void __launch_bounds__(SM_THREADS, 1) small_bwd1_kernel(const __grid_constant__ Bwd1pParams P) {
   extern __shared__ __align__(16) float smem_f[];
   __shared__ __align__(8) uint64_t bars[B1_SLICES + 1];
-  const SmallBwdItem it = items[blockIdx.x];
-  if (it.n_atoms <= 4) small_bwd1_body<4>(it, smem_f, bars);
-  else if (it.n_atoms <= 8) small_bwd1_body<8>(it, smem_f, bars);
-  else if (it.n_atoms <= 16) small_bwd1_body<16>(it, smem_f, bars);
-  else small_bwd1_body<24>(it, smem_f, bars);
+  const SmallBwdItem it = P.items[blockIdx.x];
+  const CUtensorMap* wmap = P.use_tma ? &P.wmap[it.tmap] : nullptr;
+  if (it.n_atoms <= 4) small_bwd1_body<4>(it, smem_f, bars, wmap);
+  else if (it.n_atoms <= 8) small_bwd1_body<8>(it, smem_f, bars, wmap);
+  else if (it.n_atoms <= 16) small_bwd1_body<16>(it, smem_f, bars, wmap);
+  else small_bwd1_body<24>(it, smem_f, bars, wmap);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -525,20 +560,6 @@ __device__ __forceinline__ void p1_item(const SmallBwdItem& it, const float* __r
     *reinterpret_cast<float4*>(it.out + (size_t)a * it.ldo + 4 * l) = v;
   }
   p1_consumer_sync();  // red and this item's delta buffer are free again
-}
-
-struct Bwd1pParams {
-  CUtensorMap wmap[NNP_MAX_SPECIES];  // layer-1 weight block of an element: [M * H1 rows][n_feat columns], box 32 x 128
-  const SmallBwdItem* items;  // grouped by CTA: CTA b owns items [cta_off[b], cta_off[b + 1])
-  const int* cta_off;
-  int n_items, n_stages;
-};
-
-__device__ __forceinline__ void p1_tma_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
-  asm volatile(
-      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-      ::"r"(s_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(s_u32(bar))
-      : "memory");
 }
 
 __global__ void __launch_bounds__(P1_THREADS, 1) small_bwd1p_kernel(const __grid_constant__ Bwd1pParams P) {
@@ -882,19 +903,22 @@ int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool pers
   L.n_items = (int)items.size();
   L.variant = 100;
   L.smem_bytes = 0;
+  bool maps_ok = !wops.empty() && wops.size() <= NNP_MAX_SPECIES;
+  bool fits_persistent = true;
   for (const auto& it : items) {
     if (it.n_atoms < 1 || it.n_atoms > 24 || it.n_cols > 128 || it.epi != EPI_SCALE) return -1;
     const int NA = bwd1_pad(it.n_atoms);
-    const size_t b = (std::max((size_t)it.n_out * 128, (size_t)B1_SLICES * NA * 128) + (size_t)it.n_out * NA) * 4;
+    const size_t rows32 = (size_t)((it.n_out + 31) / 32) * 32;  // the tensor copies write whole 32-row tiles
+    const size_t b = (std::max(rows32 * 128, (size_t)B1_SLICES * NA * 128) + (size_t)it.n_out * NA) * 4 + 128;
     L.smem_bytes = std::max(L.smem_bytes, b);
+    maps_ok = maps_ok && it.tmap >= 0 && it.tmap < (int)wops.size();
+    fits_persistent = fits_persistent && it.n_out <= P1_NOUT_MAX && it.n_out % 4 == 0;
   }
-  // persistent ring-fed kernel when the shapes fit its fixed buffers and the tensor maps can be made
-  bool persistent = persistent_ok && !wops.empty() && wops.size() <= NNP_MAX_SPECIES;
-  for (const auto& it : items)
-    persistent = persistent && it.n_out <= P1_NOUT_MAX && it.n_out % 4 == 0 && it.tmap >= 0 && it.tmap < (int)wops.size();
-  Bwd1pParams* P = nullptr;
-  std::vector<int> p1_off;
-  if (persistent) {
+  // tensor maps of the elements' layer-1 weight blocks: [rows][cols] f32, box 32 rows x 128 columns, no swizzle
+  Bwd1pParams* P = new Bwd1pParams();
+  memset(P, 0, sizeof(*P));
+  L.params = P;
+  if (maps_ok) {
     typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -902,24 +926,21 @@ int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool pers
     cudaDriverEntryPointQueryResult qr;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fp, cudaEnableDefault, &qr) != cudaSuccess ||
         qr != cudaDriverEntryPointSuccess || !fp)
-      persistent = false;
-    if (persistent) {
-      P = new Bwd1pParams();
-      memset(P, 0, sizeof(*P));
-      for (size_t k = 0; k < wops.size() && persistent; ++k) {
-        cuuint64_t gdim[2] = {(cuuint64_t)wops[k].cols, (cuuint64_t)std::max<long long>(wops[k].rows, 1)};
-        cuuint64_t gstr[1] = {(cuuint64_t)wops[k].ld * 4};
-        cuuint32_t box[2] = {128, (cuuint32_t)P1_TILE_ROWS};
-        cuuint32_t estr[2] = {1, 1};
-        if (((EncodeFn)fp)(&P->wmap[k], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)wops[k].base, gdim, gstr, box, estr,
-                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-          persistent = false;
-      }
-      if (!persistent) { delete P; P = nullptr; }
+      maps_ok = false;
+    for (size_t k = 0; k < wops.size() && maps_ok; ++k) {
+      cuuint64_t gdim[2] = {(cuuint64_t)wops[k].cols, (cuuint64_t)std::max<long long>(wops[k].rows, 1)};
+      cuuint64_t gstr[1] = {(cuuint64_t)wops[k].ld * 4};
+      cuuint32_t box[2] = {128, (cuuint32_t)P1_TILE_ROWS};
+      cuuint32_t estr[2] = {1, 1};
+      if (((EncodeFn)fp)(&P->wmap[k], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)wops[k].base, gdim, gstr, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        maps_ok = false;
     }
   }
-  if (persistent) {
+  P->use_tma = maps_ok ? 1 : 0;
+  std::vector<int> p1_off(1, 0);
+  if (persistent_ok && maps_ok && fits_persistent) {
     int dev = 0, sms = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -946,23 +967,19 @@ int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool pers
     }
     L.stages = (int)std::min<size_t>(P1_MAX_STAGES, (P1_SMEM - P1_FIXED) / ((size_t)P1_TILE_ROWS * 128 * 4));
     L.smem_bytes = P1_FIXED + (size_t)L.stages * P1_TILE_ROWS * 128 * 4 + 128;
-    L.params = P;
   }
   if (L.smem_bytes > (L.variant == 102 ? P1_SMEM : SMALL_SMEM_MAX)) return -1;
   if (cudaMalloc(&L.d_items, std::max<size_t>(1, items.size()) * sizeof(SmallBwdItem)) != cudaSuccess) return -1;
   if (!items.empty())
     cudaMemcpy(L.d_items, items.data(), items.size() * sizeof(SmallBwdItem), cudaMemcpyHostToDevice);
-  if (L.params) {
-    Bwd1pParams* PP = reinterpret_cast<Bwd1pParams*>(L.params);
-    PP->items = reinterpret_cast<const SmallBwdItem*>(L.d_items);
-    int* d_off = nullptr;
-    if (cudaMalloc((void**)&d_off, p1_off.size() * sizeof(int)) != cudaSuccess) return -1;
-    cudaMemcpy(d_off, p1_off.data(), p1_off.size() * sizeof(int), cudaMemcpyHostToDevice);
-    L.d_aux = d_off;
-    PP->cta_off = d_off;
-    PP->n_items = L.n_items;
-    PP->n_stages = L.stages;
-  }
+  int* d_off = nullptr;
+  if (cudaMalloc((void**)&d_off, p1_off.size() * sizeof(int)) != cudaSuccess) return -1;
+  cudaMemcpy(d_off, p1_off.data(), p1_off.size() * sizeof(int), cudaMemcpyHostToDevice);
+  L.d_aux = d_off;
+  P->items = reinterpret_cast<const SmallBwdItem*>(L.d_items);
+  P->cta_off = d_off;
+  P->n_items = L.n_items;
+  P->n_stages = L.stages;
   return 0;
 }
 
@@ -1008,7 +1025,7 @@ void small_launch_bwd(const SmallLaunch& L, cudaStream_t s, bool pdl) {
   }
   if (L.variant == 100) {
     launch_kernel(pdl, small_bwd1_kernel, dim3(L.n_items), dim3(SM_THREADS), L.smem_bytes, s,
-                  reinterpret_cast<const SmallBwdItem*>(L.d_items));
+                  *reinterpret_cast<const Bwd1pParams*>(L.params));
     return;
   }
   launch_kernel(pdl, small_bwd_kernel, dim3(L.n_items), dim3(SM_THREADS), L.smem_bytes, s,
