@@ -25,6 +25,7 @@ struct NbrArgs {
   const int* species;
   const int* mol_id;
   const int* mol_off;
+  const int2* mol_range;  // [N] (first atom, end) of the atom's molecule: one load instead of mol_id -> mol_off
   int* status;
   int pos_stride;
   float length_scale;
@@ -74,6 +75,48 @@ __device__ __forceinline__ void nbr_row_warp(const NbrArgs& a, int i, int lane, 
   }
   if (lane == 0) {
     if (nr > capR || na > capA) atomicOr(a.status, NNP_ST_CAPACITY);
+    cnt_r[i] = min(nr, capR);
+    cnt_a[i] = min(na, capA);
+  }
+}
+
+// the same search for one centre with the molecule's positions already in shared memory (fused AEV forward path)
+__device__ __forceinline__ void nbr_row_warp_smem(const float4* __restrict__ mp, int lo, int hi, int i, int lane,
+                                                  double rc_r2, double rc_a2, int capR, int capA, int* status,
+                                                  float4* __restrict__ pos4, int* __restrict__ nbr_r,
+                                                  int* __restrict__ nbr_a, int* __restrict__ cnt_r, int* __restrict__ cnt_a) {
+  const float4 pi = mp[i - lo];
+  if (lane == 0) {
+    pos4[i] = pi;
+    if (!(isfinite(pi.x) && isfinite(pi.y) && isfinite(pi.z))) atomicOr(status, NNP_ST_NONFINITE);
+  }
+  int nr = 0, na = 0;
+  for (int base = lo; base < hi; base += 32) {
+    const int j = base + lane;
+    bool in_r = false, in_a = false;
+    if (j < hi && j != i) {
+      const float4 pj = mp[j - lo];
+      const double dx = (double)pj.x - (double)pi.x;
+      const double dy = (double)pj.y - (double)pi.y;
+      const double dz = (double)pj.z - (double)pi.z;
+      const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+      in_r = d2 <= rc_r2;
+      in_a = d2 <= rc_a2;
+    }
+    const unsigned br = __ballot_sync(FULL, in_r);
+    const unsigned ba = __ballot_sync(FULL, in_a);
+    const unsigned below = (1u << lane) - 1u;
+    const int slot_r = nr + __popc(br & below);
+    if (in_r && slot_r < capR) nbr_r[(size_t)i * capR + slot_r] = j;
+    if (in_a) {
+      const int slot_a = na + __popc(ba & below);
+      if (slot_a < capA && slot_r < capR) nbr_a[(size_t)i * capA + slot_a] = slot_r;
+    }
+    nr += __popc(br);
+    na += __popc(ba);
+  }
+  if (lane == 0) {
+    if (nr > capR || na > capA) atomicOr(status, NNP_ST_CAPACITY);
     cnt_r[i] = min(nr, capR);
     cnt_a[i] = min(na, capA);
   }
@@ -215,10 +258,10 @@ __device__ __forceinline__ CentreTab carve_tab(float* smem, int capR, int capA, 
 __device__ __forceinline__ void build_tab(const CentreTab& t, int i, int nr, int na, const float4 pi,
                                           const float4* __restrict__ pos4, const int* __restrict__ nbr_r,
                                           const int* __restrict__ nbr_a, int capR, int capA, const AevConst& c,
-                                          bool want_pres, const NbrArgs* raw = nullptr) {
+                                          bool want_pres, const float4* mol_pos = nullptr, int mol_lo = 0) {
   for (int q = threadIdx.x; q < nr; q += blockDim.x) {
     const int j = nbr_r[(size_t)i * capR + q];
-    const float4 pj = raw ? raw_pos4(*raw, j) : pos4[j];  // fused neighbour search: pos4[j] is another CTA's job
+    const float4 pj = mol_pos ? mol_pos[j - mol_lo] : pos4[j];  // fused neighbour search: pos4[j] is another CTA's job
     const double dx = (double)pj.x - (double)pi.x;
     const double dy = (double)pj.y - (double)pi.y;
     const double dz = (double)pj.z - (double)pi.z;
@@ -326,7 +369,7 @@ __global__ void __launch_bounds__(AEV_THREADS, 6) aev_forward_kernel(
     const float4* __restrict__ pos4, const int* __restrict__ nbr_r, const int* __restrict__ nbr_a,
     const int* __restrict__ cnt_r, const int* __restrict__ cnt_a, const int* __restrict__ sortpos, int N,
     const __grid_constant__ AevConst c, int capR, int capA, int CH, float* __restrict__ aev,
-    const __grid_constant__ NbrArgs nb, int fused, float4* __restrict__ pos4_w, int* __restrict__ nbr_r_w,
+    const __grid_constant__ NbrArgs nb, int fused, int mp_off4, float4* __restrict__ pos4_w, int* __restrict__ nbr_r_w,
     int* __restrict__ nbr_a_w, int* __restrict__ cnt_r_w, int* __restrict__ cnt_a_w) {
   extern __shared__ __align__(16) float smem[];
   const int i = blockIdx.x;
@@ -337,18 +380,26 @@ __global__ void __launch_bounds__(AEV_THREADS, 6) aev_forward_kernel(
   float* bF2 = bF1 + c.n_shf_z * CH;   // [n_shf_a][CH]
   pdl_trigger();
   pdl_wait();
+  float4* mp = reinterpret_cast<float4*>(smem) + mp_off4;  // [max molecule size]: the molecule's positions (fused path)
+  int mlo = 0;
   if (fused) {
-    // small molecules: the centre's CTA builds its own neighbour rows (first warp) instead of a separate launch;
-    // the rows also go to global memory for the backward and gather kernels
+    // small systems: the centre's CTA builds its own neighbour rows instead of a separate launch.  All threads load
+    // the molecule's positions into shared memory (one memory round trip), the first warp runs the pair search on
+    // them; the rows also go to global memory for the backward and gather kernels.
+    const int2 rg = nb.mol_range[i];
+    mlo = rg.x;
+    for (int j = rg.x + (int)threadIdx.x; j < rg.y; j += blockDim.x) mp[j - rg.x] = raw_pos4(nb, j);
+    __syncthreads();
     if (threadIdx.x < 32)
-      nbr_row_warp(nb, i, threadIdx.x, c.rc_r2, c.rc_a2, capR, capA, pos4_w, nbr_r_w, nbr_a_w, cnt_r_w, cnt_a_w);
+      nbr_row_warp_smem(mp, rg.x, rg.y, i, threadIdx.x, c.rc_r2, c.rc_a2, capR, capA, nb.status, pos4_w, nbr_r_w, nbr_a_w,
+                        cnt_r_w, cnt_a_w);
     __syncthreads();  // the CTA's own global writes are visible to the CTA
   }
-  const float4 pi = fused ? raw_pos4(nb, i) : pos4[i];
+  const float4 pi = fused ? mp[i - mlo] : pos4[i];
   const int nr = fused ? cnt_r_w[i] : cnt_r[i], na = fused ? cnt_a_w[i] : cnt_a[i];
   for (int f = threadIdx.x; f < n_ang; f += blockDim.x) row[f] = 0.0f;
   build_tab(t, i, nr, na, pi, pos4, fused ? nbr_r_w : nbr_r, fused ? nbr_a_w : nbr_a, capR, capA, c, true,
-            fused ? &nb : nullptr);
+            fused ? mp : nullptr, mlo);
   float* out = aev + (size_t)sortpos[i] * c.n_feat;
 
   // ---- radial (O3)
@@ -434,8 +485,10 @@ __device__ __forceinline__ float warp_sum(float v) {
   return v;
 }
 
-template <int NZ, int NA>
-__global__ void __launch_bounds__(AEV_THREADS, 6) aev_backward_kernel(
+// MULTI: dE/dAEV arrives as several partial rows (ligand sizes, one per model); a separate instantiation so that its
+// wider load batch does not cost the large-system instantiation registers (occupancy)
+template <int NZ, int NA, bool MULTI>
+__global__ void __launch_bounds__(AEV_THREADS, MULTI ? 4 : 6) aev_backward_kernel(
     const float4* __restrict__ pos4, const int* __restrict__ nbr_r, const int* __restrict__ nbr_a,
     const int* __restrict__ cnt_r, const int* __restrict__ cnt_a, const int* __restrict__ sortpos, int N,
     const __grid_constant__ AevConst c, int capR, int capA, int CH, const float* __restrict__ daev, int n_parts,
@@ -455,7 +508,7 @@ __global__ void __launch_bounds__(AEV_THREADS, 6) aev_backward_kernel(
   const float4 pi = pos4[i];
   const int nr = cnt_r[i], na = cnt_a[i];
   const float* gin = daev + (size_t)sortpos[i] * c.n_feat;
-  // dE/dAEV row = fixed-order sum of the partial rows.  All loads of a pass (2 columns x 8 partial rows per thread)
+  // dE/dAEV row = fixed-order sum of the partial rows.  All loads of a pass (KC columns x 8 partial rows per thread)
   // are issued before the first add: one memory latency per pass instead of one per partial row
   if (n_parts == 1) {  // large systems: one row, keep as many columns in flight as possible
     for (int fb = 0; fb < c.n_feat; fb += 8 * AEV_THREADS) {
@@ -476,24 +529,27 @@ __global__ void __launch_bounds__(AEV_THREADS, 6) aev_backward_kernel(
       }
     }
   }
-  for (int fb = 0; n_parts > 1 && fb < c.n_feat; fb += 2 * AEV_THREADS) {
-    float acc[2] = {0.0f, 0.0f};
-    for (int p0 = 0; p0 < n_parts; p0 += 8) {
-      float x[2][8];
+  constexpr int KC = MULTI ? 4 : 2;  // columns per thread and pass: KC x 8 loads in flight before the first add
+  for (int fb = 0; n_parts > 1 && fb < c.n_feat; fb += KC * AEV_THREADS) {
+    float acc[KC];
 #pragma unroll
-      for (int k = 0; k < 2; ++k) {
+    for (int k = 0; k < KC; ++k) acc[k] = 0.0f;
+    for (int p0 = 0; p0 < n_parts; p0 += 8) {
+      float x[KC][8];
+#pragma unroll
+      for (int k = 0; k < KC; ++k) {
         const int f = fb + k * AEV_THREADS + threadIdx.x;
 #pragma unroll
         for (int u = 0; u < 8; ++u)
           x[k][u] = (f < c.n_feat && p0 + u < n_parts) ? gin[(size_t)(p0 + u) * part_stride + f] : 0.0f;
       }
 #pragma unroll
-      for (int k = 0; k < 2; ++k)
+      for (int k = 0; k < KC; ++k)
 #pragma unroll
         for (int u = 0; u < 8; ++u) acc[k] += x[k][u];
     }
 #pragma unroll
-    for (int k = 0; k < 2; ++k) {
+    for (int k = 0; k < KC; ++k) {
       const int f = fb + k * AEV_THREADS + threadIdx.x;
       if (f < c.n_radial) g[f] = acc[k];
       else if (f < c.n_feat) {
@@ -704,6 +760,7 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(
 static NbrArgs nbr_args(nnp_handle* h, const float* d_pos, int pos_stride, const int* d_atom_index) {
   NbrArgs a;
   a.pos = d_pos; a.atom_index = d_atom_index; a.species = h->d_species; a.mol_id = h->d_mol_id; a.mol_off = h->d_mol_off;
+  a.mol_range = reinterpret_cast<const int2*>(h->d_mol_range);
   a.status = h->d_status; a.pos_stride = pos_stride; a.length_scale = h->aev.length_scale;
   return a;
 }
@@ -725,7 +782,9 @@ static bool aev_small_shape(const nnp_handle* h) { return h->aev.n_shf_z <= 4 &&
 void launch_aev_forward(nnp_handle* h, const float* d_pos, int pos_stride, const int* d_atom_index, cudaStream_t s) {
   if (h->N == 0) return;
   const int blocks = h->N;
-  const size_t smem = aev_smem_bytes(h, false);
+  const size_t smem0 = aev_smem_bytes(h, false);
+  const size_t smem = smem0 + (h->fuse_nbr ? 256 * sizeof(float4) : 0);  // + the molecule's positions (<= 256 atoms)
+  const int mp_off4 = (int)(smem0 / sizeof(float4));
   const NbrArgs nb = nbr_args(h, d_pos, pos_stride, d_atom_index);
   const int fused = h->fuse_nbr ? 1 : 0;
   const bool pdl = h->pdl_now && !fused;  // fused: first kernel of the step, must not overtake the previous step
@@ -733,26 +792,33 @@ void launch_aev_forward(nnp_handle* h, const float* d_pos, int pos_stride, const
     launch_kernel(pdl, aev_forward_kernel<4, 8>, dim3(blocks), dim3(AEV_THREADS), smem, s, (const float4*)h->d_pos4,
                   (const int*)h->d_nbr_r, (const int*)h->d_nbr_a, (const int*)h->d_cnt_r, (const int*)h->d_cnt_a,
                   (const int*)h->d_sortpos, h->N, h->aev, h->capR, h->capA, trip_chunk(h, false), h->d_aev, nb, fused,
-                  h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a);
+                  mp_off4, h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a);
   else
     launch_kernel(pdl, aev_forward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>, dim3(blocks), dim3(AEV_THREADS), smem, s,
                   (const float4*)h->d_pos4, (const int*)h->d_nbr_r, (const int*)h->d_nbr_a, (const int*)h->d_cnt_r,
                   (const int*)h->d_cnt_a, (const int*)h->d_sortpos, h->N, h->aev, h->capR, h->capA,
-                  trip_chunk(h, false), h->d_aev, nb, fused, h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a);
+                  trip_chunk(h, false), h->d_aev, nb, fused, mp_off4, h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r,
+                  h->d_cnt_a);
+}
+
+template <int NZ, int NA, bool MULTI>
+static void launch_aev_backward_t(nnp_handle* h, cudaStream_t s) {
+  launch_kernel(h->pdl_now, aev_backward_kernel<NZ, NA, MULTI>, dim3(h->N), dim3(AEV_THREADS), aev_smem_bytes(h, true), s,
+                (const float4*)h->d_pos4, (const int*)h->d_nbr_r, (const int*)h->d_nbr_a, (const int*)h->d_cnt_r,
+                (const int*)h->d_cnt_a, (const int*)h->d_sortpos, h->N, h->aev, h->capR, h->capA, trip_chunk(h, true),
+                (const float*)h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
 }
 
 void launch_aev_backward(nnp_handle* h, cudaStream_t s) {
   if (h->N == 0) return;
-  const int blocks = h->N;
-  const size_t smem = aev_smem_bytes(h, true);
-  if (aev_small_shape(h))
-    launch_kernel(h->pdl_now, aev_backward_kernel<4, 8>, dim3(blocks), dim3(AEV_THREADS), smem, s, h->d_pos4,
-                  h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR, h->capA,
-                  trip_chunk(h, true), (const float*)h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
-  else
-    launch_kernel(h->pdl_now, aev_backward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>, dim3(blocks), dim3(AEV_THREADS), smem, s,
-                  h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_sortpos, h->N, h->aev, h->capR,
-                  h->capA, trip_chunk(h, true), (const float*)h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
+  const bool multi = h->n_parts > 1;
+  if (aev_small_shape(h)) {
+    if (multi) launch_aev_backward_t<4, 8, true>(h, s);
+    else launch_aev_backward_t<4, 8, false>(h, s);
+  } else {
+    if (multi) launch_aev_backward_t<NNP_MAX_SHF_Z, NNP_MAX_SHF_A, true>(h, s);
+    else launch_aev_backward_t<NNP_MAX_SHF_Z, NNP_MAX_SHF_A, false>(h, s);
+  }
 }
 
 void launch_finish(nnp_handle* h, const int* d_atom_index, double* d_energy, float* d_force, int force_stride,
@@ -767,13 +833,16 @@ void launch_finish(nnp_handle* h, const int* d_atom_index, double* d_energy, flo
 }
 
 int aev_set_smem_attributes(nnp_handle* h) {
-  const int fb = (int)aev_smem_bytes(h, false), bb = (int)aev_smem_bytes(h, true);
-  cudaError_t e[4];
+  const int fb = (int)(aev_smem_bytes(h, false) + 256 * sizeof(float4)), bb = (int)aev_smem_bytes(h, true);
+  cudaError_t e[6];
   e[0] = cudaFuncSetAttribute(aev_forward_kernel<4, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, fb);
   e[1] = cudaFuncSetAttribute(aev_forward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>,
                               cudaFuncAttributeMaxDynamicSharedMemorySize, fb);
-  e[2] = cudaFuncSetAttribute(aev_backward_kernel<4, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, bb);
-  e[3] = cudaFuncSetAttribute(aev_backward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>,
+  e[2] = cudaFuncSetAttribute(aev_backward_kernel<4, 8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bb);
+  e[3] = cudaFuncSetAttribute(aev_backward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A, false>,
+                              cudaFuncAttributeMaxDynamicSharedMemorySize, bb);
+  e[4] = cudaFuncSetAttribute(aev_backward_kernel<4, 8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bb);
+  e[5] = cudaFuncSetAttribute(aev_backward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A, true>,
                               cudaFuncAttributeMaxDynamicSharedMemorySize, bb);
   for (cudaError_t x : e)
     if (x != cudaSuccess) return -1;

@@ -65,7 +65,7 @@ extern "C" void nnp_destroy(nnp_handle* h) {
   cudaDeviceSynchronize();
   if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
   for (auto e : h->events) cudaEventDestroy(e);
-  void* ptrs[] = {h->d_species, h->d_mol_off, h->d_mol_id, h->d_sortpos, h->d_perm, h->d_grp_off, h->d_self_energy,
+  void* ptrs[] = {h->d_mol_range, h->d_species, h->d_mol_off, h->d_mol_id, h->d_sortpos, h->d_perm, h->d_grp_off, h->d_self_energy,
                   h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_aev, h->d_daev, h->d_phi,
                   h->d_eatom, h->d_status, h->d_W, h->d_b, h->d_last_act_off, h->d_last_w_off, h->d_last_b_off,
                   h->d_last_H, h->d_hpos, h->d_hforce, h->d_henergy};
@@ -203,6 +203,14 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   if (aev_smem_bytes(h, true) > (size_t)prop.sharedMemPerBlockOptin || aev_set_smem_attributes(h) != 0)
     return fail(NNP_ERR_INVALID_ARG);
 
+  {
+    std::vector<int> range(2 * (size_t)N);
+    for (int i = 0; i < N; ++i) {
+      range[2 * i] = mol_off[mol_id[i]];
+      range[2 * i + 1] = mol_off[mol_id[i] + 1];
+    }
+    if (upload(&h->d_mol_range, range)) return fail(NNP_ERR_ALLOC);
+  }
   if (upload(&h->d_species, species) || upload(&h->d_mol_off, mol_off) || upload(&h->d_mol_id, mol_id) ||
       upload(&h->d_sortpos, sortpos) || upload(&h->d_perm, perm) || upload(&h->d_grp_off, h->grp_off))
     return fail(NNP_ERR_ALLOC);

@@ -254,6 +254,7 @@ struct nnp_handle {
   std::vector<int> dims;     // [S][L+1]
   std::vector<int> grp_off;  // [S+1] host
   // device: topology
+  int* d_mol_range = nullptr;  // [N][2] (first atom, end) of every atom's molecule
   int *d_species = nullptr, *d_mol_off = nullptr, *d_mol_id = nullptr, *d_sortpos = nullptr, *d_perm = nullptr,
       *d_grp_off = nullptr;
   double* d_self_energy = nullptr;
