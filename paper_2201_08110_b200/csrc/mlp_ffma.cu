@@ -209,7 +209,7 @@ void launch_gemm(const GemmLaunch& g, cudaStream_t s) {
 // Final layer (one output): e = b + w . h, and the start of the backward pass
 // delta[o] = w[o] * CELU'(h[o]) written over h.  One warp per (atom, model); FP64 dot product.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) last_layer_kernel(LastLayerArgs a) {
+__global__ void __launch_bounds__(128) last_layer_kernel(const __grid_constant__ LastLayerArgs a) {
   const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
   if (w >= a.n_sorted * a.M) return;

@@ -67,8 +67,7 @@ extern "C" void nnp_destroy(nnp_handle* h) {
   for (auto e : h->events) cudaEventDestroy(e);
   void* ptrs[] = {h->d_mol_range, h->d_species, h->d_mol_off, h->d_mol_id, h->d_sortpos, h->d_perm, h->d_grp_off, h->d_self_energy,
                   h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_aev, h->d_daev, h->d_phi,
-                  h->d_eatom, h->d_status, h->d_W, h->d_b, h->d_last_act_off, h->d_last_w_off, h->d_last_b_off,
-                  h->d_last_H, h->d_hpos, h->d_hforce, h->d_henergy};
+                  h->d_eatom, h->d_status, h->d_W, h->d_b, h->d_hpos, h->d_hforce, h->d_henergy};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (int l = 0; l < NNP_MAX_LAYERS; ++l)
@@ -792,13 +791,13 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       flops += 4.0 * ne * (double)M * Hs[e];
       if (ne) wbytes += 4.0 * M * Hs[e];
     }
-    if (upload(&h->d_last_act_off, ao) || upload(&h->d_last_w_off, wo2) || upload(&h->d_last_b_off, bo2) ||
-        upload(&h->d_last_H, Hs))
-      return fail(NNP_ERR_ALLOC);
     LastLayerArgs& la = h->last;
+    memset(&la, 0, sizeof(la));
     la.act = h->d_act[L - 1]; la.W = h->d_W; la.bias = h->d_b; la.e_out = h->d_eatom;
-    la.grp_off = h->d_grp_off; la.act_off = h->d_last_act_off; la.w_off = h->d_last_w_off;
-    la.b_off = h->d_last_b_off; la.H = h->d_last_H;
+    for (int e = 0; e <= S; ++e) la.grp_off[e] = h->grp_off[e];
+    for (int e = 0; e < S; ++e) {
+      la.act_off[e] = ao[e]; la.w_off[e] = wo2[e]; la.b_off[e] = bo2[e]; la.H[e] = Hs[e];
+    }
     la.S = S; la.M = M; la.n_sorted = N; la.alpha = alpha;
   }
   h->work[0] = wbytes;

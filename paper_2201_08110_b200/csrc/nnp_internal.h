@@ -235,11 +235,12 @@ struct LastLayerArgs {
   const float* W;      // arena
   const float* bias;   // arena
   double* e_out;       // [n_sorted][M]
-  const int* grp_off;  // [S+1]
-  const long long* act_off;  // [S] float offset of the group's block in act
-  const long long* w_off;    // [S] float offset of W_L for (e, m=0); models contiguous with stride H
-  const long long* b_off;    // [S]
-  const int* H;        // [S]
+  // per-element tables by value (kernel parameter space: no dependent global loads before the data loads)
+  int grp_off[NNP_MAX_SPECIES + 1];       // [S+1]
+  long long act_off[NNP_MAX_SPECIES];     // [S] float offset of the group's block in act
+  long long w_off[NNP_MAX_SPECIES];       // [S] float offset of W_L for (e, m=0); models contiguous with stride H
+  long long b_off[NNP_MAX_SPECIES];       // [S]
+  int H[NNP_MAX_SPECIES];                 // [S]
   int S, M, n_sorted;
   float alpha;
 };
@@ -289,8 +290,6 @@ struct nnp_handle {
   bool use_pdl = false, pdl_now = false;  // programmatic dependent launches along the chain (pdl_now: this enqueue)
   int n_parts = 1;                   // dE/dAEV is produced as n_parts partial sums (per model at small N)
   LastLayerArgs last;
-  long long *d_last_act_off = nullptr, *d_last_w_off = nullptr, *d_last_b_off = nullptr;
-  int* d_last_H = nullptr;
   // host staging for nnp_compute_host
   float *d_hpos = nullptr, *d_hforce = nullptr;
   double* d_henergy = nullptr;
