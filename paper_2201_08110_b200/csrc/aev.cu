@@ -694,7 +694,8 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(
     const int* __restrict__ atom_index, float* __restrict__ force, int force_stride, float fscale,
     int n_force_blocks, const double* __restrict__ eatom, const int* __restrict__ sortpos,
     const int* __restrict__ species, const int* __restrict__ mol_off, int n_mol, int M,
-    const double* __restrict__ self_energy, double escale, double* __restrict__ energy) {
+    const double* __restrict__ self_energy, double escale, double* __restrict__ energy,
+    const EnergyBlock* __restrict__ eblocks, int n_eblocks, double* __restrict__ epart, int* __restrict__ ecount) {
   const int lane = threadIdx.x & 31;
   const int wib = threadIdx.x >> 5;
   pdl_trigger();
@@ -731,12 +732,16 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(
       f[2] += fscale * fz;
     }
   } else {
-    // one CTA per molecule: thread-strided atoms, warp tree, then the warps in order (fixed tree)
+    // energy blocks: a CTA sums a chunk of a molecule (thread-strided atoms, warp tree, then the warps in order).  A
+    // molecule larger than one chunk is summed by several CTAs; the last one to arrive adds their partial sums in
+    // chunk order (fixed order => bit-identical reruns whatever the arrival order).
     __shared__ double wsum[FIN_WARPS];
-    const int m = blockIdx.x - n_force_blocks;
-    if (m >= n_mol || energy == nullptr) return;
+    __shared__ int s_last;
+    const int bid = blockIdx.x - n_force_blocks;
+    if (bid >= n_eblocks || energy == nullptr) return;
+    const EnergyBlock eb = eblocks[bid];
     double acc = 0.0;
-    for (int i = mol_off[m] + (int)threadIdx.x; i < mol_off[m + 1]; i += FIN_THREADS) {
+    for (int i = eb.a0 + (int)threadIdx.x; i < eb.a1; i += FIN_THREADS) {
       const double* e = eatom + (size_t)sortpos[i] * M;
       double s = 0.0;
       for (int k = 0; k < M; ++k) s += e[k];
@@ -749,7 +754,20 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(
     if (threadIdx.x == 0) {
       double tot = 0.0;
       for (int w = 0; w < FIN_WARPS; ++w) tot += wsum[w];
-      energy[m] = escale * tot;
+      if (eb.n_chunks == 1) {
+        energy[eb.mol] = escale * tot;
+      } else {
+        epart[bid] = tot;
+        __threadfence();
+        s_last = atomicAdd(&ecount[eb.mol], 1) == eb.n_chunks - 1;
+        if (s_last) {
+          __threadfence();
+          double sum = 0.0;
+          for (int q = 0; q < eb.n_chunks; ++q) sum += __ldcg(&epart[eb.first + q]);
+          energy[eb.mol] = escale * sum;
+          ecount[eb.mol] = 0;
+        }
+      }
     }
   }
 }
@@ -825,11 +843,12 @@ void launch_finish(nnp_handle* h, const int* d_atom_index, double* d_energy, flo
                    cudaStream_t s) {
   if (h->N == 0) return;
   const int nfb = (h->N + FIN_WARPS - 1) / FIN_WARPS;
-  const int neb = h->n_mol;
+  const int neb = h->n_eblocks;
   const float fscale = (float)(h->energy_scale * h->length_scale);
   launch_kernel(h->pdl_now, finish_kernel, dim3(nfb + neb), dim3(FIN_THREADS), 0, s, h->d_nbr_r, h->d_cnt_r, h->d_phi,
                 h->N, h->capR, d_atom_index, d_force, force_stride, fscale, nfb, h->d_eatom, h->d_sortpos, h->d_species,
-                h->d_mol_off, h->n_mol, h->M, h->d_self_energy, h->energy_scale, d_energy);
+                h->d_mol_off, h->n_mol, h->M, h->d_self_energy, h->energy_scale, d_energy,
+                (const EnergyBlock*)h->d_eblocks, h->n_eblocks, h->d_epart, h->d_ecount);
 }
 
 int aev_set_smem_attributes(nnp_handle* h) {

@@ -65,7 +65,7 @@ extern "C" void nnp_destroy(nnp_handle* h) {
   cudaDeviceSynchronize();
   if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
   for (auto e : h->events) cudaEventDestroy(e);
-  void* ptrs[] = {h->d_mol_range, h->d_species, h->d_mol_off, h->d_mol_id, h->d_sortpos, h->d_perm, h->d_grp_off, h->d_self_energy,
+  void* ptrs[] = {h->d_eblocks, h->d_epart, h->d_ecount, h->d_mol_range, h->d_species, h->d_mol_off, h->d_mol_id, h->d_sortpos, h->d_perm, h->d_grp_off, h->d_self_energy,
                   h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_aev, h->d_daev, h->d_phi,
                   h->d_eatom, h->d_status, h->d_W, h->d_b, h->d_hpos, h->d_hforce, h->d_henergy};
   for (void* p : ptrs)
@@ -283,6 +283,20 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   // launch it saves (configs[2]: +36 us in the AEV forward against a 12 us neighbour kernel)
   h->fuse_nbr = N > 0 && N <= 512 && !h->use_cells && max_mol <= 256 && !(cfg->flags & NNP_FLAG_NO_NBR_FUSION);
   if (h->use_cells && cells_alloc(h) != 0) return fail(NNP_ERR_ALLOC);
+  {  // energy reduction blocks: chunks of <= 2048 atoms
+    const int ECH = 2048;
+    std::vector<EnergyBlock> eb;
+    for (int m = 0; m < n_molecules; ++m) {
+      const int a0 = mol_off[m], a1 = mol_off[m + 1];
+      const int nch = std::max(1, (a1 - a0 + ECH - 1) / ECH);
+      const int first = (int)eb.size();
+      for (int q = 0; q < nch; ++q) eb.push_back(EnergyBlock{m, std::min(a1, a0 + q * ECH), std::min(a1, a0 + (q + 1) * ECH), first, nch});
+    }
+    h->n_eblocks = (int)eb.size();
+    if (upload(&h->d_eblocks, eb) || dev_alloc(&h->d_epart, eb.size()) || dev_alloc(&h->d_ecount, (size_t)n_molecules))
+      return fail(NNP_ERR_ALLOC);
+    cudaMemset(h->d_ecount, 0, sizeof(int) * (size_t)n_molecules);
+  }
   cudaMemset(h->d_status, 0, sizeof(int));
   cudaMemset(h->d_nbr_r, 0, sizeof(int) * std::max<size_t>((size_t)N * h->capR, 1));
   cudaMemset(h->d_nbr_a, 0, sizeof(int) * std::max<size_t>((size_t)N * h->capA, 1));

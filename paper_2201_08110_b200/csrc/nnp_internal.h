@@ -230,6 +230,11 @@ int mid_build(SmallLaunch& L, std::vector<MidItem>& items);
 void mid_launch(const SmallLaunch& L, cudaStream_t s, bool pdl);
 
 // Final layer (1 output) + start of the backward pass.
+struct EnergyBlock {  // one CTA of the energy reduction: atoms [a0, a1) of molecule `mol`
+  int mol, a0, a1;
+  int first, n_chunks;  // this molecule's CTAs are blocks [first, first + n_chunks) of the energy part
+};
+
 struct LastLayerArgs {
   float* act;          // [n_atoms_sorted][M][H] per element group (arena), overwritten with delta
   const float* W;      // arena
@@ -266,6 +271,10 @@ struct nnp_handle {
   float* d_daev = nullptr;  // [n_parts][N sorted][n_feat]
   float* d_phi = nullptr;   // [N][capR][3]
   double* d_eatom = nullptr;  // [N sorted][M]
+  EnergyBlock* d_eblocks = nullptr;  // energy reduction: large molecules are summed by several CTAs
+  double* d_epart = nullptr;         // [n_eblocks] partial sums
+  int* d_ecount = nullptr;           // [n_mol] arrival counters (reset by the last CTA of a molecule)
+  int n_eblocks = 0;
   // cell-binned neighbour search (nbr_cells.cu), used for large molecules
   bool use_cells = false;
   bool fuse_nbr = false;  // small molecules: the AEV forward kernel builds the neighbour rows itself
