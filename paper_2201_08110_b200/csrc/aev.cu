@@ -186,7 +186,7 @@ __device__ __forceinline__ float gauss(float d, float khi, float klo) {
   return ex2_approx(fmaf(d2, klo, d2 * khi));
 }
 
-constexpr int AEV_THREADS = 256;  // one CTA per centre atom
+constexpr int AEV_THREADS = 256;  // one CTA per centre atom: 256 threads at latency-bound sizes, 128 at large N
 constexpr int TAB_FIELDS = 10;    // per radial slot: ux uy uz rhi rlo fcr dfcr fca dfca spec
 // triplets of a centre processed per pass through shared memory: small enough that 6-8 CTAs share an SM (the
 // phases of a centre are latency-bound, other centres fill the gaps), measured on configs[2] and configs[4]
@@ -511,16 +511,16 @@ __global__ void __launch_bounds__(AEV_THREADS, MULTI ? 4 : 6) aev_backward_kerne
   // dE/dAEV row = fixed-order sum of the partial rows.  All loads of a pass (KC columns x 8 partial rows per thread)
   // are issued before the first add: one memory latency per pass instead of one per partial row
   if (n_parts == 1) {  // large systems: one row, keep as many columns in flight as possible
-    for (int fb = 0; fb < c.n_feat; fb += 8 * AEV_THREADS) {
+    for (int fb = 0; fb < c.n_feat; fb += 8 * (int)blockDim.x) {
       float x[8];
 #pragma unroll
       for (int k = 0; k < 8; ++k) {
-        const int f = fb + k * AEV_THREADS + threadIdx.x;
+        const int f = fb + k * (int)blockDim.x + threadIdx.x;
         x[k] = f < c.n_feat ? gin[f] : 0.0f;
       }
 #pragma unroll
       for (int k = 0; k < 8; ++k) {
-        const int f = fb + k * AEV_THREADS + threadIdx.x;
+        const int f = fb + k * (int)blockDim.x + threadIdx.x;
         if (f < c.n_radial) g[f] = x[k];
         else if (f < c.n_feat) {
           const int fa = f - c.n_radial, blk = fa / c.n_sub;
@@ -530,7 +530,7 @@ __global__ void __launch_bounds__(AEV_THREADS, MULTI ? 4 : 6) aev_backward_kerne
     }
   }
   constexpr int KC = MULTI ? 4 : 2;  // columns per thread and pass: KC x 8 loads in flight before the first add
-  for (int fb = 0; n_parts > 1 && fb < c.n_feat; fb += KC * AEV_THREADS) {
+  for (int fb = 0; n_parts > 1 && fb < c.n_feat; fb += KC * (int)blockDim.x) {
     float acc[KC];
 #pragma unroll
     for (int k = 0; k < KC; ++k) acc[k] = 0.0f;
@@ -538,7 +538,7 @@ __global__ void __launch_bounds__(AEV_THREADS, MULTI ? 4 : 6) aev_backward_kerne
       float x[KC][8];
 #pragma unroll
       for (int k = 0; k < KC; ++k) {
-        const int f = fb + k * AEV_THREADS + threadIdx.x;
+        const int f = fb + k * (int)blockDim.x + threadIdx.x;
 #pragma unroll
         for (int u = 0; u < 8; ++u)
           x[k][u] = (f < c.n_feat && p0 + u < n_parts) ? gin[(size_t)(p0 + u) * part_stride + f] : 0.0f;
@@ -550,7 +550,7 @@ __global__ void __launch_bounds__(AEV_THREADS, MULTI ? 4 : 6) aev_backward_kerne
     }
 #pragma unroll
     for (int k = 0; k < KC; ++k) {
-      const int f = fb + k * AEV_THREADS + threadIdx.x;
+      const int f = fb + k * (int)blockDim.x + threadIdx.x;
       if (f < c.n_radial) g[f] = acc[k];
       else if (f < c.n_feat) {
         const int fa = f - c.n_radial, blk = fa / c.n_sub;
@@ -796,6 +796,14 @@ void launch_neighbors(nnp_handle* h, const float* d_pos, int pos_stride, const i
 }
 
 static bool aev_small_shape(const nnp_handle* h) { return h->aev.n_shf_z <= 4 && h->aev.n_shf_a <= 8; }
+// threads per centre CTA: at large N twice as many (smaller) CTAs per SM hide the barrier phases of a centre better
+// (configs[2]: forward 237 -> 215 us, backward 192 -> 167 us); at ligand sizes the wider CTA is 2 us faster
+// -- in the backward kernel only while shared memory still lets ~10 of the smaller CTAs share an SM (configs[4]
+// backward: 33 KB per CTA, 6 per SM either way, where the wider CTA wins; measured both ways)
+static int aev_block_threads(const nnp_handle* h, bool backward) {
+  if (h->N < 2048) return AEV_THREADS;
+  return (!backward || aev_smem_bytes(h, true) * 10 <= 227 * 1024) ? 128 : AEV_THREADS;
+}
 
 void launch_aev_forward(nnp_handle* h, const float* d_pos, int pos_stride, const int* d_atom_index, cudaStream_t s) {
   if (h->N == 0) return;
@@ -807,12 +815,12 @@ void launch_aev_forward(nnp_handle* h, const float* d_pos, int pos_stride, const
   const int fused = h->fuse_nbr ? 1 : 0;
   const bool pdl = h->pdl_now && !fused;  // fused: first kernel of the step, must not overtake the previous step
   if (aev_small_shape(h))
-    launch_kernel(pdl, aev_forward_kernel<4, 8>, dim3(blocks), dim3(AEV_THREADS), smem, s, (const float4*)h->d_pos4,
+    launch_kernel(pdl, aev_forward_kernel<4, 8>, dim3(blocks), dim3(aev_block_threads(h, false)), smem, s, (const float4*)h->d_pos4,
                   (const int*)h->d_nbr_r, (const int*)h->d_nbr_a, (const int*)h->d_cnt_r, (const int*)h->d_cnt_a,
                   (const int*)h->d_sortpos, h->N, h->aev, h->capR, h->capA, trip_chunk(h, false), h->d_aev, nb, fused,
                   mp_off4, h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a);
   else
-    launch_kernel(pdl, aev_forward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>, dim3(blocks), dim3(AEV_THREADS), smem, s,
+    launch_kernel(pdl, aev_forward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>, dim3(blocks), dim3(aev_block_threads(h, false)), smem, s,
                   (const float4*)h->d_pos4, (const int*)h->d_nbr_r, (const int*)h->d_nbr_a, (const int*)h->d_cnt_r,
                   (const int*)h->d_cnt_a, (const int*)h->d_sortpos, h->N, h->aev, h->capR, h->capA,
                   trip_chunk(h, false), h->d_aev, nb, fused, mp_off4, h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r,
@@ -821,7 +829,7 @@ void launch_aev_forward(nnp_handle* h, const float* d_pos, int pos_stride, const
 
 template <int NZ, int NA, bool MULTI>
 static void launch_aev_backward_t(nnp_handle* h, cudaStream_t s) {
-  launch_kernel(h->pdl_now, aev_backward_kernel<NZ, NA, MULTI>, dim3(h->N), dim3(AEV_THREADS), aev_smem_bytes(h, true), s,
+  launch_kernel(h->pdl_now, aev_backward_kernel<NZ, NA, MULTI>, dim3(h->N), dim3(aev_block_threads(h, true)), aev_smem_bytes(h, true), s,
                 (const float4*)h->d_pos4, (const int*)h->d_nbr_r, (const int*)h->d_nbr_a, (const int*)h->d_cnt_r,
                 (const int*)h->d_cnt_a, (const int*)h->d_sortpos, h->N, h->aev, h->capR, h->capA, trip_chunk(h, true),
                 (const float*)h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
