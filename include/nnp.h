@@ -88,6 +88,7 @@ typedef struct {
 #define NNP_FLAG_NO_NBR_FUSION 1024 /* small molecules: separate neighbour launch instead of building the rows inside the AEV forward kernel */
 #define NNP_FLAG_NO_ZERO_SKIP 2048 /* tensor engine: run layer 1 densely even over AEV columns that are structurally zero */
 #define NNP_FLAG_BWD1_PERSISTENT 4096 /* ligand-size engine: persistent ring-fed layer-1 backward kernel (2-D tensor copies) instead of one CTA per item; faster alone, 1.6 us slower inside the PDL chain at 50 atoms */
+#define NNP_FLAG_NO_BWD1_PAIRS 8192 /* ligand-size engine: one CTA per layer-1 backward item even for light items (<= 4 atoms), which otherwise share a CTA two by two */
 
 /*
  * nnp_create: build a handle for a fixed set of atoms.

@@ -26,6 +26,7 @@ NNP_FLAG_NO_FWD1 = 256
 NNP_FLAG_NO_NBR_FUSION = 1024
 NNP_FLAG_NO_ZERO_SKIP = 2048
 NNP_FLAG_BWD1_PERSISTENT = 4096
+NNP_FLAG_NO_BWD1_PAIRS = 8192
 ERRORS = {
     -1: "NNP_ERR_INVALID_ARG",
     -2: "NNP_ERR_CUDA",

@@ -353,6 +353,8 @@ struct Bwd1pParams {
   const int* cta_off;
   int n_items, n_stages;
   int use_tma;  // one-CTA-per-item kernel: weight chunk by 2-D tensor copies (else one bulk copy per row)
+  int n_single;      // one-CTA-per-item kernel: CTAs [0, n_single) own one item, the rest a pair of light items
+  int pair_floats;   // shared-memory floats of one half of a pair CTA
 };
 
 __device__ __forceinline__ void p1_tma_2d(void* dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
@@ -362,19 +364,29 @@ __device__ __forceinline__ void p1_tma_2d(void* dst, const CUtensorMap* map, int
       : "memory");
 }
 
-template <int NA>
+// NW = warps that work on the item: 8 (the whole CTA) or 4 (two light items share a CTA, one per half: their time is
+// start-up and weight-fetch latency, not arithmetic, so two per SM nearly halves their cost); `tid` is the thread's
+// index within its group, `bar_id` the group's named barrier.
+template <int NW>
+__device__ __forceinline__ void b1_sync(int bar_id) {
+  if (NW == SM_WARPS) __syncthreads();
+  else asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "n"(NW * 32) : "memory");
+}
+
+template <int NA, int NW>
 __device__ __forceinline__ void small_bwd1_body(const SmallBwdItem& it, float* smem_raw, uint64_t* bars,
-                                                const CUtensorMap* wmap) {
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int rps = (((it.n_out + B1_SLICES - 1) / B1_SLICES) + 3) & ~3;  // rows per slice, a multiple of 4
-  const int n_tiles = (it.n_out + 31) >> 5;                              // 32-row tiles of the tensor copies
+                                                const CUtensorMap* wmap, int tid, int bar_id) {
+  constexpr int NT = NW * 32;
+  const int warp = tid >> 5, lane = tid & 31;
+  const int rps = (((it.n_out + NW - 1) / NW) + 3) & ~3;  // rows per slice, a multiple of 4
+  const int n_tiles = (it.n_out + 31) >> 5;               // 32-row tiles of the tensor copies
   const bool tma = wmap != nullptr && n_tiles <= B1_SLICES;
   float* smem_f = smem_raw + (((128u - (s_u32(smem_raw) & 127u)) & 127u) >> 2);  // 128-byte aligned (tensor copies)
-  const size_t ws_floats = max((size_t)n_tiles * 32 * 128, (size_t)B1_SLICES * NA * 128);
-  float* ws = smem_f;               // [n_out][128]; later red [B1_SLICES][NA][128]
+  const size_t ws_floats = max((size_t)n_tiles * 32 * 128, (size_t)NW * NA * 128);
+  float* ws = smem_f;               // [n_out][128]; later red [NW][NA][128]
   float* ds = smem_f + ws_floats;   // [NA][n_out]
   uint64_t* dbar = bars + B1_SLICES;
-  if (threadIdx.x == 0) {
+  if (tid == 0) {
     for (int g = 0; g < B1_SLICES; ++g) {
       sbar_init(&bars[g], 1);
       if (tma) {
@@ -388,20 +400,19 @@ __device__ __forceinline__ void small_bwd1_body(const SmallBwdItem& it, float* s
     sbar_expect_tx(dbar, (uint32_t)(it.n_atoms * it.n_out * 4));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  __syncthreads();
+  b1_sync<NW>(bar_id);
   pdl_trigger();
   if (tma) {  // one 2-D tensor copy per 32-row tile (512-byte row segments as separate bulk copies are issue-bound)
-    if ((int)threadIdx.x < n_tiles)
-      p1_tma_2d(ws + (size_t)threadIdx.x * 32 * 128, wmap, it.t_col0, it.t_row0 + 32 * (int)threadIdx.x, &bars[threadIdx.x]);
+    if (tid < n_tiles) p1_tma_2d(ws + (size_t)tid * 32 * 128, wmap, it.t_col0, it.t_row0 + 32 * tid, &bars[tid]);
   } else {
-    for (int o = threadIdx.x; o < it.n_out; o += SM_THREADS)
+    for (int o = tid; o < it.n_out; o += NT)
       bulk_g2s(ws + (size_t)o * 128, it.W + (size_t)o * it.ldw, (uint32_t)(it.n_cols * 4), &bars[o / rps]);
   }
-  for (int idx = it.n_atoms * it.n_out + threadIdx.x; idx < NA * it.n_out; idx += SM_THREADS) ds[idx] = 0.0f;
+  for (int idx = it.n_atoms * it.n_out + tid; idx < NA * it.n_out; idx += NT) ds[idx] = 0.0f;
   pdl_wait();  // delta comes from the previous kernel
-  if (threadIdx.x < it.n_atoms)
-    bulk_g2s(ds + (size_t)threadIdx.x * it.n_out, it.D + (size_t)threadIdx.x * it.ldd, (uint32_t)(it.n_out * 4), dbar);
-  __syncthreads();  // zero rows of the padding atoms visible
+  if (tid < it.n_atoms)
+    bulk_g2s(ds + (size_t)tid * it.n_out, it.D + (size_t)tid * it.ldd, (uint32_t)(it.n_out * 4), dbar);
+  b1_sync<NW>(bar_id);  // zero rows of the padding atoms visible
   sbar_wait(dbar, 0);
 
   // acc[a][0] = columns (4 lane, 4 lane + 1), acc[a][1] = columns (4 lane + 2, 4 lane + 3) of atom a
@@ -438,7 +449,7 @@ __device__ __forceinline__ void small_bwd1_body(const SmallBwdItem& it, float* s
       }
     }
   }
-  __syncthreads();  // every warp is done with the weight buffer: reuse it for the slice sums
+  b1_sync<NW>(bar_id);  // every warp is done with the weight buffer: reuse it for the slice sums
   float4* red = reinterpret_cast<float4*>(ws);
   if (col_ok) {
 #pragma unroll
@@ -447,13 +458,13 @@ __device__ __forceinline__ void small_bwd1_body(const SmallBwdItem& it, float* s
       red[((size_t)warp * NA + a) * 32 + lane] = make_float4(lo.x, lo.y, hi.x, hi.y);
     }
   }
-  __syncthreads();
-  for (int idx = threadIdx.x; idx < it.n_atoms * 32; idx += SM_THREADS) {
+  b1_sync<NW>(bar_id);
+  for (int idx = tid; idx < it.n_atoms * 32; idx += NT) {
     const int a = idx >> 5, l = idx & 31;
     if (4 * l >= it.n_cols) continue;
     float4 v = red[(size_t)a * 32 + l];
 #pragma unroll
-    for (int s = 1; s < B1_SLICES; ++s) {  // fixed order
+    for (int s = 1; s < NW; ++s) {  // fixed order
       const float4 u = red[((size_t)s * NA + a) * 32 + l];
       v.x += u.x; v.y += u.y; v.z += u.z; v.w += u.w;
     }
@@ -464,13 +475,20 @@ __device__ __forceinline__ void small_bwd1_body(const SmallBwdItem& it, float* s
 
 __global__ void __launch_bounds__(SM_THREADS, 1) small_bwd1_kernel(const __grid_constant__ Bwd1pParams P) {
   extern __shared__ __align__(16) float smem_f[];
-  __shared__ __align__(8) uint64_t bars[B1_SLICES + 1];
+  __shared__ __align__(8) uint64_t bars[2][B1_SLICES + 1];
+  if ((int)blockIdx.x >= P.n_single) {  // two light items (<= 4 atoms), one per half of the CTA
+    const int half = threadIdx.x >> 7;
+    const SmallBwdItem it = P.items[P.n_single + 2 * ((int)blockIdx.x - P.n_single) + half];
+    small_bwd1_body<4, SM_WARPS / 2>(it, smem_f + (size_t)half * P.pair_floats, bars[half],
+                                     P.use_tma ? &P.wmap[it.tmap] : nullptr, threadIdx.x & 127, 1 + half);
+    return;
+  }
   const SmallBwdItem it = P.items[blockIdx.x];
   const CUtensorMap* wmap = P.use_tma ? &P.wmap[it.tmap] : nullptr;
-  if (it.n_atoms <= 4) small_bwd1_body<4>(it, smem_f, bars, wmap);
-  else if (it.n_atoms <= 8) small_bwd1_body<8>(it, smem_f, bars, wmap);
-  else if (it.n_atoms <= 16) small_bwd1_body<16>(it, smem_f, bars, wmap);
-  else small_bwd1_body<24>(it, smem_f, bars, wmap);
+  if (it.n_atoms <= 4) small_bwd1_body<4, SM_WARPS>(it, smem_f, bars[0], wmap, threadIdx.x, 0);
+  else if (it.n_atoms <= 8) small_bwd1_body<8, SM_WARPS>(it, smem_f, bars[0], wmap, threadIdx.x, 0);
+  else if (it.n_atoms <= 16) small_bwd1_body<16, SM_WARPS>(it, smem_f, bars[0], wmap, threadIdx.x, 0);
+  else small_bwd1_body<24, SM_WARPS>(it, smem_f, bars[0], wmap, threadIdx.x, 0);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -902,7 +920,7 @@ int small_build_bwd(SmallLaunch& L, std::vector<SmallBwdItem>& items) {
 static int bwd1_pad(int n_atoms) { return n_atoms <= 4 ? 4 : n_atoms <= 8 ? 8 : n_atoms <= 16 ? 16 : 24; }
 
 // layer-1 backward items: n_atoms <= 24, n_cols <= 128, epilogue EPI_SCALE
-int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool persistent_ok,
+int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool persistent_ok, bool pairs_ok,
                      const std::vector<TmaOperand>& wops) {
   std::stable_sort(items.begin(), items.end(), [](const SmallBwdItem& a, const SmallBwdItem& b) {
     return (long long)a.n_out * a.n_cols * (a.n_atoms + 4) > (long long)b.n_out * b.n_cols * (b.n_atoms + 4);
@@ -975,6 +993,33 @@ int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool pers
     L.stages = (int)std::min<size_t>(P1_MAX_STAGES, (P1_SMEM - P1_FIXED) / ((size_t)P1_TILE_ROWS * 128 * 4));
     L.smem_bytes = P1_FIXED + (size_t)L.stages * P1_TILE_ROWS * 128 * 4 + 128;
   }
+  // one CTA per item, except that light items (<= 4 atoms) go two to a CTA, one per half, when both fit
+  int n_single = (int)items.size();
+  size_t pair_floats = 0;
+  if (L.variant == 100) {
+    L.grid = (int)items.size();
+    if (pairs_ok) {
+      auto item_bytes = [](const SmallBwdItem& it) {
+        const size_t rows32 = (size_t)((it.n_out + 31) / 32) * 32;
+        return (std::max(rows32 * 128, (size_t)(B1_SLICES / 2) * 4 * 128) + (size_t)it.n_out * 4) * 4 + 128;
+      };
+      size_t half = 0;
+      for (const auto& it : items)
+        if (it.n_atoms <= 4) half = std::max(half, item_bytes(it));
+      half = (half + 127) & ~(size_t)127;
+      if (half && 2 * half <= SMALL_SMEM_MAX) {
+        auto mid = std::stable_partition(items.begin(), items.end(), [](const SmallBwdItem& it) { return it.n_atoms > 4; });
+        int n_light = (int)(items.end() - mid);
+        n_light &= ~1;  // an odd one out runs alone
+        n_single = (int)items.size() - n_light;
+        pair_floats = half / 4;
+        if (n_light) L.smem_bytes = std::max(L.smem_bytes, 2 * half);
+        L.grid = n_single + n_light / 2;
+      }
+    }
+  }
+  P->n_single = n_single;
+  P->pair_floats = (int)pair_floats;
   if (L.smem_bytes > (L.variant == 102 ? P1_SMEM : SMALL_SMEM_MAX)) return -1;
   if (cudaMalloc(&L.d_items, std::max<size_t>(1, items.size()) * sizeof(SmallBwdItem)) != cudaSuccess) return -1;
   if (!items.empty())
@@ -1031,7 +1076,7 @@ void small_launch_bwd(const SmallLaunch& L, cudaStream_t s, bool pdl) {
     return;
   }
   if (L.variant == 100) {
-    launch_kernel(pdl, small_bwd1_kernel, dim3(L.n_items), dim3(SM_THREADS), L.smem_bytes, s,
+    launch_kernel(pdl, small_bwd1_kernel, dim3(L.grid), dim3(SM_THREADS), L.smem_bytes, s,
                   *reinterpret_cast<const Bwd1pParams*>(L.params));
     return;
   }

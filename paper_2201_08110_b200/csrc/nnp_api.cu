@@ -788,7 +788,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       }
       SmallLaunch sl;
       sl.name = "mlp_bwd_l" + std::to_string(l);
-      if (bwd1 ? small_build_bwd1(sl, items, (cfg->flags & NNP_FLAG_BWD1_PERSISTENT) != 0, wops) : small_build_bwd(sl, items)) { small_free_launch(sl); return fail(NNP_ERR_CUDA); }
+      if (bwd1 ? small_build_bwd1(sl, items, (cfg->flags & NNP_FLAG_BWD1_PERSISTENT) != 0, (cfg->flags & NNP_FLAG_NO_BWD1_PAIRS) == 0, wops) : small_build_bwd(sl, items)) { small_free_launch(sl); return fail(NNP_ERR_CUDA); }
       h->sbwd.push_back(sl);
     }
   }

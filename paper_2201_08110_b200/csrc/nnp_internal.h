@@ -204,7 +204,7 @@ int small_init();
 void small_bwd_shape(int n_atoms, int* AW, int* G);
 int small_build_fwd(SmallLaunch& L, std::vector<SmallFwdItem>& items);
 int small_build_bwd(SmallLaunch& L, std::vector<SmallBwdItem>& items);
-int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool persistent_ok,
+int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool persistent_ok, bool pairs_ok,
                      const std::vector<TmaOperand>& wops);  // wops[tmap]: the [rows][cols] layer-1 weight block of an element
 int small_build_fwd1(SmallLaunch& L, std::vector<Fwd1Item>& items);
 int small_fwd1_tile_rows();  // layer 1: persistent, weights streamed through a ring  // layer 1: weights read once, FFMA2

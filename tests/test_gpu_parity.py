@@ -14,13 +14,13 @@ torch = pytest.importorskip("torch")
 
 from oracle.ani_oracle import AniOracle  # noqa: E402
 from paper_2201_08110_b200 import workloads as wl  # noqa: E402
-from paper_2201_08110_b200.binding import (NNP, NNP_FLAG_BWD1_PERSISTENT, NNP_FLAG_FORCE_CELLS, NNP_FLAG_NO_CELLS, NNP_FLAG_NO_GRAPH,  # noqa: E402
+from paper_2201_08110_b200.binding import (NNP, NNP_FLAG_BWD1_PERSISTENT, NNP_FLAG_NO_BWD1_PAIRS, NNP_FLAG_FORCE_CELLS, NNP_FLAG_NO_CELLS, NNP_FLAG_NO_GRAPH,  # noqa: E402
                                             NNP_FLAG_NO_FWD1, NNP_FLAG_NO_MID, NNP_FLAG_NO_NBR_FUSION, NNP_FLAG_NO_PDL, NNP_FLAG_NO_SMALL, NNP_FLAG_NO_TMA,
                                             NNP_FLAG_NO_UMMA, NNP_FLAG_NO_ZERO_SKIP, NNPError)
 
 # MLP engines: ligand-size weight-streaming FFMA (default at these sizes; with the fused middle launch or
 # one launch per layer), tcgen05 3xTF32, TMA+FFMA, plain FFMA
-ENGINES = {"small": 0, "small_bwd1p": NNP_FLAG_BWD1_PERSISTENT, "small_layers": NNP_FLAG_NO_MID | NNP_FLAG_NO_FWD1 | NNP_FLAG_NO_NBR_FUSION, "umma": NNP_FLAG_NO_SMALL, "tma": NNP_FLAG_NO_SMALL | NNP_FLAG_NO_UMMA,
+ENGINES = {"small": 0, "small_bwd1p": NNP_FLAG_BWD1_PERSISTENT, "small_nopairs": NNP_FLAG_NO_BWD1_PAIRS, "small_layers": NNP_FLAG_NO_MID | NNP_FLAG_NO_FWD1 | NNP_FLAG_NO_NBR_FUSION, "umma": NNP_FLAG_NO_SMALL, "tma": NNP_FLAG_NO_SMALL | NNP_FLAG_NO_UMMA,
            "ffma": NNP_FLAG_NO_SMALL | NNP_FLAG_NO_UMMA | NNP_FLAG_NO_TMA}
 
 E_TOL_PER_ATOM = 1e-5  # kcal/mol
@@ -129,7 +129,7 @@ def test_config1_stagewise(engine):
     nnp.destroy()
 
 
-@pytest.mark.parametrize("engine", ["small", "small_bwd1p", "small_layers", "umma"])
+@pytest.mark.parametrize("engine", ["small", "small_bwd1p", "small_nopairs", "small_layers", "umma"])
 def test_config2_trajectory_steps(engine):
     """configs[1]: 50 atoms, 8 models, perturbed steps 0,1,10,100,999 of the 1000-step trajectory."""
     w = wl.config2()
@@ -318,7 +318,7 @@ def test_biases_self_energy_scales_and_embedding():
 
 @pytest.mark.parametrize("n_species,hidden,n,seed", [(3, (16, 12, 8), 37, 1), (2, (32, 20, 4), 70, 2),
                                                       (5, (64, 32, 16), 150, 3)])
-@pytest.mark.parametrize("engine", ["small", "small_bwd1p", "small_layers", "umma"])
+@pytest.mark.parametrize("engine", ["small", "small_bwd1p", "small_nopairs", "small_layers", "umma"])
 def test_small_parameter_sets(n_species, hidden, n, seed, engine):
     """Generic nnp_config (other species counts / layer widths): ragged tiles in every GEMM."""
     p = wl.small_params(n_species, hidden)
