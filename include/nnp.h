@@ -77,8 +77,8 @@ typedef struct {
 } nnp_config;
 
 #define NNP_FLAG_NO_GRAPH 1 /* launch kernels one by one instead of replaying a CUDA graph */
-#define NNP_FLAG_NO_TMA 2   /* run the MLP layers on the plain (non-TMA) grouped FFMA kernel */
-#define NNP_FLAG_NO_UMMA 4  /* keep the MLP layers off the tcgen05 tensor-core engine (FP32 FFMA engines instead) */
+#define NNP_FLAG_NO_UMMA 4  /* keep the MLP layers off the tcgen05 tensor-core engine (grouped FP32 FFMA GEMMs instead: the engine of
+                              shapes the tensor engine does not take, i.e. hidden widths that are not multiples of 32) */
 #define NNP_FLAG_NO_SMALL 8 /* do not use the ligand-size weight-streaming engine even when every element group is small */
 #define NNP_FLAG_NO_MID 16  /* ligand-size engine: one launch per layer instead of the fused middle-of-the-network launch */
 #define NNP_FLAG_NO_PDL 32  /* plain stream-ordered launches instead of programmatic dependent launches along the chain */
@@ -87,8 +87,6 @@ typedef struct {
 #define NNP_FLAG_NO_FWD1 256     /* ligand-size engine: row-pair layer-1 forward kernel instead of the persistent ring-fed one */
 #define NNP_FLAG_NO_NBR_FUSION 1024 /* small molecules: separate neighbour launch instead of building the rows inside the AEV forward kernel */
 #define NNP_FLAG_NO_ZERO_SKIP 2048 /* tensor engine: run layer 1 densely even over AEV columns that are structurally zero */
-#define NNP_FLAG_BWD1_PERSISTENT 4096 /* ligand-size engine: persistent ring-fed layer-1 backward kernel (2-D tensor copies) instead of one CTA per item; faster alone, 1.6 us slower inside the PDL chain at 50 atoms */
-#define NNP_FLAG_NO_BWD1_PAIRS 8192 /* ligand-size engine: one CTA per layer-1 backward item even for light items (<= 4 atoms), which otherwise share a CTA two by two */
 
 /*
  * nnp_create: build a handle for a fixed set of atoms.

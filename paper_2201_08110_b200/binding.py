@@ -15,7 +15,6 @@ LIB_PATH = os.path.join(_HERE, "libnnp_b200.so")
 
 NNP_OK = 0
 NNP_FLAG_NO_GRAPH = 1
-NNP_FLAG_NO_TMA = 2
 NNP_FLAG_NO_UMMA = 4
 NNP_FLAG_NO_SMALL = 8
 NNP_FLAG_NO_MID = 16
@@ -25,8 +24,6 @@ NNP_FLAG_FORCE_CELLS = 128
 NNP_FLAG_NO_FWD1 = 256
 NNP_FLAG_NO_NBR_FUSION = 1024
 NNP_FLAG_NO_ZERO_SKIP = 2048
-NNP_FLAG_BWD1_PERSISTENT = 4096
-NNP_FLAG_NO_BWD1_PAIRS = 8192
 ERRORS = {
     -1: "NNP_ERR_INVALID_ARG",
     -2: "NNP_ERR_CUDA",

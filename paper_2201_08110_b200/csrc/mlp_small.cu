@@ -492,186 +492,6 @@ __global__ void __launch_bounds__(SM_THREADS, 1) small_bwd1_kernel(const __grid_
 }
 
 // ------------------------------------------------------------------------------------------------
-// backward through layer 1, persistent: the same items and arithmetic as small_bwd1_kernel, but one CTA per SM
-// walks a list of items (round-robin over the heavy-first order) while a producer warp streams the weight chunks
-// of successive items as [32 rows][128 columns] tiles through a ring -- ahead of the consumers, across item
-// boundaries and before griddepcontrol.wait -- so the per-item start-up chain (item fetch, 256 bulk copies,
-// first wait) of the 3 waves of the one-item-per-CTA kernel disappears.  A consumer warp owns 4 rows of every
-// tile and keeps the NA x 4 accumulators of its lane in registers over the whole item; the delta tiles of
-// successive items are double-buffered by the consumers themselves; 8-way fixed-order sum at the end of an item.
-constexpr int P1_TILE_ROWS = 32;
-constexpr int P1_MAX_STAGES = 8;
-constexpr int P1_NA_MAX = 24;
-constexpr int P1_NOUT_MAX = 256;
-constexpr int P1_CONSUMERS = SM_THREADS;            // 8 consumer warps
-constexpr int P1_THREADS = P1_CONSUMERS + 32;       // + producer warp
-static const size_t P1_SMEM = 208 * 1024 + 128;
-static const size_t P1_FIXED = (size_t)(2 * P1_NA_MAX * P1_NOUT_MAX + (SM_WARPS / 2) * P1_NA_MAX * 128) * 4;  // D x2 + red
-
-__device__ __forceinline__ void p1_consumer_sync() { asm volatile("bar.sync 2, %0;" ::"n"(P1_CONSUMERS) : "memory"); }
-
-template <int NA>
-__device__ __forceinline__ void p1_item(const SmallBwdItem& it, const float* __restrict__ ring, const float* __restrict__ ds,
-                                        float4* __restrict__ red, uint64_t* full, uint64_t* empty, uint32_t& slot,
-                                        uint32_t& phase, int n_stages) {
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  unsigned long long acc[NA][2];
-#pragma unroll
-  for (int a = 0; a < NA; ++a) acc[a][0] = acc[a][1] = 0ull;
-  const bool col_ok = 4 * lane < it.n_cols;
-  for (int o0 = 0; o0 < it.n_out; o0 += P1_TILE_ROWS) {
-    sbar_wait(&full[slot], phase);
-    const int o = o0 + 4 * warp;  // n_out % 4 == 0: the warp's four rows are valid together
-    if (col_ok && o < it.n_out) {
-      const float4* wp = reinterpret_cast<const float4*>(ring + (size_t)slot * P1_TILE_ROWS * 128) + (4 * warp) * 32 + lane;
-      unsigned long long wlo[4], whi[4];
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const float4 w = wp[i * 32];
-        wlo[i] = pack2(w.x, w.y);
-        whi[i] = pack2(w.z, w.w);
-      }
-#pragma unroll
-      for (int a = 0; a < NA; ++a) {
-        const float4 d = *reinterpret_cast<const float4*>(ds + (size_t)a * P1_NOUT_MAX + o);
-        const unsigned long long d0 = pack2(d.x, d.x), d1 = pack2(d.y, d.y), d2 = pack2(d.z, d.z), d3 = pack2(d.w, d.w);
-        acc[a][0] = ffma2(d0, wlo[0], acc[a][0]); acc[a][1] = ffma2(d0, whi[0], acc[a][1]);
-        acc[a][0] = ffma2(d1, wlo[1], acc[a][0]); acc[a][1] = ffma2(d1, whi[1], acc[a][1]);
-        acc[a][0] = ffma2(d2, wlo[2], acc[a][0]); acc[a][1] = ffma2(d2, whi[2], acc[a][1]);
-        acc[a][0] = ffma2(d3, wlo[3], acc[a][0]); acc[a][1] = ffma2(d3, whi[3], acc[a][1]);
-      }
-    }
-    __syncwarp();
-    if (lane == 0) sbar_arrive(&empty[slot]);
-    if (++slot == (uint32_t)n_stages) { slot = 0; phase ^= 1u; }
-  }
-  // 8 warp partials -> 4 (upper warps hand theirs to the lower ones through shared memory) -> 1, fixed order
-  constexpr int HW = SM_WARPS / 2;
-  if (col_ok && warp >= HW) {
-#pragma unroll
-    for (int a = 0; a < NA; ++a) {
-      const float2 lo = unpack2(acc[a][0]), hi = unpack2(acc[a][1]);
-      red[((size_t)(warp - HW) * NA + a) * 32 + lane] = make_float4(lo.x, lo.y, hi.x, hi.y);
-    }
-  }
-  p1_consumer_sync();
-  if (col_ok && warp < HW) {
-#pragma unroll
-    for (int a = 0; a < NA; ++a) {
-      const float2 lo = unpack2(acc[a][0]), hi = unpack2(acc[a][1]);
-      float4 u = red[((size_t)warp * NA + a) * 32 + lane];
-      u.x += lo.x; u.y += lo.y; u.z += hi.x; u.w += hi.y;
-      red[((size_t)warp * NA + a) * 32 + lane] = u;
-    }
-  }
-  p1_consumer_sync();
-  for (int idx = threadIdx.x; idx < it.n_atoms * 32; idx += P1_CONSUMERS) {
-    const int a = idx >> 5, l = idx & 31;
-    if (4 * l >= it.n_cols) continue;
-    float4 v = red[(size_t)a * 32 + l];
-#pragma unroll
-    for (int s = 1; s < HW; ++s) {  // fixed order
-      const float4 u = red[((size_t)s * NA + a) * 32 + l];
-      v.x += u.x; v.y += u.y; v.z += u.z; v.w += u.w;
-    }
-    v.x *= it.scale; v.y *= it.scale; v.z *= it.scale; v.w *= it.scale;
-    *reinterpret_cast<float4*>(it.out + (size_t)a * it.ldo + 4 * l) = v;
-  }
-  p1_consumer_sync();  // red and this item's delta buffer are free again
-}
-
-__global__ void __launch_bounds__(P1_THREADS, 1) small_bwd1p_kernel(const __grid_constant__ Bwd1pParams P) {
-  const SmallBwdItem* __restrict__ items = P.items;
-  const int n_stages = P.n_stages;
-  const int q_begin = P.cta_off[blockIdx.x], q_end = P.cta_off[blockIdx.x + 1];
-  extern __shared__ __align__(16) float smem_f[];
-  __shared__ __align__(8) uint64_t full[P1_MAX_STAGES];
-  __shared__ __align__(8) uint64_t empty[P1_MAX_STAGES];
-  __shared__ __align__(8) uint64_t dfull[2];
-  __shared__ SmallBwdItem s_it[2];
-  // [n_stages][32][128], 128-byte aligned for the tensor copies
-  float* ring = smem_f + (((128u - (s_u32(smem_f) & 127u)) & 127u) >> 2);
-  float* dbuf = ring + (size_t)n_stages * P1_TILE_ROWS * 128;            // [2][P1_NA_MAX][P1_NOUT_MAX]
-  float4* red = reinterpret_cast<float4*>(dbuf + 2 * P1_NA_MAX * P1_NOUT_MAX);  // [4][NA][32]
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  if (threadIdx.x == 0) {
-    for (int s = 0; s < n_stages; ++s) {
-      sbar_init(&full[s], 1);
-      sbar_init(&empty[s], SM_WARPS);
-    }
-    sbar_init(&dfull[0], 1);
-    sbar_init(&dfull[1], 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncthreads();
-  pdl_trigger();
-
-  if (warp == SM_WARPS) {
-    // ------------------------------------------------------------ producer: weight tiles of all my items, one 2-D
-    // tensor copy per [32 rows][128 columns] tile (512-byte row segments as separate bulk copies are issue-bound:
-    // ~60 cycles each; columns beyond the matrix are zero-filled, rows beyond n_out are never read)
-    if (lane == 0) {
-      uint32_t slot = 0, phase = 0;
-      for (int q = q_begin; q < q_end; ++q) {
-        const CUtensorMap* map = &P.wmap[items[q].tmap];
-        const int row0 = items[q].t_row0, col0 = items[q].t_col0, n_out = items[q].n_out;
-        for (int o0 = 0; o0 < n_out; o0 += P1_TILE_ROWS) {
-          sbar_wait(&empty[slot], phase ^ 1u);
-          sbar_expect_tx(&full[slot], (uint32_t)(P1_TILE_ROWS * 128 * 4));
-          p1_tma_2d(ring + (size_t)slot * P1_TILE_ROWS * 128, map, col0, row0 + o0, &full[slot]);
-          if (++slot == (uint32_t)n_stages) { slot = 0; phase ^= 1u; }
-        }
-      }
-    }
-    pdl_wait();
-    return;
-  }
-
-  // -------------------------------------------------------------- consumers
-  pdl_wait();  // the delta rows come from the previous kernel
-  auto issue_delta = [&](int q, int buf) {  // one thread: expect + the item's delta rows into dbuf[buf]
-    const SmallBwdItem* g = items + q;
-    const int na = g->n_atoms, no = g->n_out, ldd = g->ldd;
-    const float* D = g->D;
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // earlier generic zero-fills of this buffer
-    sbar_expect_tx(&dfull[buf], (uint32_t)(na * no * 4));
-    for (int a = 0; a < na; ++a)
-      bulk_g2s(dbuf + ((size_t)buf * P1_NA_MAX + a) * P1_NOUT_MAX, D + (size_t)a * ldd, (uint32_t)(no * 4), &dfull[buf]);
-  };
-  auto load_item = [&](int q, int buf) {
-    const int* src = reinterpret_cast<const int*>(items + q);
-    int* dst = reinterpret_cast<int*>(&s_it[buf]);
-    for (int w = threadIdx.x; w < (int)(sizeof(SmallBwdItem) / 4); w += P1_CONSUMERS) dst[w] = src[w];
-  };
-  int q = q_begin;
-  if (q < q_end) {
-    load_item(q, 0);
-    if (threadIdx.x == 0) issue_delta(q, 0);
-  }
-  p1_consumer_sync();
-  uint32_t slot = 0, phase = 0;
-  for (int k = 0; q < q_end; ++q, ++k) {
-    const int cur = k & 1;
-    const int qn = q + 1;
-    if (qn < q_end) {  // next item: descriptor and delta rows into the other buffers (free since item k-1 ended)
-      load_item(qn, cur ^ 1);
-      if (threadIdx.x == 0) issue_delta(qn, cur ^ 1);
-    }
-    const SmallBwdItem& it = s_it[cur];
-    const int NAp = it.n_atoms <= 4 ? 4 : it.n_atoms <= 8 ? 8 : it.n_atoms <= 16 ? 16 : 24;
-    float* ds = dbuf + (size_t)cur * P1_NA_MAX * P1_NOUT_MAX;
-    sbar_wait(&dfull[cur], (uint32_t)((k >> 1) & 1));
-    // rows of the padding atoms: zero (rows sit at the fixed pitch P1_NOUT_MAX)
-    for (int idx = it.n_atoms * P1_NOUT_MAX + threadIdx.x; idx < NAp * P1_NOUT_MAX; idx += P1_CONSUMERS) ds[idx] = 0.0f;
-    p1_consumer_sync();
-    if (NAp == 4) p1_item<4>(it, ring, ds, red, full, empty, slot, phase, n_stages);
-    else if (NAp == 8) p1_item<8>(it, ring, ds, red, full, empty, slot, phase, n_stages);
-    else if (NAp == 16) p1_item<16>(it, ring, ds, red, full, empty, slot, phase, n_stages);
-    else p1_item<24>(it, ring, ds, red, full, empty, slot, phase, n_stages);
-  }
-}
-
-// ------------------------------------------------------------------------------------------------
 // forward through layer 1 (the 43 MB layer): out[a][r] = CELU(b[r] + sum_k W[r][k] X[a][k]),  K = 1008
 // ------------------------------------------------------------------------------------------------
 // Persistent: one CTA per SM-sized share of ONE element's weight rows (the rows of all models of an (element,
@@ -867,7 +687,6 @@ int small_init() {
   rc |= set_smem(small_fwd_kernel<8>, SMALL_SMEM_MAX);
   rc |= set_smem(small_bwd_kernel, SMALL_SMEM_MAX);
   rc |= set_smem(small_bwd1_kernel, SMALL_SMEM_MAX);
-  rc |= set_smem(small_bwd1p_kernel, P1_SMEM);
   rc |= set_smem(small_fwd1_kernel, F1_SMEM);
   return rc;
 }
@@ -920,8 +739,7 @@ int small_build_bwd(SmallLaunch& L, std::vector<SmallBwdItem>& items) {
 static int bwd1_pad(int n_atoms) { return n_atoms <= 4 ? 4 : n_atoms <= 8 ? 8 : n_atoms <= 16 ? 16 : 24; }
 
 // layer-1 backward items: n_atoms <= 24, n_cols <= 128, epilogue EPI_SCALE
-int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool persistent_ok, bool pairs_ok,
-                     const std::vector<TmaOperand>& wops) {
+int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, const std::vector<TmaOperand>& wops) {
   std::stable_sort(items.begin(), items.end(), [](const SmallBwdItem& a, const SmallBwdItem& b) {
     return (long long)a.n_out * a.n_cols * (a.n_atoms + 4) > (long long)b.n_out * b.n_cols * (b.n_atoms + 4);
   });
@@ -929,7 +747,6 @@ int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool pers
   L.variant = 100;
   L.smem_bytes = 0;
   bool maps_ok = !wops.empty() && wops.size() <= NNP_MAX_SPECIES;
-  bool fits_persistent = true;
   for (const auto& it : items) {
     if (it.n_atoms < 1 || it.n_atoms > 24 || it.n_cols > 128 || it.epi != EPI_SCALE) return -1;
     const int NA = bwd1_pad(it.n_atoms);
@@ -937,7 +754,6 @@ int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool pers
     const size_t b = (std::max(rows32 * 128, (size_t)B1_SLICES * NA * 128) + (size_t)it.n_out * NA) * 4 + 128;
     L.smem_bytes = std::max(L.smem_bytes, b);
     maps_ok = maps_ok && it.tmap >= 0 && it.tmap < (int)wops.size();
-    fits_persistent = fits_persistent && it.n_out <= P1_NOUT_MAX && it.n_out % 4 == 0;
   }
   // tensor maps of the elements' layer-1 weight blocks: [rows][cols] f32, box 32 rows x 128 columns, no swizzle
   Bwd1pParams* P = new Bwd1pParams();
@@ -955,7 +771,7 @@ int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool pers
     for (size_t k = 0; k < wops.size() && maps_ok; ++k) {
       cuuint64_t gdim[2] = {(cuuint64_t)wops[k].cols, (cuuint64_t)std::max<long long>(wops[k].rows, 1)};
       cuuint64_t gstr[1] = {(cuuint64_t)wops[k].ld * 4};
-      cuuint32_t box[2] = {128, (cuuint32_t)P1_TILE_ROWS};
+      cuuint32_t box[2] = {128, 32};
       cuuint32_t estr[2] = {1, 1};
       if (((EncodeFn)fp)(&P->wmap[k], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)wops[k].base, gdim, gstr, box, estr,
                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -965,40 +781,12 @@ int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool pers
   }
   P->use_tma = maps_ok ? 1 : 0;
   std::vector<int> p1_off(1, 0);
-  if (persistent_ok && maps_ok && fits_persistent) {
-    int dev = 0, sms = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    L.variant = 102;
-    L.grid = std::max(1, std::min((int)items.size(), sms));
-    // static balance (deterministic): heavy-first, each item to the least loaded CTA; cost model from cycle traces
-    // (a tile costs ~300 + 60 NA cycles, an item ~1500 cycles of set-up and reduction)
-    std::vector<long long> load(L.grid, 0);
-    std::vector<std::vector<SmallBwdItem>> per(L.grid);
-    for (const auto& it : items) {
-      const int NA = bwd1_pad(it.n_atoms);
-      const long long c = (long long)((it.n_out + P1_TILE_ROWS - 1) / P1_TILE_ROWS) * (300 + 60 * NA) + 1500;
-      int best = 0;
-      for (int b = 1; b < L.grid; ++b)
-        if (load[b] < load[best]) best = b;
-      load[best] += c;
-      per[best].push_back(it);
-    }
-    items.clear();
-    p1_off.assign(L.grid + 1, 0);
-    for (int b = 0; b < L.grid; ++b) {
-      for (const auto& it : per[b]) items.push_back(it);
-      p1_off[b + 1] = (int)items.size();
-    }
-    L.stages = (int)std::min<size_t>(P1_MAX_STAGES, (P1_SMEM - P1_FIXED) / ((size_t)P1_TILE_ROWS * 128 * 4));
-    L.smem_bytes = P1_FIXED + (size_t)L.stages * P1_TILE_ROWS * 128 * 4 + 128;
-  }
   // one CTA per item, except that light items (<= 4 atoms) go two to a CTA, one per half, when both fit
   int n_single = (int)items.size();
   size_t pair_floats = 0;
-  if (L.variant == 100) {
+  {
     L.grid = (int)items.size();
-    if (pairs_ok) {
+    {
       auto item_bytes = [](const SmallBwdItem& it) {
         const size_t rows32 = (size_t)((it.n_out + 31) / 32) * 32;
         return (std::max(rows32 * 128, (size_t)(B1_SLICES / 2) * 4 * 128) + (size_t)it.n_out * 4) * 4 + 128;
@@ -1020,7 +808,7 @@ int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool pers
   }
   P->n_single = n_single;
   P->pair_floats = (int)pair_floats;
-  if (L.smem_bytes > (L.variant == 102 ? P1_SMEM : SMALL_SMEM_MAX)) return -1;
+  if (L.smem_bytes > SMALL_SMEM_MAX) return -1;
   if (cudaMalloc(&L.d_items, std::max<size_t>(1, items.size()) * sizeof(SmallBwdItem)) != cudaSuccess) return -1;
   if (!items.empty())
     cudaMemcpy(L.d_items, items.data(), items.size() * sizeof(SmallBwdItem), cudaMemcpyHostToDevice);
@@ -1070,11 +858,6 @@ void small_launch_fwd(const SmallLaunch& L, cudaStream_t s, bool pdl) {
 
 void small_launch_bwd(const SmallLaunch& L, cudaStream_t s, bool pdl) {
   if (L.n_items == 0) return;
-  if (L.variant == 102) {
-    launch_kernel(pdl, small_bwd1p_kernel, dim3(L.grid), dim3(P1_THREADS), L.smem_bytes, s,
-                  *reinterpret_cast<const Bwd1pParams*>(L.params));
-    return;
-  }
   if (L.variant == 100) {
     launch_kernel(pdl, small_bwd1_kernel, dim3(L.grid), dim3(SM_THREADS), L.smem_bytes, s,
                   *reinterpret_cast<const Bwd1pParams*>(L.params));

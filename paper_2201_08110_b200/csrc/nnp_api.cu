@@ -77,8 +77,6 @@ extern "C" void nnp_destroy(nnp_handle* h) {
       if (g.d_probs) cudaFree(g.d_probs);
       if (g.d_tiles) cudaFree(g.d_tiles);
     }
-  for (auto* v : {&h->tfwd, &h->tbwd})
-    for (auto& g : *v) tma_free_launch(g);
   for (auto* v : {&h->ufwd, &h->ubwd})
     for (auto& g : *v) umma_free_launch(g);
   for (auto* v : {&h->sfwd, &h->sbwd})
@@ -250,12 +248,11 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     if (upload(&h->d_W, W) || upload(&h->d_b, B)) return fail(NNP_ERR_ALLOC);
   }
 
-  // ---- MLP engine: TMA-staged persistent GEMMs when the shapes allow 32-float boxes
-  bool tma_ok = !(cfg->flags & NNP_FLAG_NO_TMA) && n_feat % 4 == 0 && N > 0;
-  for (int e = 0; e < S && tma_ok; ++e)
+  // ---- MLP engine: the tensor-core engine needs hidden widths that are whole 32-float TMA boxes
+  bool box_ok = n_feat % 4 == 0 && N > 0;
+  for (int e = 0; e < S && box_ok; ++e)
     for (int l = 1; l < L; ++l)
-      if (h->dims[e * (L + 1) + l] % 32 != 0) tma_ok = false;
-  if (tma_ok && tma_init() != 0) tma_ok = false;
+      if (h->dims[e * (L + 1) + l] % 32 != 0) box_ok = false;
   // ligand-size engine: every element group is small, so the layers are weight-streaming problems
   int max_grp = 0, max_dim = n_feat;
   for (int e = 0; e < S; ++e) {
@@ -265,11 +262,10 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   const bool parts_fit = (size_t)N * M * n_feat * 4 <= ((size_t)8 << 20);
   h->use_small = !(cfg->flags & NNP_FLAG_NO_SMALL) && N > 0 && n_feat % 4 == 0 && max_dim <= 1024 && max_grp <= 64 &&
                  parts_fit && small_init() == 0;
-  h->use_umma = !h->use_small && tma_ok && !(cfg->flags & NNP_FLAG_NO_UMMA) && umma_init() == 0;
-  h->use_tma = !h->use_small && tma_ok && !h->use_umma;
+  h->use_umma = !h->use_small && box_ok && !(cfg->flags & NNP_FLAG_NO_UMMA) && umma_init() == 0;
   // at ligand sizes the layer-1 backward is split per model (every CTA streams its own slice of W1
   // exactly once); the M partial dE/dAEV rows are summed by the AEV backward kernel
-  h->n_parts = ((tma_ok || h->use_small) && parts_fit) ? M : 1;
+  h->n_parts = (h->use_small && parts_fit) ? M : 1;
 
   // ---- workspaces
   if (dev_alloc(&h->d_pos4, (size_t)N) || dev_alloc(&h->d_nbr_r, (size_t)N * h->capR) ||
@@ -401,82 +397,6 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     g.name = "mlp_bwd_l" + std::to_string(l);
     if (upload_launch(g, probs)) return fail(NNP_ERR_ALLOC);
     h->bwd.push_back(g);
-  }
-  if (h->use_tma) {
-    std::vector<int> slot(S, -1);
-    int ns = 0;
-    for (int e = 0; e < S; ++e)
-      if (h->grp_off[e + 1] > h->grp_off[e]) slot[e] = ns++;
-    for (int pass = 0; pass < 2; ++pass) {
-      for (int li = 0; li < L - 1; ++li) {
-        const int l = pass == 0 ? li + 1 : L - 1 - li;  // fwd: 1..L-1, bwd: L-1..1
-        std::vector<GemmProblem> probs;
-        std::vector<TmaOperand> aops(ns), bops(ns);
-        std::vector<TmaProbExtra> extra;
-        for (int e = 0; e < S; ++e) {
-          if (slot[e] < 0) continue;
-          const int ne = h->grp_off[e + 1] - h->grp_off[e];
-          const int nin = h->dims[e * (L + 1) + l - 1], nout = h->dims[e * (L + 1) + l];
-          const float* Wl = h->d_W + h->w_off[e * L + l - 1];
-          bops[slot[e]] = TmaOperand{Wl, (long long)M * nout, nin, nin};
-          if (pass == 0) {
-            if (l == 1) aops[slot[e]] = TmaOperand{h->d_aev + (size_t)h->grp_off[e] * n_feat, ne, n_feat, n_feat};
-            else aops[slot[e]] = TmaOperand{h->d_act[l - 1] + h->act_off[l - 1][e], ne, (long long)M * nin, (long long)M * nin};
-          } else {
-            aops[slot[e]] = TmaOperand{h->d_act[l] + h->act_off[l][e], ne, (long long)M * nout, (long long)M * nout};
-          }
-          const int n_prob = (pass == 1 && l == 1 && h->n_parts == 1) ? 1 : M;
-          for (int m = 0; m < n_prob; ++m) {
-            GemmProblem p;
-            memset(&p, 0, sizeof(p));
-            TmaProbExtra x;
-            x.amap = x.bmap = slot[e];
-            x.a_row0 = 0;
-            p.alpha = alpha;
-            p.inv_alpha = 1.0f / alpha;
-            p.M = ne;
-            if (pass == 0) {
-              p.transB = 0; p.N = nout; p.K = nin;
-              p.C = h->d_act[l] + h->act_off[l][e] + (size_t)m * nout;
-              p.ldc = M * nout;
-              p.bias = h->d_b + h->b_off[e * L + l - 1] + (size_t)m * nout;
-              p.epi = EPI_BIAS_CELU;
-              x.a_col0 = l == 1 ? 0 : m * nin;
-              x.b_row0 = m * nout;
-            } else if (l > 1) {
-              p.transB = 1; p.N = nin; p.K = nout;
-              p.C = h->d_act[l - 1] + h->act_off[l - 1][e] + (size_t)m * nin;
-              p.ldc = M * nin;
-              p.aux = p.C; p.ldaux = p.ldc;
-              p.epi = EPI_MUL_DCELU;
-              x.a_col0 = m * nout;
-              x.b_row0 = m * nout;
-            } else {
-              p.transB = 1; p.N = nin;
-              p.epi = EPI_SCALE;
-              p.scale = 1.0f / (float)M;
-              p.ldc = n_feat;
-              if (h->n_parts == 1) {
-                p.K = M * nout; x.a_col0 = 0; x.b_row0 = 0;
-                p.C = h->d_daev + (size_t)h->grp_off[e] * n_feat;
-              } else {
-                p.K = nout; x.a_col0 = m * nout; x.b_row0 = m * nout;
-                p.C = h->d_daev + ((size_t)m * N + h->grp_off[e]) * n_feat;
-              }
-            }
-            probs.push_back(p);
-            extra.push_back(x);
-          }
-        }
-        TmaLaunch tl;
-        tl.name = (pass == 0 ? "mlp_fwd_l" : "mlp_bwd_l") + std::to_string(l);
-        if (tma_build_launch(tl, probs, aops, bops, extra, prop.multiProcessorCount)) {
-          tma_free_launch(tl);
-          return fail(NNP_ERR_CUDA);
-        }
-        (pass == 0 ? h->tfwd : h->tbwd).push_back(tl);
-      }
-    }
   }
   // Structural zeros of the AEV: the radial block of species s and the angular blocks of pairs (s, t) are zero for
   // every atom when s (or t) does not occur in the system.  Layer 1 can skip the 32-wide contraction boxes that hold
@@ -788,7 +708,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       }
       SmallLaunch sl;
       sl.name = "mlp_bwd_l" + std::to_string(l);
-      if (bwd1 ? small_build_bwd1(sl, items, (cfg->flags & NNP_FLAG_BWD1_PERSISTENT) != 0, (cfg->flags & NNP_FLAG_NO_BWD1_PAIRS) == 0, wops) : small_build_bwd(sl, items)) { small_free_launch(sl); return fail(NNP_ERR_CUDA); }
+      if (bwd1 ? small_build_bwd1(sl, items, wops) : small_build_bwd(sl, items)) { small_free_launch(sl); return fail(NNP_ERR_CUDA); }
       h->sbwd.push_back(sl);
     }
   }
@@ -864,16 +784,12 @@ static void enqueue_chain(nnp_handle* h, const float* d_pos, int ps, const int* 
   }
   if (h->use_umma) {
     for (auto& g : h->ufwd) { umma_launch(g, s); mark(); }
-  } else if (h->use_tma) {
-    for (auto& g : h->tfwd) { tma_launch(g, s); mark(); }
   } else {
     for (auto& g : h->fwd) { launch_gemm(g, s); mark(); }
   }
   launch_last_layer(h, s); mark();
   if (h->use_umma) {
     for (auto& g : h->ubwd) { umma_launch(g, s); mark(); }
-  } else if (h->use_tma) {
-    for (auto& g : h->tbwd) { tma_launch(g, s); mark(); }
   } else {
     for (auto& g : h->bwd) { launch_gemm(g, s); mark(); }
   }
@@ -885,7 +801,11 @@ extern "C" int nnp_compute(nnp_handle* h, const float* d_pos, int32_t pos_stride
                            const int32_t* d_atom_index, double* d_energy, float* d_force_accum,
                            int32_t force_stride_floats, void* cuda_stream) {
   if (!h) return NNP_ERR_INVALID_ARG;
-  if (h->N == 0) return NNP_OK;
+  if (h->N == 0) {  // no atoms: every (empty) molecule has energy 0; d_energy is WRITTEN as documented
+    if (d_energy) CK(cudaMemsetAsync(d_energy, 0, sizeof(double) * (size_t)h->n_mol, (cudaStream_t)cuda_stream));
+    h->last_stream = (cudaStream_t)cuda_stream;
+    return NNP_OK;
+  }
   if (!d_pos || pos_stride_floats < 3 || (d_force_accum && force_stride_floats < 3)) return NNP_ERR_INVALID_ARG;
   cudaStream_t s = (cudaStream_t)cuda_stream;
   h->last_stream = s;
@@ -928,7 +848,10 @@ extern "C" int nnp_compute(nnp_handle* h, const float* d_pos, int32_t pos_stride
 extern "C" int nnp_compute_host(nnp_handle* h, const float* pos_host, double* energy_host, float* force_host,
                                 void* cuda_stream) {
   if (!h || (h->N > 0 && !pos_host)) return NNP_ERR_INVALID_ARG;
-  if (h->N == 0) return NNP_OK;
+  if (h->N == 0) {
+    if (energy_host) memset(energy_host, 0, sizeof(double) * (size_t)h->n_mol);
+    return NNP_OK;
+  }
   cudaStream_t s = (cudaStream_t)cuda_stream;
   CK(cudaMemcpyAsync(h->d_hpos, pos_host, sizeof(float) * 3 * (size_t)h->N, cudaMemcpyHostToDevice, s));
   CK(cudaMemsetAsync(h->d_hforce, 0, sizeof(float) * 3 * (size_t)h->N, s));

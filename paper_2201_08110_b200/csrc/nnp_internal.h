@@ -91,35 +91,11 @@ struct GemmLaunch {
   double flops = 0, weight_bytes = 0;
 };
 
-// ---- TMA engine (mlp_tma.cu)
-struct TmaTile {
-  int prob, m0, n0, ta;      // problem, first atom row / output column of the tile, tile height
-  int amap, bmap;            // tensor-map slots
-  int a_row0, a_col0;        // A box origin (row = atom, col = contraction)
-  int b_row0, b_col0;        // W box origin
-  int K, transB;             // contraction length, 0 = NT / 1 = NN (copied from the problem)
-  long long cost;
-};
+// a row-major f32 matrix [rows][cols] with pitch ld floats, as a TMA tensor-map operand
 struct TmaOperand {
   const float* base;
-  long long rows, cols, ld;  // row-major [rows][cols], pitch ld floats
+  long long rows, cols, ld;
 };
-struct TmaProbExtra {
-  int amap, bmap, a_row0, a_col0, b_row0;
-};
-struct TmaLaunch {
-  void* params = nullptr;  // TmaGemmParams (host copy, passed by value as __grid_constant__)
-  GemmProblem* d_probs = nullptr;
-  TmaTile* d_tiles = nullptr;
-  int n_tiles = 0, grid = 0;
-  size_t smem_bytes = 0;
-  std::string name;
-};
-int tma_init();
-int tma_build_launch(TmaLaunch& L, const std::vector<GemmProblem>& probs, const std::vector<TmaOperand>& aops,
-                     const std::vector<TmaOperand>& bops, const std::vector<TmaProbExtra>& extra, int num_sms);
-void tma_launch(const TmaLaunch& L, cudaStream_t s);
-void tma_free_launch(TmaLaunch& L);
 
 // ---- tcgen05 engine (mlp_umma.cu): D[f][a] = sum_k A[f][k] B[a][k], f = output feature, a = atom
 struct UmmaItem {            // one tile of one GEMM, as the persistent CTAs consume it
@@ -204,7 +180,7 @@ int small_init();
 void small_bwd_shape(int n_atoms, int* AW, int* G);
 int small_build_fwd(SmallLaunch& L, std::vector<SmallFwdItem>& items);
 int small_build_bwd(SmallLaunch& L, std::vector<SmallBwdItem>& items);
-int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items, bool persistent_ok, bool pairs_ok,
+int small_build_bwd1(SmallLaunch& L, std::vector<SmallBwdItem>& items,
                      const std::vector<TmaOperand>& wops);  // wops[tmap]: the [rows][cols] layer-1 weight block of an element
 int small_build_fwd1(SmallLaunch& L, std::vector<Fwd1Item>& items);
 int small_fwd1_tile_rows();  // layer 1: persistent, weights streamed through a ring  // layer 1: weights read once, FFMA2
@@ -291,11 +267,10 @@ struct nnp_handle {
   std::vector<long long> act_off[NNP_MAX_LAYERS];  // [S] float offsets
   // MLP launches
   std::vector<GemmLaunch> fwd, bwd;  // fwd: layers 1..L-1; bwd: layers L-1..1
-  std::vector<TmaLaunch> tfwd, tbwd; // the same launches on the TMA+FFMA engine (used when use_tma)
   std::vector<UmmaLaunch> ufwd, ubwd; // the same launches on the tcgen05 engine (used when use_umma)
   std::vector<SmallLaunch> sfwd, sbwd; // ligand-size engine (used when use_small); no separate last-layer launch
   SmallLaunch smid;                    // fused middle launch of the ligand-size engine (used when use_mid)
-  bool use_tma = false, use_umma = false, use_small = false, use_mid = false;
+  bool use_umma = false, use_small = false, use_mid = false;
   bool use_pdl = false, pdl_now = false;  // programmatic dependent launches along the chain (pdl_now: this enqueue)
   int n_parts = 1;                   // dE/dAEV is produced as n_parts partial sums (per model at small N)
   LastLayerArgs last;
