@@ -368,7 +368,7 @@ template <int NZ, int NA>
 __global__ void __launch_bounds__(AEV_THREADS, 6) aev_forward_kernel(
     const float4* __restrict__ pos4, const int* __restrict__ nbr_r, const int* __restrict__ nbr_a,
     const int* __restrict__ cnt_r, const int* __restrict__ cnt_a, const int* __restrict__ sortpos, int N,
-    const __grid_constant__ AevConst c, int capR, int capA, int CH, float* __restrict__ aev,
+    const __grid_constant__ AevConst c, int capR, int capA, int CH, float* __restrict__ aev, float* __restrict__ aev_lo,
     const __grid_constant__ NbrArgs nb, int fused, int mp_off4, float4* __restrict__ pos4_w, int* __restrict__ nbr_r_w,
     int* __restrict__ nbr_a_w, int* __restrict__ cnt_r_w, int* __restrict__ cnt_a_w) {
   extern __shared__ __align__(16) float smem[];
@@ -401,6 +401,9 @@ __global__ void __launch_bounds__(AEV_THREADS, 6) aev_forward_kernel(
   build_tab(t, i, nr, na, pi, pos4, fused ? nbr_r_w : nbr_r, fused ? nbr_a_w : nbr_a, capR, capA, c, true,
             fused ? mp : nullptr, mlo);
   float* out = aev + (size_t)sortpos[i] * c.n_feat;
+  // tensor engine: the row is written as two TF32-exact planes (hi = rna_tf32(G), lo = G - hi), the operand format of
+  // the 3xTF32 layer-1 GEMM
+  float* out_lo = aev_lo ? aev_lo + (size_t)sortpos[i] * c.n_feat : nullptr;
 
   // ---- radial (O3)
   for (int col = threadIdx.x; col < c.n_radial; col += blockDim.x) {
@@ -413,7 +416,13 @@ __global__ void __launch_bounds__(AEV_THREADS, 6) aev_forward_kernel(
       const float v = 0.25f * gauss(d, c.kr_hi, c.kr_lo) * t.fcr[q];
       acc += t.spec[q] == s ? v : 0.0f;
     }
-    out[col] = acc;
+    if (out_lo) {
+      const float hi = __uint_as_float((__float_as_uint(acc) + 0x1000u) & 0xFFFFE000u);
+      out[col] = hi;
+      out_lo[col] = acc - hi;
+    } else {
+      out[col] = acc;
+    }
   }
 
   // ---- angular (O4)
@@ -467,7 +476,16 @@ __global__ void __launch_bounds__(AEV_THREADS, 6) aev_forward_kernel(
     }
     __syncthreads();
   }
-  for (int f = threadIdx.x; f < n_ang; f += blockDim.x) out[c.n_radial + f] = row[f];
+  if (out_lo) {
+    for (int f = threadIdx.x; f < n_ang; f += blockDim.x) {
+      const float v = row[f];
+      const float hi = __uint_as_float((__float_as_uint(v) + 0x1000u) & 0xFFFFE000u);
+      out[c.n_radial + f] = hi;
+      out_lo[c.n_radial + f] = v - hi;
+    }
+  } else {
+    for (int f = threadIdx.x; f < n_ang; f += blockDim.x) out[c.n_radial + f] = row[f];
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -817,13 +835,13 @@ void launch_aev_forward(nnp_handle* h, const float* d_pos, int pos_stride, const
   if (aev_small_shape(h))
     launch_kernel(pdl, aev_forward_kernel<4, 8>, dim3(blocks), dim3(aev_block_threads(h, false)), smem, s, (const float4*)h->d_pos4,
                   (const int*)h->d_nbr_r, (const int*)h->d_nbr_a, (const int*)h->d_cnt_r, (const int*)h->d_cnt_a,
-                  (const int*)h->d_sortpos, h->N, h->aev, h->capR, h->capA, trip_chunk(h, false), h->d_aev, nb, fused,
+                  (const int*)h->d_sortpos, h->N, h->aev, h->capR, h->capA, trip_chunk(h, false), h->d_aev, h->d_aev_lo, nb, fused,
                   mp_off4, h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a);
   else
     launch_kernel(pdl, aev_forward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>, dim3(blocks), dim3(aev_block_threads(h, false)), smem, s,
                   (const float4*)h->d_pos4, (const int*)h->d_nbr_r, (const int*)h->d_nbr_a, (const int*)h->d_cnt_r,
                   (const int*)h->d_cnt_a, (const int*)h->d_sortpos, h->N, h->aev, h->capR, h->capA,
-                  trip_chunk(h, false), h->d_aev, nb, fused, mp_off4, h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r,
+                  trip_chunk(h, false), h->d_aev, h->d_aev_lo, nb, fused, mp_off4, h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r,
                   h->d_cnt_a);
 }
 

@@ -217,13 +217,22 @@ __global__ void __launch_bounds__(128) last_layer_kernel(const __grid_constant__
   int e = 0;
   while (e + 1 < a.S && row >= a.grp_off[e + 1]) ++e;
   const int H = a.H[e];
-  float* h = a.act + a.act_off[e] + ((size_t)(row - a.grp_off[e]) * a.M + m) * H;
+  const size_t hoff = a.act_off[e] + ((size_t)(row - a.grp_off[e]) * a.M + m) * H;
+  float* h = a.act + hoff;
+  float* hl = a.act_lo ? a.act_lo + hoff : nullptr;  // tensor engine: activations are stored split (hi, lo planes)
   const float* wv = a.W + a.w_off[e] + (size_t)m * H;
   double acc = 0.0;
   for (int o = lane; o < H; o += 32) {
-    const float hv = h[o], ww = wv[o];
+    const float hv = hl ? h[o] + hl[o] : h[o], ww = wv[o];  // hi + lo is exact
     acc += (double)ww * (double)hv;
-    h[o] = ww * dcelu_from_h(hv, a.alpha);
+    const float d = ww * dcelu_from_h(hv, a.alpha);
+    if (hl) {
+      const float dh = __uint_as_float((__float_as_uint(d) + 0x1000u) & 0xFFFFE000u);  // rna_tf32
+      h[o] = dh;
+      hl[o] = d - dh;
+    } else {
+      h[o] = d;
+    }
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);

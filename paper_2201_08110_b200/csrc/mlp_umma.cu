@@ -1,35 +1,29 @@
 // tcgen05 (5th-gen tensor core) GEMM engine for the per-element atomic MLPs (A4 forward, A6 backward).
 //
 // Mathematics: DESIGN.md O5/O7 -- the layer GEMMs  D[f][a] = sum_k W[f][k] X[a][k]  (forward, f = output
-// feature, a = atom) and  D[n][a] = sum_o W[o][n] delta[a][o]  (input-gradient backward).
+// feature, a = atom) and  D[n][a] = sum_o W[o][n] delta[a][o]  (input-gradient backward; the weights are kept
+// transposed for this pass, so both passes read K-major operands).
 //
-// Precision ("3xTF32, no tensor-core accumulation of the main term").  Measured on B200 (DESIGN.md
-// section 7): tcgen05 TRUNCATES FP32 inputs to TF32 and TRUNCATES when it adds into the FP32 accumulator,
-// so accumulating a long contraction in TMEM is biased towards zero (-6.5e-6 relative at K = 1024) and the
-// bias shows up as a coherent energy error.  Therefore
-//   * weights  w = hi + lo with hi = trunc_tf32(w) (what the tensor core makes of the raw FP32 box, so the
-//     TMA-written box is used as it is) and lo = rna_tf32(w - hi);
-//     activations x = hi + lo with hi = rna_tf32(x), lo = x - hi (random sign, so the dropped lo*lo term,
-//     <= 2^-21 relative, has no preferred sign);
-//   * the hi*hi products (exact: 11 x 11 bits) of every k-step (8 contraction elements) go into a FRESH
-//     TMEM slot; the drain warps add the slots in FP32 round-to-nearest registers (two-level for tiles of
-//     up to 64 atoms: 8 slots -> partial -> total);
-//   * lo*hi + hi*lo go into a second accumulator over the whole contraction (2^-10 of the result, so its
-//     truncation is irrelevant).
+// Precision ("3xTF32 from pre-split operands").  Every operand exists in global memory as two TF32-exact planes:
+//   weights      hi = rna_tf32(w), lo = rna_tf32(w - hi)           (split once in nnp_create)
+//   activations  hi = rna_tf32(x), lo = x - hi                     (written by the kernel that produces x)
+// and a product is  hi*hi + (lo*hi + hi*lo);  the dropped lo*lo term is <= 2^-22 relative with no preferred sign.
+// tcgen05 TRUNCATES when it adds into its FP32 accumulator (measured): a contraction
+// accumulated entirely in TMEM is biased towards zero.  Therefore the contraction is cut into SLOTS of `kps`
+// k-steps (8 contraction elements each): every slot starts a FRESH TMEM accumulator, receives its cross terms
+// first (2^-11 of the result: their truncation is irrelevant) and its hi*hi terms last, and the drain warps add
+// the finished slots in FP32 round-to-nearest registers.
 //
-// Structure: persistent CTAs (one per SM), 14 warps:
-//   warp 0      TMA producer      cp.async.bulk.tensor boxes [rows][32 floats] -> deep raw ring (full barriers)
-//   warp 1      MMA issuer        one thread issues tcgen05.mma kind::tf32 (M = 128, N = 16..128, K = 8)
-//   warps 2-5   converters        raw box -> lo parts in a short second ring (conv barriers)
-//   warps 6-13  drain + epilogue  tcgen05.ld of finished slot groups, FP32 adds, fused bias+CELU / CELU' /
-//                                  scale, coalesced stores (group_full / group_empty barriers)
-// The raw ring is what keeps HBM busy in the weight-streaming regime (ligand sizes): up to 8 x 16 KB of
-// weights in flight per SM.
-// Operand layouts: weights are read in their natural row-major layout in both passes -- forward as a
-// K-major operand (128-byte swizzle), backward as an MN-major operand (TF32 MN-major needs the
-// "128B swizzle, 32B atom" layout: CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B + UMMA layout type 1).
+// Structure: persistent CTAs (one per SM), 10 warps:
+//   warp 0      TMA producer   four boxes per stage: W hi/lo [128 rows][32 floats], X hi/lo [n_pad rows][32 floats]
+//   warp 1      MMA issuer     one thread: per slot 2*kps cross MMAs + kps main MMAs (kind::tf32, M = 128,
+//                              N = 16..128, K = 8), then tcgen05.commit to the slot's barrier; per stage a commit
+//                              that frees the operand ring entry
+//   warps 2-9   drain + epilogue   tcgen05.ld of finished slots, FP32 adds, fused bias+CELU / CELU' / scale; the
+//                              output is written split (hi, lo planes) when a tensor-engine launch consumes it
+// Slots are self-contained, so the ring of TMEM slots runs across item boundaries: the epilogue of item i overlaps
+// the MMAs of item i+1.  No shared-memory traffic other than TMA writes and tensor-core operand reads.
 #include <cuda.h>
-#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -38,13 +32,16 @@
 
 namespace {
 
-constexpr int U_THREADS = 448;
-constexpr int U_DRAIN_THREADS = 256;
+#ifndef U_ISSUERS
+#define U_ISSUERS 2
+#endif
+constexpr int U_DRAIN_THREADS = 256;     // 8 drain warps (two per TMEM lane quarter)
+constexpr int U_FIRST_DRAIN = 1 + U_ISSUERS;  // warp 0: TMA producer, then the MMA issuer warp(s), then the drain warps
+constexpr int U_THREADS = 32 * U_FIRST_DRAIN + U_DRAIN_THREADS;
 constexpr int BOXF = 32;                 // floats per box row (128 B)
-constexpr int A_BOX_BYTES = 128 * 128;   // weight box: 128 feature rows x 32 contraction floats
-constexpr int U_MAX_RAW = 10;            // raw ring depth (upper bound)
-constexpr int U_LO_STAGES = 2;           // lo ring depth
-constexpr int U_MAX_GROUPS = 8;
+constexpr int A_BOX_BYTES = 128 * 128;   // weight box: 128 feature rows x 32 contraction floats (one plane)
+constexpr int U_MAX_STAGES = 6;          // operand ring depth (upper bound)
+constexpr int U_MAX_SLOTS = 8;           // TMEM accumulator slots (upper bound)
 constexpr int L1_SLOTS = 8;              // two-level summation: slots per first-level partial sum
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -77,6 +74,19 @@ __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, i
       ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar))
       : "memory");
 }
+// warp-converged issue: every lane runs the role loop with warp-uniform values (so the compiler keeps descriptors and
+// addresses in uniform registers), one elected lane executes the asynchronous instructions
+__device__ __forceinline__ uint32_t elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred;
+}
+__device__ __forceinline__ void tma_load_2d_s(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+      ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar)
+      : "memory");
+}
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_commit(uint64_t* bar) {
@@ -98,19 +108,9 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo, uint
          ((uint64_t)((sbo >> 4) & 0x3FFF) << 32) | (1ull << 46) | ((uint64_t)layout << 61);
 }
 // round to TF32 (10 explicit mantissa bits), nearest, ties away from zero == cvt.rna.tf32.f32 for finite inputs,
-// done on the integer ALU (the conversion instruction runs at a fraction of the ALU rate and paced the converters)
+// done on the integer ALU
 __device__ __forceinline__ float tf32_rna(float x) {
   return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xFFFFE000u);
-}
-// weights: hi = trunc_tf32(w) is implicit (the tensor core truncates the raw value); lo = rna(w - hi)
-__device__ __forceinline__ float w_lo(float w) {
-  return tf32_rna(w - __uint_as_float(__float_as_uint(w) & 0xFFFFE000u));
-}
-__device__ __forceinline__ float4 w_lo4(const float4 v) { return make_float4(w_lo(v.x), w_lo(v.y), w_lo(v.z), w_lo(v.w)); }
-// activations: hi = rna(x), lo = x - hi
-__device__ __forceinline__ void x_split4(const float4 v, float4& h, float4& l) {
-  h.x = tf32_rna(v.x); h.y = tf32_rna(v.y); h.z = tf32_rna(v.z); h.w = tf32_rna(v.w);
-  l.x = v.x - h.x; l.y = v.y - h.y; l.z = v.z - h.z; l.w = v.w - h.w;
 }
 // CELU with the hardware exponential: alpha (2^(x log2e / alpha) - 1).  Near x = 0 the subtraction leaves an ABSOLUTE
 // error of ~2^-24 alpha = 6e-9 on an activation of order 0.1..1 (unbiased), far below the TF32-split error of the
@@ -122,9 +122,14 @@ __device__ __forceinline__ float celu_f(float x, float alpha, float inv_alpha) {
 }
 __device__ __forceinline__ float dcelu_from_h(float h, float inv_alpha) { return h > 0.0f ? 1.0f : fmaf(h, inv_alpha, 1.0f); }
 
-// acc[0..CNT-1] += CNT consecutive TMEM columns of this thread's lane (CNT = 8, 16 or 32)
+// acc[0..CNT-1] += CNT consecutive TMEM columns of this thread's lane (CNT = 8, 16 or 32).
+// comp = 1: every value read is first moved one ulp AWAY from zero.  tcgen05 truncates towards zero each time it adds
+// into its accumulator (measured: mean -0.27 ulp per accumulating k-step, -1.07 ulp over the 4 k-steps of a slot,
+// DESIGN.md section 7); adding the expected loss back removes the coherent shrink of every pre-activation, which
+// otherwise shows up as an energy bias of -4e-6 kcal/mol per atom.  An exact zero becomes the smallest denormal
+// (1.4e-45): harmless, and padding rows / columns are never stored.
 template <int CNT>
-__device__ __forceinline__ void tmem_add(uint32_t taddr, float* acc) {
+__device__ __forceinline__ void tmem_add(uint32_t taddr, float* acc, uint32_t comp) {
   uint32_t r[CNT];
   if constexpr (CNT == 8) {
     asm volatile(
@@ -155,42 +160,111 @@ __device__ __forceinline__ void tmem_add(uint32_t taddr, float* acc) {
         : "memory");
   }
 #pragma unroll
-  for (int j = 0; j < CNT; ++j) acc[j] += __uint_as_float(r[j]);
+  for (int j = 0; j < CNT; ++j) acc[j] += __uint_as_float(r[j] + comp);
 }
 // CT columns starting at taddr (CT = 8, 16, 32 or 64)
 template <int CT>
-__device__ __forceinline__ void tmem_add_cols(uint32_t taddr, float* acc) {
-  if constexpr (CT <= 32) {
-    tmem_add<CT>(taddr, acc);
-  } else {
+__device__ __forceinline__ void tmem_add_cols(uint32_t taddr, float* acc, uint32_t comp) {
+  if constexpr (CT <= 16) {
+    tmem_add<CT>(taddr, acc, comp);
+  } else {  // 16 columns at a time: the staging registers count against the 112 of a thread
 #pragma unroll
-    for (int g = 0; g < CT / 32; ++g) tmem_add<32>(taddr + 32 * g, acc + 32 * g);
+    for (int g = 0; g < CT / 16; ++g) tmem_add<16>(taddr + 16 * g, acc + 16 * g, comp);
   }
 }
 
 }  // namespace
 
 struct UmmaParams {
-  CUtensorMap amap[NNP_MAX_SPECIES];
-  CUtensorMap bmap[NNP_MAX_SPECIES];
+  CUtensorMap ahi[NNP_MAX_SPECIES], alo[NNP_MAX_SPECIES];  // weights of an element (hi / lo planes)
+  CUtensorMap bhi[NNP_MAX_SPECIES], blo[NNP_MAX_SPECIES];  // activations of an element
   const UmmaItem* items;
   const int* cta_off;  // [grid + 1] item range of every persistent CTA
-  int b_box_bytes;     // largest activation box of the launch (n_pad_max * 128)
-  int stage_bytes;     // A_BOX_BYTES + b_box_bytes (raw and lo stages have the same layout)
-  int n_raw;           // raw ring depth
-  int slot_cols;       // TMEM columns per accumulator slot (= n_pad_max); cross accumulator at column 0
-  int kps;             // k-steps (8 contraction elements each) accumulated in TMEM per slot: 1 or 4
-  int gslots;          // slots per group = commit / drain granularity
-  int n_groups;        // slot-group ring depth
+  int b_box_bytes;     // largest activation box of the launch (n_pad_max * 128), one plane
+  int stage_bytes;     // 2 * A_BOX_BYTES + 2 * b_box_bytes
+  int n_stages;        // operand ring depth
+  int staging_rows;    // atoms per epilogue round = rows of the staging tile (min(n_pad_max, 64))
+  int slot_cols;       // TMEM columns per accumulator slot (= n_pad_max)
+  int n_slots;         // TMEM slot ring depth: 4 or 8
+  int slot_shift;      // log2(n_slots)
+  int comp;            // 1: add the expected truncation loss of a slot (one ulp away from zero, see tmem_add) back
 };
 
+__device__ __forceinline__ float4 ld4(const float* p) { return *reinterpret_cast<const float4*>(p); }
+__device__ __forceinline__ void st4(float* p, const float4 v) { *reinterpret_cast<float4*>(p) = v; }
+__device__ __forceinline__ void split4(const float4 v, float4& h, float4& l) {
+  h.x = tf32_rna(v.x); h.y = tf32_rna(v.y); h.z = tf32_rna(v.z); h.w = tf32_rna(v.w);
+  l.x = v.x - h.x; l.y = v.y - h.y; l.z = v.z - h.z; l.w = v.w - h.w;
+}
+__device__ __forceinline__ void drain_sync() { asm volatile("bar.sync 1, %0;" ::"n"(U_DRAIN_THREADS) : "memory"); }
+
+// epilogue of `na` atoms (rows of the staging tile [atom][128 features]) by the 256 drain threads: bias + CELU /
+// x CELU' / scale, four consecutive features of one atom per thread and step (16-byte loads and stores), four steps
+// in flight.  Global row of staging row r is a0 + r.
+__device__ __forceinline__ void epilogue_rows(const UmmaItem& t, const float* staging, int a0, int na, int dt) {
+  constexpr int U = 4;
+  const int n_vec = na * 32;
+  const int g = dt & 31;          // the thread's feature group is the same in every step (256 % 32 == 0)
+  if (4 * g >= t.f_valid) return;
+  float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (t.epi == EPI_BIAS_CELU && t.bias) b = ld4(t.bias + 4 * g);
+  for (int base = dt; base < n_vec; base += U * U_DRAIN_THREADS) {
+    float4 v[U], d[U];
+    bool ok[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int idx = base + u * U_DRAIN_THREADS;
+      ok[u] = idx < n_vec;
+      const int r = idx >> 5;
+      v[u] = ok[u] ? ld4(staging + r * 128 + 4 * g) : make_float4(0.f, 0.f, 0.f, 0.f);
+      if (t.epi == EPI_MUL_DCELU) {  // h of the layer below (hi + lo is exact), for CELU'
+        d[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (ok[u]) {
+          const size_t o = (size_t)(a0 + r) * t.ldaux + 4 * g;
+          d[u] = ld4(t.aux + o);
+          if (t.aux_lo) {
+            const float4 l = ld4(t.aux_lo + o);
+            d[u].x += l.x; d[u].y += l.y; d[u].z += l.z; d[u].w += l.w;
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      if (!ok[u]) continue;
+      const int r = (base + u * U_DRAIN_THREADS) >> 5;
+      float4 x = v[u];
+      if (t.epi == EPI_BIAS_CELU) {
+        x.x = celu_f(x.x + b.x, t.alpha, t.inv_alpha); x.y = celu_f(x.y + b.y, t.alpha, t.inv_alpha);
+        x.z = celu_f(x.z + b.z, t.alpha, t.inv_alpha); x.w = celu_f(x.w + b.w, t.alpha, t.inv_alpha);
+      } else if (t.epi == EPI_MUL_DCELU) {
+        x.x *= dcelu_from_h(d[u].x, t.inv_alpha); x.y *= dcelu_from_h(d[u].y, t.inv_alpha);
+        x.z *= dcelu_from_h(d[u].z, t.inv_alpha); x.w *= dcelu_from_h(d[u].w, t.inv_alpha);
+      } else {
+        x.x *= t.scale; x.y *= t.scale; x.z *= t.scale; x.w *= t.scale;
+      }
+      const size_t o = (size_t)(a0 + r) * t.ldc + 4 * g;
+      if (t.C_lo) {
+        float4 h, l;
+        split4(x, h, l);
+        st4(t.C + o, h);
+        st4(t.C_lo + o, l);
+      } else {
+        st4(t.C + o, x);
+      }
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
-// drain + epilogue of one item: this thread owns feature row (TMEM lane) `quarter*32 + lane` and the
-// atom columns [half*CT, half*CT + CT) of the tile.
+// drain + epilogue of one item: this thread owns feature row (TMEM lane) `quarter*32 + lane` and the atom columns
+// [half*CT, half*CT + CT) of the tile; it adds the item's slots in FP32 registers.  The totals then go through a
+// shared-memory staging tile [64 atoms][128 features] (one half of the tile at a time), which transposes them for
+// an epilogue with 16-byte global accesses by all drain threads.
 template <int NP>
-__device__ __forceinline__ void drain_item(const UmmaItem& t, const UmmaParams& P, uint32_t tmem, uint64_t* group_full,
-                                           uint64_t* group_empty, uint64_t* cross_empty, uint32_t& grp, uint32_t& gphase,
-                                           int quarter, int half, int lane) {
+__device__ __forceinline__ void drain_item(const UmmaItem& t, const UmmaParams& P, uint32_t tmem, uint64_t* slot_full,
+                                           uint64_t* slot_empty, float* staging, uint32_t slot_ctr, int quarter, int half,
+                                           int lane, int dt) {
   constexpr int CT = NP >= 32 ? NP / 2 : NP;       // columns per thread
   constexpr bool TWO_LEVEL = NP <= 64;
   const bool active = NP >= 32 || half == 0;
@@ -203,101 +277,80 @@ __device__ __forceinline__ void drain_item(const UmmaItem& t, const UmmaParams& 
 #pragma unroll
     for (int j = 0; j < CT; ++j) part[j] = 0.0f;
   }
-  int ks_left = ((t.kb1 - t.kb0) * 4 + P.kps - 1) / P.kps;  // slots of this item
   const uint32_t lane_base = tmem + ((uint32_t)(quarter * 32) << 16) + (uint32_t)col0;
+  const uint32_t slot_mask = (uint32_t)P.n_slots - 1u, slot_shift = (uint32_t)P.slot_shift;
+  if (t.epi == EPI_MUL_DCELU) {
+    // the epilogue reads h of the layer below (written several launches ago, usually no longer in L2): start those
+    // lines towards L2 now, while the tile is being accumulated, with the addresses epilogue_rows will use
+    const int g = dt & 31;
+    if (4 * g < t.f_valid)
+      for (int r = dt >> 5; r < t.n_valid; r += U_DRAIN_THREADS / 32) {
+        const size_t o = (size_t)r * t.ldaux + 4 * g;
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(t.aux + o));
+        if (t.aux_lo) asm volatile("prefetch.global.L2 [%0];" ::"l"(t.aux_lo + o));
+      }
+  }
   int in_part = 0;
-  while (ks_left > 0) {
-    const int ns = min(P.gslots, ks_left);
-    mbar_wait(&group_full[grp], gphase);
+  for (int q = 0; q < t.nkb; ++q, ++slot_ctr) {
+    const uint32_t slot = slot_ctr & slot_mask, sphase = (slot_ctr >> slot_shift) & 1u;
+    mbar_wait(&slot_full[slot], sphase);
     tc_fence_after();
     if (active) {
-      const uint32_t src = lane_base + (uint32_t)P.slot_cols * (1u + grp * (uint32_t)P.gslots);
-      for (int q = 0; q < ns; ++q) {
-        if constexpr (TWO_LEVEL) {
-          tmem_add_cols<CT>(src + (uint32_t)(q * P.slot_cols), part);
-          if (++in_part == L1_SLOTS) {
+      const uint32_t src = lane_base + (uint32_t)P.slot_cols * slot;
+      if constexpr (TWO_LEVEL) {
+        tmem_add_cols<CT>(src, part, (uint32_t)P.comp);
+        if (++in_part == L1_SLOTS) {
 #pragma unroll
-            for (int j = 0; j < CT; ++j) { tot[j] += part[j]; part[j] = 0.0f; }
-            in_part = 0;
-          }
-        } else {
-          tmem_add_cols<CT>(src + (uint32_t)(q * P.slot_cols), tot);
+          for (int j = 0; j < CT; ++j) { tot[j] += part[j]; part[j] = 0.0f; }
+          in_part = 0;
         }
+      } else {
+        tmem_add_cols<CT>(src, tot, (uint32_t)P.comp);
       }
     }
     tc_fence_before();
-    mbar_arrive(&group_empty[grp]);
-    if (++grp == (uint32_t)P.n_groups) { grp = 0; gphase ^= 1u; }
-    ks_left -= ns;
+    mbar_arrive(&slot_empty[slot]);
   }
   if constexpr (TWO_LEVEL) {
 #pragma unroll
     for (int j = 0; j < CT; ++j) tot[j] += part[j];
   }
-  // cross terms (complete: the commit of the last group tracks every earlier MMA of the issuing thread)
-  if (active) tmem_add_cols<CT>(lane_base, tot);
-  tc_fence_before();
-  mbar_arrive(cross_empty);
-  // ---- epilogue
-  const int f = quarter * 32 + lane;
-  if (active && f < t.f_valid) {
-    float* C = t.C + (size_t)col0 * t.ldc + f;
-    const int nv = t.n_valid - col0;
-    if (t.epi == EPI_BIAS_CELU) {
-      const float b = t.bias ? t.bias[f] : 0.0f;
+  // ---- epilogue, one half of the tile per round
+  constexpr int ROUNDS = NP >= 32 ? 2 : 1;
 #pragma unroll
-      for (int j = 0; j < CT; ++j)
-        if (j < nv) C[(size_t)j * t.ldc] = celu_f(tot[j] + b, t.alpha, t.inv_alpha);
-    } else if (t.epi == EPI_MUL_DCELU) {
-      // aux may alias C (delta overwrites the activation in place): read every activation of this thread first, so
-      // the loads are independent and in flight together instead of being ordered behind the stores
-      const float* aux = t.aux + (size_t)col0 * t.ldaux + f;
-      constexpr int HB = CT < 16 ? CT : 16;  // batch size: enough loads in flight, no register spills
+  for (int h = 0; h < ROUNDS; ++h) {
+    if (active && half == h) {
+      float* dst = staging + quarter * 32 + lane;
 #pragma unroll
-      for (int j0 = 0; j0 < CT; j0 += HB) {
-        float hv[HB];
-#pragma unroll
-        for (int j = 0; j < HB; ++j) hv[j] = j0 + j < nv ? aux[(size_t)(j0 + j) * t.ldaux] : 0.0f;
-#pragma unroll
-        for (int j = 0; j < HB; ++j)
-          if (j0 + j < nv) C[(size_t)(j0 + j) * t.ldc] = tot[j0 + j] * dcelu_from_h(hv[j], t.inv_alpha);
-      }
-    } else {
-#pragma unroll
-      for (int j = 0; j < CT; ++j)
-        if (j < nv) C[(size_t)j * t.ldc] = tot[j] * t.scale;
+      for (int j = 0; j < CT; ++j) dst[j * 128] = tot[j];
     }
+    drain_sync();
+    const int na = min(CT, t.n_valid - h * CT);
+    if (na > 0) epilogue_rows(t, staging, h * CT, na, dt);
+    drain_sync();
   }
 }
 
 __global__ void __launch_bounds__(U_THREADS, 1) gemm_umma_kernel(const __grid_constant__ UmmaParams P) {
   extern __shared__ __align__(1024) unsigned char smem_dyn[];
-  unsigned char* raw = smem_dyn + ((1024u - (smem_u32(smem_dyn) & 1023u)) & 1023u);
-  unsigned char* los = raw + (size_t)P.n_raw * P.stage_bytes;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(los + (size_t)U_LO_STAGES * P.stage_bytes);
-  uint64_t* full = bars;                              // [U_MAX_RAW]   TMA landed
-  uint64_t* raw_empty = full + U_MAX_RAW;             // [U_MAX_RAW]   MMAs that read the raw stage are done
-  uint64_t* conv = raw_empty + U_MAX_RAW;             // [U_LO_STAGES] lo parts written
-  uint64_t* lo_empty = conv + U_LO_STAGES;            // [U_LO_STAGES]
-  uint64_t* group_full = lo_empty + U_LO_STAGES;      // [U_MAX_GROUPS]
-  uint64_t* group_empty = group_full + U_MAX_GROUPS;  // [U_MAX_GROUPS]
-  uint64_t* cross_empty = group_empty + U_MAX_GROUPS; // [1]
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(cross_empty + 1);
+  unsigned char* ring = smem_dyn + ((1024u - (smem_u32(smem_dyn) & 1023u)) & 1023u);
+  float* staging = reinterpret_cast<float*>(ring + (size_t)P.n_stages * P.stage_bytes);  // [<= 64 atoms][128]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(staging + (size_t)P.staging_rows * 128);
+  uint64_t* full = bars;                            // [U_MAX_STAGES] TMA landed
+  uint64_t* empty = full + U_MAX_STAGES;            // [U_MAX_STAGES] MMAs that read the stage are done
+  uint64_t* slot_full = empty + U_MAX_STAGES;       // [U_MAX_SLOTS]  slot accumulated
+  uint64_t* slot_empty = slot_full + U_MAX_SLOTS;   // [U_MAX_SLOTS]  slot drained
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(slot_empty + U_MAX_SLOTS);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
-    for (int s = 0; s < P.n_raw; ++s) {
+    for (int s = 0; s < P.n_stages; ++s) {
       mbar_init(&full[s], 1);
-      mbar_init(&raw_empty[s], 1);
+      mbar_init(&empty[s], U_ISSUERS);
     }
-    for (int s = 0; s < U_LO_STAGES; ++s) {
-      mbar_init(&conv[s], 128);
-      mbar_init(&lo_empty[s], 1);
+    for (int g = 0; g < P.n_slots; ++g) {
+      mbar_init(&slot_full[g], 1);
+      mbar_init(&slot_empty[g], U_DRAIN_THREADS);
     }
-    for (int g = 0; g < P.n_groups; ++g) {
-      mbar_init(&group_full[g], 1);
-      mbar_init(&group_empty[g], U_DRAIN_THREADS);
-    }
-    mbar_init(cross_empty, U_DRAIN_THREADS);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
@@ -309,145 +362,117 @@ __global__ void __launch_bounds__(U_THREADS, 1) gemm_umma_kernel(const __grid_co
   tc_fence_after();
   const uint32_t tmem = *tmem_slot;
   const int it0 = P.cta_off[blockIdx.x], it1 = P.cta_off[blockIdx.x + 1];
+  const uint32_t slot_mask = (uint32_t)P.n_slots - 1u, slot_shift = (uint32_t)P.slot_shift;
+  pdl_trigger();
+  pdl_wait();  // operands come from the previous kernel of the chain
 
   if (warp == 0) {
-    // ------------------------------------------------------------ TMA producer
-    if (lane == 0) {
-      uint32_t rs = 0, rphase = 0;
-      for (int it = it0; it < it1; ++it) {
-        const UmmaItem& t = P.items[it];
-        const CUtensorMap* am = &P.amap[t.amap];
-        const CUtensorMap* bm = &P.bmap[t.bmap];
-        const int a_mn = t.a_mn, a_c0 = t.a_c0, a_c1 = t.a_c1, b_c0 = t.b_c0, b_c1 = t.b_c1, kb1 = t.kb1;
-        const uint32_t tx = A_BOX_BYTES + (uint32_t)t.n_pad * 128u;
-        unsigned long long live = t.kmask;
-        for (int kbi = t.kb0; kbi < kb1; ++kbi) {
-          int kb = kbi;
-          if (live) {  // skip the contraction boxes that only hold structural zeros
-            kb = __ffsll((long long)live) - 1;
-            live &= live - 1;
-          }
-          mbar_wait(&raw_empty[rs], rphase ^ 1);
-          unsigned char* sa = raw + (size_t)rs * P.stage_bytes;
-          unsigned char* sb = sa + A_BOX_BYTES;
-          mbar_expect_tx(&full[rs], tx);
-          if (!a_mn) {
-            tma_load_2d(sa, am, a_c0 + kb * BOXF, a_c1, &full[rs]);
-          } else {
-#pragma unroll
-            for (int q = 0; q < 4; ++q) tma_load_2d(sa + q * 4096, am, a_c0 + q * BOXF, a_c1 + kb * BOXF, &full[rs]);
-          }
-          tma_load_2d(sb, bm, b_c0 + kb * BOXF, b_c1, &full[rs]);
-          if (++rs == (uint32_t)P.n_raw) { rs = 0; rphase ^= 1; }
-        }
-      }
-    }
-  } else if (warp == 1) {
-    // ------------------------------------------------------------ MMA issuer
-    // One thread; its instruction stream is the critical path of the CTA (every instruction of a single thread
-    // costs its full latency), so everything loop-invariant lives in registers and the four shared-memory
-    // descriptors of a box are formed once and advanced by an integer add per k-step.
-    if (lane == 0) {
-      uint32_t rs = 0, ls = 0, lphase = 0, grp = 0, gphase = 0, item_ctr = 0;
-      const uint32_t d_x = tmem;
-      const uint32_t n_raw = (uint32_t)P.n_raw, n_groups = (uint32_t)P.n_groups, gslots = (uint32_t)P.gslots,
-                     kps = (uint32_t)P.kps, slot_cols = (uint32_t)P.slot_cols, stage_bytes = (uint32_t)P.stage_bytes;
-      const uint32_t raw0 = smem_u32(raw), lo0 = smem_u32(los);
-      // descriptor templates (address field zero): K-major 128B swizzle / MN-major 128B swizzle with 32B atoms
-      const uint64_t desc_k = smem_desc(0, 16, 1024, 2), desc_mn = smem_desc(0, 4096, 512, 1);
-      uint32_t d_hi = tmem + slot_cols;  // slot (grp 0, in_group 0)
-      for (int it = it0; it < it1; ++it) {
-        const UmmaItem& t = P.items[it];
-        const int a_mn = t.a_mn, nb = t.kb1 - t.kb0;
-        const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)a_mn << 15) |
-                               ((uint32_t)(t.n_pad >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-        const uint64_t desc_a = a_mn ? desc_mn : desc_k;
-        const uint32_t a_step = a_mn ? (1024u >> 4) : (32u >> 4);  // descriptor address units (16 B) per k-step
-        mbar_wait(cross_empty, (item_ctr & 1u) ^ 1u);
-        uint32_t in_group = 0, in_slot = 0, ks_left = (uint32_t)nb * 4u, first = 1u;
-        for (int b = 0; b < nb; ++b) {
-          mbar_wait(&conv[ls], lphase);  // lo parts written (and, transitively, the raw stage has landed)
-          tc_fence_after();
-          const uint32_t sa = (raw0 + rs * stage_bytes) >> 4, sal = (lo0 + ls * stage_bytes) >> 4;
-          uint64_t ah = desc_a | sa, al = desc_a | sal;
-          uint64_t bh = desc_k | (sa + (A_BOX_BYTES >> 4)), bl = desc_k | (sal + (A_BOX_BYTES >> 4));
-#pragma unroll
-          for (int ks = 0; ks < 4; ++ks) {
-            if ((in_group | in_slot) == 0) {
-              mbar_wait(&group_empty[grp], gphase ^ 1u);
-              tc_fence_after();
-            }
-            mma_tf32(d_x, al, bh, idesc, first ^ 1u);
-            mma_tf32(d_x, ah, bl, idesc, 1u);
-            mma_tf32(d_hi, ah, bh, idesc, in_slot);
-            first = 0u;
-            ah += a_step; al += a_step; bh += 2; bl += 2;
-            --ks_left;
-            if (++in_slot == kps || ks_left == 0) {
-              in_slot = 0;
-              d_hi += slot_cols;
-              if (++in_group == gslots || ks_left == 0) {
-                tc_commit(&group_full[grp]);
-                in_group = 0;
-                if (++grp == n_groups) { grp = 0; gphase ^= 1u; }
-                d_hi = tmem + slot_cols * (1u + grp * gslots);
-              }
-            }
-          }
-          tc_commit(&raw_empty[rs]);  // frees the stages when these MMAs have read them
-          tc_commit(&lo_empty[ls]);
-          if (++rs == n_raw) rs = 0;
-          if (++ls == U_LO_STAGES) { ls = 0; lphase ^= 1u; }
-        }
-        ++item_ctr;
-      }
-    }
-  } else if (warp < 6) {
-    // ------------------------------------------------------------ converters
-    const int ct = threadIdx.x - 64;
-    uint32_t rs = 0, rphase = 0, ls = 0, lphase = 0;
+    // ------------------------------------------------------------ TMA producer (warp-converged, one lane issues)
+    const uint32_t leader = elect_one();
+    uint32_t rs = 0, rphase = 0;
+    const uint32_t ring0 = __shfl_sync(0xffffffffu, smem_u32(ring), 0);
     for (int it = it0; it < it1; ++it) {
       const UmmaItem& t = P.items[it];
-      const int nbv = t.n_pad * 8;  // float4 count of the activation box
-      const int nb = t.kb1 - t.kb0;
-      for (int b = 0; b < nb; ++b) {
-        mbar_wait(&lo_empty[ls], lphase ^ 1u);
-        mbar_wait(&full[rs], rphase);
-        unsigned char* sa = raw + (size_t)rs * P.stage_bytes;
-        unsigned char* sl = los + (size_t)ls * P.stage_bytes;
-        const float4* aw = reinterpret_cast<const float4*>(sa);
-        float4* al = reinterpret_cast<float4*>(sl);
-        float4* bh = reinterpret_cast<float4*>(sa + A_BOX_BYTES);
-        float4* bl = reinterpret_cast<float4*>(sl + A_BOX_BYTES);
+      const int amap = __shfl_sync(0xffffffffu, t.amap, 0), bmap = __shfl_sync(0xffffffffu, t.bmap, 0);
+      const CUtensorMap* ah = &P.ahi[amap];
+      const CUtensorMap* al = &P.alo[amap];
+      const CUtensorMap* bh = &P.bhi[bmap];
+      const CUtensorMap* bl = &P.blo[bmap];
+      const int a_c0 = __shfl_sync(0xffffffffu, t.a_c0, 0), a_c1 = __shfl_sync(0xffffffffu, t.a_c1, 0),
+                b_c0 = __shfl_sync(0xffffffffu, t.b_c0, 0), b_c1 = __shfl_sync(0xffffffffu, t.b_c1, 0),
+                nkb = __shfl_sync(0xffffffffu, t.nkb, 0);
+      const uint32_t tx = 2u * A_BOX_BYTES + 2u * (uint32_t)__shfl_sync(0xffffffffu, t.n_pad, 0) * 128u;
+      unsigned long long live = __shfl_sync(0xffffffffu, t.kmask, 0);
+      for (int kbi = 0; kbi < nkb; ++kbi) {
+        int kb = kbi;
+        if (live) {  // skip the contraction boxes that only hold structural zeros
+          kb = __ffsll((long long)live) - 1;
+          live &= live - 1;
+        }
+        mbar_wait(&empty[rs], rphase ^ 1u);
+        if (leader) {
+          const uint32_t sa = ring0 + rs * (uint32_t)P.stage_bytes;
+          const uint32_t sb = sa + 2 * A_BOX_BYTES;
+          const uint32_t bar = smem_u32(&full[rs]);
+          asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(tx) : "memory");
+          tma_load_2d_s(sa, ah, a_c0 + kb * BOXF, a_c1, bar);
+          tma_load_2d_s(sb, bh, b_c0 + kb * BOXF, b_c1, bar);
+          tma_load_2d_s(sa + A_BOX_BYTES, al, a_c0 + kb * BOXF, a_c1, bar);
+          tma_load_2d_s(sb + (uint32_t)P.b_box_bytes, bl, b_c0 + kb * BOXF, b_c1, bar);
+        }
+        __syncwarp();
+        if (++rs == (uint32_t)P.n_stages) { rs = 0; rphase ^= 1u; }
+      }
+    }
+  } else if (warp < U_FIRST_DRAIN) {
+    // ------------------------------------------------------------ MMA issuer warp(s); two of them alternate boxes
+    // A warp runs this loop converged; every value it uses is warp-uniform (kernel parameters, loop counters,
+    // broadcasts of the item fields), so descriptors and addresses live in uniform registers and the tcgen05
+    // instructions of the elected lane issue back to back.  (Under `if (lane == 0)` the compiler cannot prove
+    // uniformity and wraps every MMA in a register-to-uniform broadcast loop: ~200 cycles per MMA, measured.)
+    // The barrier round trips of a box (operands landed, slot drained, two commits: ~600 cycles, measured) would
+    // leave the tensor pipe idle between boxes if one warp did them all; boxes are independent (each fills a fresh
+    // TMEM slot), so two warps take them in turn and one waits while the other issues.  The slot ring has an even
+    // depth (a slot barrier is always waited on by the same warp); the stage ring may be odd, so both warps wait on
+    // the "landed" barrier of every box (a parity wait cannot tell phase k from phase k - 2) and a stage is refilled
+    // only after both have seen it.
+    const uint32_t me = (uint32_t)(warp - 1);
+    const uint32_t leader = elect_one();
+    uint32_t box = 0, rs = 0, rphase = 0;
+    const uint32_t n_stages = (uint32_t)P.n_stages;
+    const uint32_t slot_cols = (uint32_t)P.slot_cols, stage_bytes = (uint32_t)P.stage_bytes, b_box = (uint32_t)P.b_box_bytes;
+    const uint32_t ring0 = __shfl_sync(0xffffffffu, smem_u32(ring), 0);
+    const uint32_t tmem_u = __shfl_sync(0xffffffffu, tmem, 0);
+    const uint64_t desc_k = smem_desc(0, 16, 1024, 2);  // K-major, 128-byte swizzle (address field zero)
+    for (int it = it0; it < it1; ++it) {
+      const int nb = __shfl_sync(0xffffffffu, P.items[it].nkb, 0);
+      const uint32_t n_pad = (uint32_t)__shfl_sync(0xffffffffu, P.items[it].n_pad, 0);
+      const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((n_pad >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+      for (int b = 0; b < nb; ++b, ++box) {
+        const uint32_t my_rs = rs, my_phase = rphase;
+        if (++rs == n_stages) { rs = 0; rphase ^= 1u; }
+        mbar_wait(&full[my_rs], my_phase);  // every box: a warp must see every phase of a barrier it waits on
+        if (U_ISSUERS == 2 && (box & 1u) != me) {
+          // the other warp's box: having seen it land, let the producer refill the stage (it needs both warps'
+          // arrivals, so neither can be lapped on this barrier -- a lapped parity wait would never return)
+          if (leader) mbar_arrive(&empty[my_rs]);
+          __syncwarp();
+          continue;
+        }
+        const uint32_t slot = box & slot_mask, sphase = (box >> slot_shift) & 1u;
+        mbar_wait(&slot_empty[slot], sphase ^ 1u);
+        tc_fence_after();
+        const uint32_t sa = (ring0 + my_rs * stage_bytes) >> 4;
+        const uint64_t ah = desc_k | sa, al = desc_k | (sa + (A_BOX_BYTES >> 4));
+        const uint64_t bh = desc_k | (sa + (2 * A_BOX_BYTES >> 4)), bl = desc_k | (sa + ((2 * A_BOX_BYTES + b_box) >> 4));
+        const uint32_t d = tmem_u + slot_cols * slot;
+        if (leader) {
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-          const int idx = ct + 128 * i;
-          al[idx] = w_lo4(aw[idx]);
+          for (uint32_t ks = 0; ks < 4; ++ks) {  // cross terms first: a fresh accumulator
+            mma_tf32(d, al + 2 * ks, bh + 2 * ks, idesc, ks != 0);
+            mma_tf32(d, ah + 2 * ks, bl + 2 * ks, idesc, 1u);
+          }
+#pragma unroll
+          for (uint32_t ks = 0; ks < 4; ++ks) mma_tf32(d, ah + 2 * ks, bh + 2 * ks, idesc, 1u);
+          tc_commit(&slot_full[slot]);
+          tc_commit(&empty[my_rs]);  // frees the stage when these MMAs have read it
         }
-        for (int idx = ct; idx < nbv; idx += 128) {
-          float4 h, l;
-          x_split4(bh[idx], h, l);
-          bh[idx] = h;
-          bl[idx] = l;
-        }
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        mbar_arrive(&conv[ls]);
-        if (++rs == (uint32_t)P.n_raw) { rs = 0; rphase ^= 1u; }
-        if (++ls == U_LO_STAGES) { ls = 0; lphase ^= 1u; }
+        __syncwarp();
       }
     }
   } else {
-    // ------------------------------------------------------------ drain + epilogue (TMEM lane quarter = warp % 4)
-    const int quarter = warp & 3, half = (warp - 6) >> 2;
-    uint32_t grp = 0, gphase = 0;
+    // ------------------------------------------------------------ drain + epilogue (8 warps; TMEM lane quarter = warp % 4)
+    const int quarter = warp & 3, half = (warp - U_FIRST_DRAIN) >> 2, dt = threadIdx.x - 32 * U_FIRST_DRAIN;
+    uint32_t slot_ctr = 0;
     for (int it = it0; it < it1; ++it) {
       const UmmaItem t = P.items[it];
       switch (t.n_pad) {
-        case 16: drain_item<16>(t, P, tmem, group_full, group_empty, cross_empty, grp, gphase, quarter, half, lane); break;
-        case 32: drain_item<32>(t, P, tmem, group_full, group_empty, cross_empty, grp, gphase, quarter, half, lane); break;
-        case 64: drain_item<64>(t, P, tmem, group_full, group_empty, cross_empty, grp, gphase, quarter, half, lane); break;
-        default: drain_item<128>(t, P, tmem, group_full, group_empty, cross_empty, grp, gphase, quarter, half, lane); break;
+        case 16: drain_item<16>(t, P, tmem, slot_full, slot_empty, staging, slot_ctr, quarter, half, lane, dt); break;
+        case 32: drain_item<32>(t, P, tmem, slot_full, slot_empty, staging, slot_ctr, quarter, half, lane, dt); break;
+        case 64: drain_item<64>(t, P, tmem, slot_full, slot_empty, staging, slot_ctr, quarter, half, lane, dt); break;
+        default: drain_item<128>(t, P, tmem, slot_full, slot_empty, staging, slot_ctr, quarter, half, lane, dt); break;
       }
+      slot_ctr += (uint32_t)t.nkb;
     }
   }
   tc_fence_before();
@@ -474,9 +499,8 @@ static EncodeTiledFn get_encode() {
   return fn;
 }
 
-// 2-D f32 tensor [rows][cols], row pitch ld floats; box = [box_rows][32 floats]
-static int encode_map(CUtensorMap* m, const float* base, long long rows, long long cols, long long ld, int box_rows,
-                      CUtensorMapSwizzle swz) {
+// 2-D f32 tensor [rows][cols], row pitch ld floats; box = [box_rows][32 floats], 128-byte swizzle
+static int encode_map(CUtensorMap* m, const float* base, long long rows, long long cols, long long ld, int box_rows) {
   EncodeTiledFn enc = get_encode();
   if (!enc) return -1;
   if (rows <= 0) rows = 1;
@@ -485,44 +509,47 @@ static int encode_map(CUtensorMap* m, const float* base, long long rows, long lo
   cuuint32_t box[2] = {(cuuint32_t)BOXF, (cuuint32_t)box_rows};
   cuuint32_t estr[2] = {1, 1};
   CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)base, gdim, gstr, box, estr,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, swz, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS ? 0 : -1;
 }
 
-int umma_atom_tile(int n_rows) {
-  if (n_rows <= 16) return 16;
-  if (n_rows <= 32) return 32;
-  if (n_rows <= 64) return 64;
-  return 128;
+static int atom_tile(int n_rows, int cap) {
+  int t = 16;
+  while (t < cap && t < n_rows) t *= 2;
+  return t;
 }
 
-static const size_t UMMA_SMEM_BUDGET = 220 * 1024;
+// cycles of one contraction box (32 elements) of a 128 x nt tile: the larger of the tensor-pipe time (12 MMAs of
+// nt/2 cycles) and the shared-memory time (operand reads of the 12 MMAs + the TMA writes, 128 B/clk)
+static long long box_cycles(int nt) {
+  const long long mma = 12LL * (nt / 2);
+  const long long smem = (12LL * (4096 + nt * 32) + 2LL * A_BOX_BYTES + 2LL * nt * 128) / 128;
+  return std::max(mma, smem) + 40;
+}
 
-int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, const std::vector<TmaOperand>& aops,
-                      const std::vector<TmaOperand>& bops, int a_mn, int num_sms) {
-  UmmaParams* P = new UmmaParams();
-  memset(P, 0, sizeof(*P));
-  L.params = P;
-  if (aops.size() > NNP_MAX_SPECIES || bops.size() > NNP_MAX_SPECIES) return -1;
-  std::vector<int> tile_of_bmap(bops.size(), 16);
-  int np_max = 16;
-  for (size_t i = 0; i < bops.size(); ++i) {
-    tile_of_bmap[i] = umma_atom_tile((int)bops[i].rows);
-    np_max = std::max(np_max, tile_of_bmap[i]);
-    if (encode_map(&P->bmap[i], bops[i].base, bops[i].rows, bops[i].cols, bops[i].ld, tile_of_bmap[i],
-                   CU_TENSOR_MAP_SWIZZLE_128B))
-      return -1;
-  }
-  for (size_t i = 0; i < aops.size(); ++i)
-    if (encode_map(&P->amap[i], aops[i].base, aops[i].rows, aops[i].cols, aops[i].ld, a_mn ? 32 : 128,
-                   a_mn ? CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B : CU_TENSOR_MAP_SWIZZLE_128B))
-      return -1;
+static const size_t UMMA_SMEM_BUDGET = 227 * 1024;
+
+struct UmmaPlan {
   std::vector<UmmaItem> items;
   std::vector<long long> cost;
+  std::vector<int> tile_of_bmap;
+  int np_max = 16;
+  long long makespan = 0;
+  double flops = 0;
+};
+
+static void plan_items(UmmaPlan& pl, const std::vector<UmmaProblem>& probs, const std::vector<UmmaOperand>& bops, int cap,
+                       int num_sms) {
+  pl.tile_of_bmap.assign(bops.size(), 16);
+  pl.np_max = 16;
+  for (size_t i = 0; i < bops.size(); ++i) {
+    pl.tile_of_bmap[i] = atom_tile((int)bops[i].rows, cap);
+    pl.np_max = std::max(pl.np_max, pl.tile_of_bmap[i]);
+  }
   for (const UmmaProblem& p : probs) {
     if (p.n_atoms <= 0 || p.F <= 0 || p.K <= 0) continue;
-    const int nt = tile_of_bmap[p.bmap];
+    const int nt = pl.tile_of_bmap[p.bmap];
     const int nkb_all = (p.K + BOXF - 1) / BOXF;
     unsigned long long kmask = nkb_all <= 64 ? p.kmask : 0ull;
     if (nkb_all < 64) kmask &= (1ull << nkb_all) - 1ull;
@@ -532,27 +559,69 @@ int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, cons
       for (int a0 = 0; a0 < p.n_atoms; a0 += nt) {
         UmmaItem t;
         memset(&t, 0, sizeof(t));
-        t.amap = p.amap; t.bmap = p.bmap; t.a_mn = a_mn;
-        if (!a_mn) { t.a_c0 = p.a_c0; t.a_c1 = p.a_c1 + f0; }  // (k col, feature row)
-        else { t.a_c0 = p.a_c0 + f0; t.a_c1 = p.a_c1; }        // (feature col, contraction row)
+        t.amap = p.amap; t.bmap = p.bmap;
+        t.a_c0 = p.a_c0; t.a_c1 = p.a_c1 + f0;  // (k col, feature row)
         t.b_c0 = p.b_c0; t.b_c1 = p.b_c1 + a0;
-        t.kb0 = 0; t.kb1 = nkb;
+        t.nkb = nkb;
         t.kmask = kmask;
         t.n_pad = nt;
         t.n_valid = std::min(nt, p.n_atoms - a0);
         t.f_valid = std::min(128, p.F - f0);
         t.epi = p.epi;
         t.C = p.C + (size_t)a0 * p.ldc + f0;
+        t.C_lo = p.C_lo ? p.C_lo + (size_t)a0 * p.ldc + f0 : nullptr;
         t.ldc = p.ldc;
         t.bias = p.bias ? p.bias + f0 : nullptr;
         t.aux = p.aux ? p.aux + (size_t)a0 * p.ldaux + f0 : nullptr;
+        t.aux_lo = p.aux_lo ? p.aux_lo + (size_t)a0 * p.ldaux + f0 : nullptr;
         t.ldaux = p.ldaux;
         t.scale = p.scale; t.alpha = p.alpha; t.inv_alpha = p.inv_alpha;
-        items.push_back(t);
-        cost.push_back((long long)nkb * (128 + 2 * nt));
+        pl.items.push_back(t);
+        pl.cost.push_back((long long)nkb * box_cycles(nt) + 1500);
+        pl.flops += 2.0 * t.f_valid * t.n_valid * 32.0 * nkb;
       }
     }
   }
+  // makespan of the static schedule below (heavy first, snake order over the CTAs)
+  const size_t n = pl.items.size();
+  const size_t G = std::max<size_t>(1, std::min<size_t>(n, (size_t)num_sms));
+  std::vector<long long> sorted(pl.cost);
+  std::sort(sorted.begin(), sorted.end(), [](long long a, long long b) { return a > b; });
+  std::vector<long long> load(G, 0);
+  for (size_t i = 0; i < n; ++i) {
+    const size_t round = i / G, posn = i % G;
+    load[(round & 1) ? G - 1 - posn : posn] += sorted[i];
+  }
+  pl.makespan = 0;
+  for (long long v : load) pl.makespan = std::max(pl.makespan, v);
+}
+
+int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, const std::vector<UmmaOperand>& aops,
+                      const std::vector<UmmaOperand>& bops, int num_sms) {
+  UmmaParams* P = new UmmaParams();
+  memset(P, 0, sizeof(*P));
+  L.params = P;
+  if (aops.size() > NNP_MAX_SPECIES || bops.size() > NNP_MAX_SPECIES) return -1;
+  // atom-tile width: wide tiles use the operands best (a weight box serves 128 atoms), narrow tiles fill the machine
+  // when the element groups are small; take the width with the shortest estimated makespan
+  UmmaPlan best;
+  bool have = false;
+  for (int cap : {128, 64, 32}) {
+    UmmaPlan pl;
+    plan_items(pl, probs, bops, cap, num_sms);
+    if (!have || pl.makespan < best.makespan) { best = std::move(pl); have = true; }
+  }
+  for (size_t i = 0; i < bops.size(); ++i) {
+    if (encode_map(&P->bhi[i], bops[i].hi, bops[i].rows, bops[i].cols, bops[i].ld, best.tile_of_bmap[i])) return -1;
+    if (encode_map(&P->blo[i], bops[i].lo, bops[i].rows, bops[i].cols, bops[i].ld, best.tile_of_bmap[i])) return -1;
+  }
+  for (size_t i = 0; i < aops.size(); ++i) {
+    if (encode_map(&P->ahi[i], aops[i].hi, aops[i].rows, aops[i].cols, aops[i].ld, 128)) return -1;
+    if (encode_map(&P->alo[i], aops[i].lo, aops[i].rows, aops[i].cols, aops[i].ld, 128)) return -1;
+  }
+  std::vector<UmmaItem>& items = best.items;
+  std::vector<long long>& cost = best.cost;
+  const int np_max = best.np_max;
   // heavy items first, dealt to the persistent CTAs in snake order (static => deterministic)
   const size_t n = items.size();
   std::vector<size_t> order(n);
@@ -572,18 +641,19 @@ int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, cons
   }
   L.n_items = (int)n;
   L.grid = n ? (int)G : 0;
+  L.tile = np_max;
+  L.issued_flops = best.flops;
   P->b_box_bytes = np_max * 128;
-  P->stage_bytes = A_BOX_BYTES + P->b_box_bytes;
-  const size_t bar_bytes = (2 * U_MAX_RAW + 2 * U_LO_STAGES + 2 * U_MAX_GROUPS + 1) * 8 + 16;
-  P->n_raw = (int)std::min<size_t>(U_MAX_RAW, (UMMA_SMEM_BUDGET - 1024 - bar_bytes) / P->stage_bytes - U_LO_STAGES);
-  L.smem_bytes = (size_t)(P->n_raw + U_LO_STAGES) * P->stage_bytes + bar_bytes + 1024;
+  P->stage_bytes = 2 * A_BOX_BYTES + 2 * P->b_box_bytes;
+  const size_t bar_bytes = (2 * U_MAX_STAGES + 2 * U_MAX_SLOTS) * 8 + 16;
+  P->staging_rows = std::min(np_max, 64);
+  const size_t staging_bytes = (size_t)P->staging_rows * 512;  // [atoms of a round][128 features] f32
+  P->n_stages = (int)std::min<size_t>(U_MAX_STAGES, (UMMA_SMEM_BUDGET - 1024 - bar_bytes - staging_bytes) / P->stage_bytes);
+  L.smem_bytes = (size_t)P->n_stages * P->stage_bytes + staging_bytes + bar_bytes + 1024;
   P->slot_cols = np_max;
-  {
-    const char* e = getenv("NNP_UMMA_KPS");  // experiment knob: k-steps accumulated in TMEM per slot
-    P->kps = (e && atoi(e) == 1) ? 1 : 4;
-  }
-  P->gslots = std::max(1, std::min(4, 128 / np_max));
-  P->n_groups = std::min(U_MAX_GROUPS, (512 - np_max) / (P->gslots * np_max));
+  P->n_slots = std::min(U_MAX_SLOTS, 512 / np_max);
+  P->slot_shift = P->n_slots == 8 ? 3 : 2;
+  P->comp = 1;
   if (cudaMalloc((void**)&L.d_items, std::max<size_t>(1, n) * sizeof(UmmaItem)) != cudaSuccess) return -1;
   if (cudaMalloc((void**)&L.d_cta_off, (G + 1) * sizeof(int)) != cudaSuccess) return -1;
   if (n) cudaMemcpy(L.d_items, flat.data(), n * sizeof(UmmaItem), cudaMemcpyHostToDevice);
@@ -593,9 +663,10 @@ int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, cons
   return 0;
 }
 
-void umma_launch(const UmmaLaunch& L, cudaStream_t s) {
+void umma_launch(const UmmaLaunch& L, cudaStream_t s, bool pdl) {
   if (L.n_items == 0) return;
-  gemm_umma_kernel<<<L.grid, U_THREADS, L.smem_bytes, s>>>(*reinterpret_cast<const UmmaParams*>(L.params));
+  launch_kernel(pdl, gemm_umma_kernel, dim3(L.grid), dim3(U_THREADS), L.smem_bytes, s,
+                *reinterpret_cast<const UmmaParams*>(L.params));
 }
 
 int umma_init() {

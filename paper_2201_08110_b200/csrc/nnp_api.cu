@@ -67,11 +67,14 @@ extern "C" void nnp_destroy(nnp_handle* h) {
   for (auto e : h->events) cudaEventDestroy(e);
   void* ptrs[] = {h->d_eblocks, h->d_epart, h->d_ecount, h->d_mol_range, h->d_species, h->d_mol_off, h->d_mol_id, h->d_sortpos, h->d_perm, h->d_grp_off, h->d_self_energy,
                   h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_aev, h->d_daev, h->d_phi,
-                  h->d_eatom, h->d_status, h->d_W, h->d_b, h->d_hpos, h->d_hforce, h->d_henergy};
+                  h->d_eatom, h->d_status, h->d_W, h->d_b, h->d_hpos, h->d_hforce, h->d_henergy,
+                  h->d_aev_lo, h->d_Whi, h->d_Wlo, h->d_WThi, h->d_WTlo};
   for (void* p : ptrs)
     if (p) cudaFree(p);
-  for (int l = 0; l < NNP_MAX_LAYERS; ++l)
+  for (int l = 0; l < NNP_MAX_LAYERS; ++l) {
     if (h->d_act[l]) cudaFree(h->d_act[l]);
+    if (h->d_act_lo[l]) cudaFree(h->d_act_lo[l]);
+  }
   for (auto* v : {&h->fwd, &h->bwd})
     for (auto& g : *v) {
       if (g.d_probs) cudaFree(g.d_probs);
@@ -232,8 +235,8 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   h->w_floats = (size_t)wo;
   h->b_floats = (size_t)bo;
   std::vector<float> B((size_t)bo, 0.f);  // host copy of the biases (the ligand-size engine folds b_L into its items)
+  std::vector<float> Wh((size_t)wo, 0.f);  // host copy of the weight arena (split for the tensor engine below)
   {
-    std::vector<float> W((size_t)wo, 0.f);
     for (int m = 0; m < M; ++m)
       for (int e = 0; e < S; ++e)
         for (int l = 0; l < L; ++l) {
@@ -241,11 +244,11 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
           const size_t idx = ((size_t)m * S + e) * L + l;
           const float* src = cfg->weights[idx];
           if (!src) return fail(NNP_ERR_INVALID_ARG);
-          memcpy(&W[h->w_off[e * L + l] + (size_t)m * nout * nin], src, sizeof(float) * (size_t)nout * nin);
+          memcpy(&Wh[h->w_off[e * L + l] + (size_t)m * nout * nin], src, sizeof(float) * (size_t)nout * nin);
           if (cfg->biases && cfg->biases[idx])
             memcpy(&B[h->b_off[e * L + l] + (size_t)m * nout], cfg->biases[idx], sizeof(float) * nout);
         }
-    if (upload(&h->d_W, W) || upload(&h->d_b, B)) return fail(NNP_ERR_ALLOC);
+    if (upload(&h->d_W, Wh) || upload(&h->d_b, B)) return fail(NNP_ERR_ALLOC);
   }
 
   // ---- MLP engine: the tensor-core engine needs hidden widths that are whole 32-float TMA boxes
@@ -266,6 +269,52 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   // at ligand sizes the layer-1 backward is split per model (every CTA streams its own slice of W1
   // exactly once); the M partial dE/dAEV rows are summed by the AEV backward kernel
   h->n_parts = (h->use_small && parts_fit) ? M : 1;
+  if (h->use_umma) {
+    // layer-1 backward on the tensor engine: one GEMM per element with K = M*H1.  When that leaves most SMs without a
+    // tile (few hundred atoms), the contraction is cut into n_parts groups of models whose partial dE/dAEV rows the
+    // AEV backward kernel sums (as it does at ligand sizes).
+    long long tiles = 0;
+    for (int e = 0; e < S; ++e) tiles += ((h->grp_off[e + 1] - h->grp_off[e] + 127) / 128) * (long long)((n_feat + 127) / 128);
+    int parts = 1;
+    while (parts < M && M % (2 * parts) == 0 && tiles * parts < 2LL * prop.multiProcessorCount &&
+           (size_t)N * (2 * parts) * n_feat * 4 <= ((size_t)64 << 20))
+      parts *= 2;
+    h->n_parts = parts;
+    // 3xTF32 operand planes: weights hi = rna_tf32(w), lo = rna_tf32(w - hi), in the forward layout and transposed
+    // (layer 1: [n_feat][M*H1]; layers l > 1: per model [H_{l-1}][H_l]) so that both passes read K-major boxes
+    auto rna = [](float x) {
+      uint32_t u;
+      memcpy(&u, &x, 4);
+      u = (u + 0x1000u) & 0xFFFFE000u;
+      float r;
+      memcpy(&r, &u, 4);
+      return r;
+    };
+    std::vector<float> hi(Wh.size()), lo(Wh.size()), thi(Wh.size(), 0.f), tlo(Wh.size(), 0.f);
+    for (size_t i = 0; i < Wh.size(); ++i) {
+      hi[i] = rna(Wh[i]);
+      lo[i] = rna(Wh[i] - hi[i]);
+    }
+    for (int e = 0; e < S; ++e)
+      for (int l = 0; l < L - 1; ++l) {
+        const int nin = h->dims[e * (L + 1) + l], nout = h->dims[e * (L + 1) + l + 1];
+        const size_t base = (size_t)h->w_off[e * L + l];
+        for (int m = 0; m < M; ++m)
+          for (int o = 0; o < nout; ++o) {
+            const size_t src = base + ((size_t)m * nout + o) * nin;
+            for (int n = 0; n < nin; ++n) {
+              const size_t dst = l == 0 ? base + (size_t)n * M * nout + (size_t)m * nout + o
+                                        : base + ((size_t)m * nin + n) * nout + o;
+              thi[dst] = hi[src + n];
+              tlo[dst] = lo[src + n];
+            }
+          }
+      }
+    if (upload(&h->d_Whi, hi) || upload(&h->d_Wlo, lo) || upload(&h->d_WThi, thi) || upload(&h->d_WTlo, tlo))
+      return fail(NNP_ERR_ALLOC);
+  }
+  Wh.clear();
+  Wh.shrink_to_fit();
 
   // ---- workspaces
   if (dev_alloc(&h->d_pos4, (size_t)N) || dev_alloc(&h->d_nbr_r, (size_t)N * h->capR) ||
@@ -275,6 +324,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       dev_alloc(&h->d_eatom, (size_t)N * M) || dev_alloc(&h->d_status, 1) || dev_alloc(&h->d_hpos, (size_t)N * 3) ||
       dev_alloc(&h->d_hforce, (size_t)N * 3) || dev_alloc(&h->d_henergy, (size_t)n_molecules))
     return fail(NNP_ERR_ALLOC);
+  if (h->use_umma && dev_alloc(&h->d_aev_lo, (size_t)N * n_feat)) return fail(NNP_ERR_ALLOC);
   // latency-bound sizes only: in a large batch the serial row build inside every centre's CTA costs more than the
   // launch it saves (configs[2]: +36 us in the AEV forward against a 12 us neighbour kernel)
   h->fuse_nbr = N > 0 && N <= 512 && !h->use_cells && max_mol <= 256 && !(cfg->flags & NNP_FLAG_NO_NBR_FUSION);
@@ -312,6 +362,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       o = align_up(o + ne * M * h->dims[e * (L + 1) + l], 64);
     }
     if (dev_alloc(&h->d_act[l], (size_t)o)) return fail(NNP_ERR_ALLOC);
+    if (h->use_umma && dev_alloc(&h->d_act_lo[l], (size_t)o)) return fail(NNP_ERR_ALLOC);
   }
 
   // ---- MLP launches (grouped GEMMs), shapes fixed at create time
@@ -436,18 +487,25 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       for (int li = 0; li < L - 1; ++li) {
         const int l = pass == 0 ? li + 1 : L - 1 - li;  // fwd: 1..L-1, bwd: L-1..1
         std::vector<UmmaProblem> probs;
-        std::vector<TmaOperand> aops(ns), bops(ns);
+        std::vector<UmmaOperand> aops(ns), bops(ns);
         for (int e = 0; e < S; ++e) {
           if (slot[e] < 0) continue;
           const int ne = h->grp_off[e + 1] - h->grp_off[e];
           const int nin = h->dims[e * (L + 1) + l - 1], nout = h->dims[e * (L + 1) + l];
-          const float* Wl = h->d_W + h->w_off[e * L + l - 1];
-          aops[slot[e]] = TmaOperand{Wl, (long long)M * nout, nin, nin};
+          const long long wofs = h->w_off[e * L + l - 1];
           if (pass == 0) {
-            if (l == 1) bops[slot[e]] = TmaOperand{h->d_aev + (size_t)h->grp_off[e] * n_feat, ne, n_feat, n_feat};
-            else bops[slot[e]] = TmaOperand{h->d_act[l - 1] + h->act_off[l - 1][e], ne, (long long)M * nin, (long long)M * nin};
+            aops[slot[e]] = UmmaOperand{h->d_Whi + wofs, h->d_Wlo + wofs, (long long)M * nout, nin, nin};
+            if (l == 1)
+              bops[slot[e]] = UmmaOperand{h->d_aev + (size_t)h->grp_off[e] * n_feat, h->d_aev_lo + (size_t)h->grp_off[e] * n_feat,
+                                          ne, n_feat, n_feat};
+            else
+              bops[slot[e]] = UmmaOperand{h->d_act[l - 1] + h->act_off[l - 1][e], h->d_act_lo[l - 1] + h->act_off[l - 1][e], ne,
+                                          (long long)M * nin, (long long)M * nin};
           } else {
-            bops[slot[e]] = TmaOperand{h->d_act[l] + h->act_off[l][e], ne, (long long)M * nout, (long long)M * nout};
+            if (l == 1) aops[slot[e]] = UmmaOperand{h->d_WThi + wofs, h->d_WTlo + wofs, nin, (long long)M * nout, (long long)M * nout};
+            else aops[slot[e]] = UmmaOperand{h->d_WThi + wofs, h->d_WTlo + wofs, (long long)M * nin, nout, nout};
+            bops[slot[e]] = UmmaOperand{h->d_act[l] + h->act_off[l][e], h->d_act_lo[l] + h->act_off[l][e], ne,
+                                        (long long)M * nout, (long long)M * nout};
           }
           UmmaProblem p;
           memset(&p, 0, sizeof(p));
@@ -458,8 +516,8 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
           if (pass == 0 && l == 1) {
             p.kmask = l1_kmask;
             p.F = M * nout; p.K = nin;
-            p.a_c0 = 0; p.a_c1 = 0; p.b_c0 = 0; p.b_c1 = 0;
             p.C = h->d_act[1] + h->act_off[1][e];
+            p.C_lo = h->d_act_lo[1] + h->act_off[1][e];
             p.ldc = M * nout;
             p.bias = h->d_b + h->b_off[e * L + 0];
             p.epi = EPI_BIAS_CELU;
@@ -470,46 +528,42 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
               q.F = nout; q.K = nin;
               q.a_c0 = 0; q.a_c1 = m * nout; q.b_c0 = m * nin; q.b_c1 = 0;
               q.C = h->d_act[l] + h->act_off[l][e] + (size_t)m * nout;
+              q.C_lo = h->d_act_lo[l] + h->act_off[l][e] + (size_t)m * nout;
               q.ldc = M * nout;
               q.bias = h->d_b + h->b_off[e * L + l - 1] + (size_t)m * nout;
               q.epi = EPI_BIAS_CELU;
               probs.push_back(q);
             }
           } else if (l > 1) {
-            for (int m = 0; m < M; ++m) {
+            for (int m = 0; m < M; ++m) {  // delta_{l-1}[a][n] = CELU'(h_{l-1}) sum_o WT[m][n][o] delta_l[a][m][o]
               UmmaProblem q = p;
               q.F = nin; q.K = nout;
-              q.a_c0 = 0; q.a_c1 = m * nout; q.b_c0 = m * nout; q.b_c1 = 0;
+              q.a_c0 = 0; q.a_c1 = m * nin; q.b_c0 = m * nout; q.b_c1 = 0;
               q.C = h->d_act[l - 1] + h->act_off[l - 1][e] + (size_t)m * nin;
+              q.C_lo = h->d_act_lo[l - 1] + h->act_off[l - 1][e] + (size_t)m * nin;
               q.ldc = M * nin;
-              q.aux = q.C; q.ldaux = q.ldc;
+              q.aux = q.C; q.aux_lo = q.C_lo; q.ldaux = q.ldc;
               q.epi = EPI_MUL_DCELU;
               probs.push_back(q);
             }
-          } else {
-            const int n_prob = h->n_parts == 1 ? 1 : M;
-            for (int m = 0; m < n_prob; ++m) {
+          } else {  // dE/dAEV[a][n] = (1/M) sum_{m,o} W1T[n][m*H1 + o] delta_1[a][m][o], in n_parts groups of models
+            const int mg = M / h->n_parts;
+            for (int pt = 0; pt < h->n_parts; ++pt) {
               UmmaProblem q = p;
               q.fmask = l1_fmask;
-              q.F = nin;
+              q.F = nin; q.K = mg * nout;
+              q.a_c0 = pt * mg * nout; q.a_c1 = 0; q.b_c0 = pt * mg * nout; q.b_c1 = 0;
               q.epi = EPI_SCALE;
               q.scale = 1.0f / (float)M;
               q.ldc = n_feat;
-              q.a_c0 = 0; q.b_c1 = 0;
-              if (h->n_parts == 1) {
-                q.K = M * nout; q.a_c1 = 0; q.b_c0 = 0;
-                q.C = h->d_daev + (size_t)h->grp_off[e] * n_feat;
-              } else {
-                q.K = nout; q.a_c1 = m * nout; q.b_c0 = m * nout;
-                q.C = h->d_daev + ((size_t)m * N + h->grp_off[e]) * n_feat;
-              }
+              q.C = h->d_daev + ((size_t)pt * N + h->grp_off[e]) * n_feat;
               probs.push_back(q);
             }
           }
         }
         UmmaLaunch ul;
         ul.name = (pass == 0 ? "mlp_fwd_l" : "mlp_bwd_l") + std::to_string(l);
-        if (umma_build_launch(ul, probs, aops, bops, pass, prop.multiProcessorCount)) {
+        if (umma_build_launch(ul, probs, aops, bops, prop.multiProcessorCount)) {
           umma_free_launch(ul);
           return fail(NNP_ERR_CUDA);
         }
@@ -727,7 +781,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     }
     LastLayerArgs& la = h->last;
     memset(&la, 0, sizeof(la));
-    la.act = h->d_act[L - 1]; la.W = h->d_W; la.bias = h->d_b; la.e_out = h->d_eatom;
+    la.act = h->d_act[L - 1]; la.act_lo = h->d_act_lo[L - 1]; la.W = h->d_W; la.bias = h->d_b; la.e_out = h->d_eatom;
     for (int e = 0; e <= S; ++e) la.grp_off[e] = h->grp_off[e];
     for (int e = 0; e < S; ++e) {
       la.act_off[e] = ao[e]; la.w_off[e] = wo2[e]; la.b_off[e] = bo2[e]; la.H[e] = Hs[e];
@@ -783,13 +837,13 @@ static void enqueue_chain(nnp_handle* h, const float* d_pos, int ps, const int* 
     return;
   }
   if (h->use_umma) {
-    for (auto& g : h->ufwd) { umma_launch(g, s); mark(); }
+    for (auto& g : h->ufwd) { umma_launch(g, s, pdl); mark(); }
   } else {
     for (auto& g : h->fwd) { launch_gemm(g, s); mark(); }
   }
   launch_last_layer(h, s); mark();
   if (h->use_umma) {
-    for (auto& g : h->ubwd) { umma_launch(g, s); mark(); }
+    for (auto& g : h->ubwd) { umma_launch(g, s, pdl); mark(); }
   } else {
     for (auto& g : h->bwd) { launch_gemm(g, s); mark(); }
   }
@@ -953,7 +1007,15 @@ static int export_rows(nnp_handle* h, const float* d_rows, float* host) {
   return NNP_OK;
 }
 
-extern "C" int nnp_debug_aev(nnp_handle* h, float* aev_host) { return export_rows(h, h ? h->d_aev : nullptr, aev_host); }
+extern "C" int nnp_debug_aev(nnp_handle* h, float* aev_host) {
+  if (!h) return NNP_ERR_INVALID_ARG;
+  int rc = export_rows(h, h->d_aev, aev_host);
+  if (rc != NNP_OK || !h->d_aev_lo) return rc;
+  std::vector<float> lo((size_t)h->N * h->n_feat);  // tensor engine: the row is stored split, G = hi + lo exactly
+  rc = export_rows(h, h->d_aev_lo, lo.data());
+  for (size_t i = 0; rc == NNP_OK && i < lo.size(); ++i) aev_host[i] += lo[i];
+  return rc;
+}
 extern "C" int nnp_debug_daev(nnp_handle* h, float* g_host) {
   if (!h) return NNP_ERR_INVALID_ARG;
   int rc = export_rows(h, h->d_daev, g_host);

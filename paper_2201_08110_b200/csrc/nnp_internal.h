@@ -97,18 +97,27 @@ struct TmaOperand {
   long long rows, cols, ld;
 };
 
-// ---- tcgen05 engine (mlp_umma.cu): D[f][a] = sum_k A[f][k] B[a][k], f = output feature, a = atom
+// ---- tcgen05 engine (mlp_umma.cu): D[f][a] = sum_k A[f][k] B[a][k], f = output feature, a = atom.
+// Both operands arrive PRE-SPLIT for 3xTF32: every matrix is a pair of planes (hi, lo) with hi = rna_tf32(x),
+// lo = x - hi (activations, written by the producing kernel) or rna_tf32(x - hi) (weights, split at create time).
+struct UmmaOperand {         // a row-major f32 matrix pair [rows][cols], pitch ld floats
+  const float* hi;
+  const float* lo;
+  long long rows, cols, ld;
+};
 struct UmmaItem {            // one tile of one GEMM, as the persistent CTAs consume it
-  int amap, bmap, a_mn;      // tensor-map slots; a_mn = 1: weights read as an MN-major operand (backward)
-  int a_c0, a_c1;            // weight box origin: K-major (k col, feature row) / MN-major (feature col, k row)
+  int amap, bmap;            // tensor-map slots (weights / activations)
+  int a_c0, a_c1;            // weight box origin (k col, feature row)
   int b_c0, b_c1;            // activation box origin (k col, atom row)
-  int kb0, kb1;              // contraction boxes (32 wide) [kb0, kb1) as the consumers count them
-  unsigned long long kmask;  // non-zero: the boxes actually loaded are the set bits (popcount = kb1 - kb0)
+  int nkb;                   // contraction boxes (32 wide) of the item
+  unsigned long long kmask;  // non-zero: the boxes actually loaded are the set bits (popcount = nkb)
   int n_pad, n_valid, f_valid;  // MMA N (16/32/64/128), atoms and feature rows actually stored
   int epi, ldc, ldaux;
-  float* C;                  // C[a * ldc + f]
+  float* C;                  // C[a * ldc + f]: hi plane (or the whole value when C_lo is null)
+  float* C_lo;               // lo plane of the output, or null
   const float* bias;         // [f] or null
-  const float* aux;          // aux[a * ldaux + f]: activations h for EPI_MUL_DCELU (may alias C)
+  const float* aux;          // aux[a * ldaux + f]: activations h (hi plane) for EPI_MUL_DCELU (may alias C)
+  const float* aux_lo;       // lo plane of h (may alias C_lo), or null
   float scale, alpha, inv_alpha;
 };
 struct UmmaProblem {
@@ -119,22 +128,25 @@ struct UmmaProblem {
   int F, n_atoms, K;
   int epi, ldc, ldaux;
   float* C;
+  float* C_lo;
   const float* bias;
   const float* aux;
+  const float* aux_lo;
   float scale, alpha, inv_alpha;
 };
 struct UmmaLaunch {
   void* params = nullptr;  // UmmaParams (host copy, passed by value as __grid_constant__)
   UmmaItem* d_items = nullptr;
   int* d_cta_off = nullptr;
-  int n_items = 0, grid = 0;
+  int n_items = 0, grid = 0, tile = 0;
   size_t smem_bytes = 0;
+  double issued_flops = 0;  // 2 x MACs of the boxes actually run (padding and structural zeros excluded/included as issued)
   std::string name;
 };
 int umma_init();
-int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, const std::vector<TmaOperand>& aops,
-                      const std::vector<TmaOperand>& bops, int a_mn, int num_sms);
-void umma_launch(const UmmaLaunch& L, cudaStream_t s);
+int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, const std::vector<UmmaOperand>& aops,
+                      const std::vector<UmmaOperand>& bops, int num_sms);
+void umma_launch(const UmmaLaunch& L, cudaStream_t s, bool pdl);
 void umma_free_launch(UmmaLaunch& L);
 
 // ---- ligand-size engine (mlp_small.cu): weight-streaming FFMA kernels, one CTA per item
@@ -213,6 +225,7 @@ struct EnergyBlock {  // one CTA of the energy reduction: atoms [a0, a1) of mole
 
 struct LastLayerArgs {
   float* act;          // [n_atoms_sorted][M][H] per element group (arena), overwritten with delta
+  float* act_lo;       // tensor engine: lo plane of the same arena (h = act + act_lo; delta is written split), else null
   const float* W;      // arena
   const float* bias;   // arena
   double* e_out;       // [n_sorted][M]
@@ -244,6 +257,7 @@ struct nnp_handle {
   float4* d_pos4 = nullptr;
   int *d_nbr_r = nullptr, *d_nbr_a = nullptr, *d_cnt_r = nullptr, *d_cnt_a = nullptr;
   float* d_aev = nullptr;   // [N sorted][n_feat]
+  float* d_aev_lo = nullptr;  // tensor engine: lo plane (d_aev then holds rna_tf32(G), d_aev_lo = G - that)
   float* d_daev = nullptr;  // [n_parts][N sorted][n_feat]
   float* d_phi = nullptr;   // [N][capR][3]
   double* d_eatom = nullptr;  // [N sorted][M]
@@ -260,10 +274,13 @@ struct nnp_handle {
   int* d_status = nullptr;
   // weights
   float *d_W = nullptr, *d_b = nullptr;
+  // tensor engine: weights split for 3xTF32 (hi, lo), in the forward layout and transposed for the backward pass
+  float *d_Whi = nullptr, *d_Wlo = nullptr, *d_WThi = nullptr, *d_WTlo = nullptr;
   std::vector<long long> w_off, b_off;  // [S][L] float offsets of the (e,l) block, models contiguous
   size_t w_floats = 0, b_floats = 0;
   // activations: act[l] for l = 1..L-1
   float* d_act[NNP_MAX_LAYERS] = {nullptr};
+  float* d_act_lo[NNP_MAX_LAYERS] = {nullptr};  // tensor engine: lo planes
   std::vector<long long> act_off[NNP_MAX_LAYERS];  // [S] float offsets
   // MLP launches
   std::vector<GemmLaunch> fwd, bwd;  // fwd: layers 1..L-1; bwd: layers L-1..1
