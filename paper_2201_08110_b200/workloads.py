@@ -361,3 +361,55 @@ def random_molecule(n: int, n_species: int, seed: int, side: float | None = None
     spc = rng.integers(0, n_species, size=n).astype(np.int32)
     p = params if params is not None else ani2x_params()
     return Workload(f"rand{n}", 0, pos, spc, np.array([0, n], np.int32), n_models, 1, seed + 2, seed + 3, p)
+
+
+# ------------------------------------------------------------------------------------------------
+# NNP/MM system for the coupling term (Eq. 4): the ligand-sized NNP region of configs[1] inside
+# an MM environment of water-like density.  The paper's systems (Table 1: 48-75 ligand atoms in
+# 26-40 thousand-atom solvated complexes) are not in this container; this generator takes their sizes.  Charges and
+# Lennard-Jones parameters are drawn in the ranges of a biomolecular force field; no arithmetic of the method here.
+@dataclasses.dataclass(frozen=True)
+class CouplingSystem:
+    positions: np.ndarray  # f32[n_rows][3], A; rows of NNP and MM atoms interleaved at random
+    nnp_rows: np.ndarray   # i32[n_nnp]
+    mm_rows: np.ndarray    # i32[n_mm]
+    q_nnp: np.ndarray      # f32, e
+    sigma_nnp: np.ndarray  # f32, A
+    eps_nnp: np.ndarray    # f32, kcal/mol
+    q_mm: np.ndarray
+    sigma_mm: np.ndarray
+    eps_mm: np.ndarray
+
+    @property
+    def n_rows(self) -> int:
+        return int(self.positions.shape[0])
+
+
+def coupling_system(n_mm: int = 30000, seed: int = BASE_SEED + 77, density: float = 0.1,
+                    min_dist: float = 1.6) -> CouplingSystem:
+    """configs[1]'s 50-atom NNP region at the centre of a cube of n_mm MM atoms at `density` atoms/A^3; MM atoms keep
+    `min_dist` from the NNP atoms (no clash with the ligand), not from each other (MM-MM pairs are not in Eq. 4)."""
+    rng = np.random.default_rng(seed)
+    lig = config2()
+    n_nnp = lig.n_atoms
+    side = ((n_mm + n_nnp) / density) ** (1.0 / 3.0)
+    nnp_pos = lig.positions.astype(np.float64)  # centred at the origin (ball of radius 6 A)
+    mm = np.empty((0, 3))
+    while mm.shape[0] < n_mm:
+        cand = rng.uniform(-side / 2, side / 2, size=(2 * (n_mm - mm.shape[0]) + 64, 3))
+        near = cand[np.abs(cand).max(axis=1) < 8.0]
+        ok = np.ones(cand.shape[0], bool)
+        idx = np.nonzero(np.abs(cand).max(axis=1) < 8.0)[0]
+        if idx.size:
+            d = np.linalg.norm(near[:, None, :] - nnp_pos[None, :, :], axis=2).min(axis=1)
+            ok[idx[d < min_dist]] = False
+        mm = np.concatenate([mm, cand[ok]])[:n_mm]
+    n_rows = n_nnp + n_mm
+    perm = rng.permutation(n_rows).astype(np.int32)
+    pos = np.empty((n_rows, 3), np.float32)
+    nnp_rows, mm_rows = perm[:n_nnp].copy(), perm[n_nnp:].copy()
+    pos[nnp_rows] = nnp_pos.astype(np.float32)
+    pos[mm_rows] = mm.astype(np.float32)
+    f32 = lambda lo, hi, n: rng.uniform(lo, hi, size=n).astype(np.float32)
+    return CouplingSystem(pos, nnp_rows, mm_rows, f32(-0.6, 0.6, n_nnp), f32(1.0, 3.6, n_nnp), f32(0.01, 0.25, n_nnp),
+                          f32(-0.9, 0.9, n_mm), f32(0.4, 3.6, n_mm), f32(0.0, 0.25, n_mm))
