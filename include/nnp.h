@@ -104,6 +104,23 @@ int nnp_create(nnp_handle **out, const nnp_config *cfg, int32_t n_atoms, const i
                int32_t n_molecules, const int32_t *mol_offsets_host);
 
 /*
+ * nnp_create_from_file: nnp_create from a parameter file holding a whole ANI-style parameter set (element list in
+ * the set's own species order, AEV constants, layer shapes, weights AND biases of every (model, element, layer),
+ * self-energies, energy scale); PAPER.md:36 (ANI-2x), :166-175 (ANI-1x as a second set).  The container format is
+ * this library's own, documented in csrc/params_file.cu and written by binding.write_parameter_file (the trained
+ * sets are not distributed with the library).
+ *   path                 host; file name
+ *   atomic_numbers_host  host i32[N]: the atoms by ATOMIC NUMBER; mapped to species indices through the file's
+ *                        element list (an element the set does not cover => NNP_ERR_INVALID_ARG)
+ *   n_models_to_use      0 = the whole ensemble; k > 0 = its first k networks (1 = the "1 NN" variant)
+ *   length_scale, flags  as in nnp_config
+ * Errors: NNP_ERR_INVALID_ARG for an unreadable / malformed file, else as nnp_create.
+ */
+int nnp_create_from_file(nnp_handle **out, const char *path, int32_t n_atoms, const int32_t *atomic_numbers_host,
+                         int32_t n_molecules, const int32_t *mol_offsets_host, int32_t n_models_to_use,
+                         double length_scale, int32_t flags);
+
+/*
  * nnp_compute: one energy+force evaluation (one MD step), enqueued on `cuda_stream`.
  *   d_pos               device f32; position of NNP atom a is at d_pos[row(a)*pos_stride_floats + 0..2]
  *                       in caller length units (x length_scale = A)
@@ -129,6 +146,32 @@ int nnp_compute(nnp_handle *h, const float *d_pos, int32_t pos_stride_floats, co
  */
 int nnp_compute_host(nnp_handle *h, const float *pos_host, double *energy_host, float *force_host,
                      void *cuda_stream);
+
+/*
+ * nnp_compute_fixed: nnp_compute with the forces accumulated in 64-bit fixed point ("performs the NNP
+ * and MM calculations on a GPU sequentially, but it would be more efficient to do that concurrently").
+ *   d_force_fixed       device i64; round(F * 2^32) is added with integer atomics at
+ *                       d_force_fixed[row(a)*force_stride_int64 + 0..2] (the accumulation format of GPU MD engines).
+ *                       Integer additions commute, so kernels of the MM engine may add into the same buffer AT THE
+ *                       SAME TIME on another stream and the sum has the same bits in any order.  nnp_compute's
+ *                       float read-modify-write is only safe when every other adder is ordered with its stream.
+ * Everything else as nnp_compute.
+ */
+int nnp_compute_fixed(nnp_handle *h, const float *d_pos, int32_t pos_stride_floats, const int32_t *d_atom_index,
+                      double *d_energy, int64_t *d_force_fixed, int32_t force_stride_int64, void *cuda_stream);
+
+/*
+ * nnp_compute_async: the evaluation on a stream OWNED BY THE LIBRARY, so that the caller's MM kernels overlap it.
+ *   wait_event   a cudaEvent_t the caller recorded after the positions were written, or NULL (positions ready now)
+ *   done_event   a cudaEvent_t the library records when energy and forces are in, or NULL; the caller makes its
+ *                integrator wait on it (cudaStreamWaitEvent) -- no host synchronisation anywhere
+ *   d_force / force_stride / force_is_fixed64
+ *                as d_force_accum of nnp_compute (0) or d_force_fixed of nnp_compute_fixed (1).  Concurrent adders
+ *                into the same buffer require the fixed-point format.
+ */
+int nnp_compute_async(nnp_handle *h, const float *d_pos, int32_t pos_stride_floats, const int32_t *d_atom_index,
+                      double *d_energy, void *d_force, int32_t force_stride, int32_t force_is_fixed64,
+                      void *wait_event, void *done_event);
 
 /* nnp_status: synchronises the last used stream and returns the sticky device status (NNP_OK or
  * NNP_ERR_CAPACITY / NNP_ERR_NONFINITE / NNP_ERR_CUDA); the flag is cleared by the call. */
@@ -159,6 +202,13 @@ const char *nnp_stage_name(nnp_handle *h, int32_t stage);
 int nnp_get_work(nnp_handle *h, double *what_host, int32_t n);
 
 /*
+ * nnp_measure_peaks (measurement only): micro-benchmarks on the current device; peaks_host f64[n], n <= 4:
+ * [0] FP32 FFMA TFLOP/s, [1] tcgen05 kind::tf32 TFLOP/s issued from shared-memory operands (M=128, N=256, K=8),
+ * [2] L2-resident read GB/s, [3] DRAM read GB/s.  Synchronises the device; takes ~0.1 s.
+ */
+int nnp_measure_peaks(double *peaks_host, int32_t n);
+
+/*
  * Debug / parity exports: copy device workspace of the LAST compute to the host after synchronising.
  * Not on the timed path.  Atom indices are the caller's NNP atom order (0..N-1).
  *   nnp_debug_pairs   which = 0 radial / 1 angular; writes directed pairs (i,j) as i32 pairs, row-major
@@ -174,6 +224,31 @@ int nnp_debug_aev(nnp_handle *h, float *aev_host);
 int nnp_debug_atomic_energies(nnp_handle *h, double *e_host);
 int nnp_debug_daev(nnp_handle *h, float *g_host);
 int nnp_n_features(nnp_handle *h);
+
+/*
+ * NNP-MM coupling term of mechanical embedding, Eq. 4:
+ *   V_NNP-MM = sum_{i in NNP} sum_{j in MM} [ kc q_i q_j / r_ij + 4 eps_ij ((sigma_ij/r_ij)^12 - (sigma_ij/r_ij)^6) ]
+ * with sigma_ij = (sigma_i + sigma_j)/2, eps_ij = sqrt(eps_i eps_j) (reading C1), kc = 1/(4 pi eps0) supplied by the
+ * caller in its units (C2), an optional inclusive plain cutoff on r_ij in A (C3; <= 0: none) and no periodic images
+ * (C4).  Only NNP-MM pairs enter.  Forces on the atoms of BOTH regions are ADDED to the caller's buffer.
+ *
+ * nnp_coupling_create: all pointers HOST, copied.  *_rows are rows of the atoms in the caller's position / force
+ * buffers; q in e, sigma in A, eps in the output energy unit; length_scale = A per caller length unit.
+ * nnp_coupling_compute: d_pos / d_force_accum as in nnp_compute (device, strides in floats); d_energy device f64[1],
+ * WRITTEN, may be NULL; asynchronous on cuda_stream.  nnp_coupling_compute_fixed: 64-bit fixed-point forces as in
+ * nnp_compute_fixed.  Errors: NNP_ERR_INVALID_ARG (negative row or eps, bad stride, NULL handle), NNP_ERR_CUDA,
+ * NNP_ERR_UNSUPPORTED_ARCH, NNP_ERR_ALLOC.
+ */
+typedef struct nnp_coupling nnp_coupling; /* opaque; owned by the library */
+int nnp_coupling_create(nnp_coupling **out, int32_t n_nnp, const int32_t *nnp_rows_host, const float *q_nnp_host,
+                        const float *sigma_nnp_host, const float *eps_nnp_host, int32_t n_mm,
+                        const int32_t *mm_rows_host, const float *q_mm_host, const float *sigma_mm_host,
+                        const float *eps_mm_host, double coulomb_const, double cutoff, double length_scale);
+int nnp_coupling_compute(nnp_coupling *c, const float *d_pos, int32_t pos_stride_floats, double *d_energy,
+                         float *d_force_accum, int32_t force_stride_floats, void *cuda_stream);
+int nnp_coupling_compute_fixed(nnp_coupling *c, const float *d_pos, int32_t pos_stride_floats, double *d_energy,
+                               int64_t *d_force_fixed, int32_t force_stride_int64, void *cuda_stream);
+void nnp_coupling_destroy(nnp_coupling *c);
 
 #ifdef __cplusplus
 }

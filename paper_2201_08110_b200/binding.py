@@ -38,7 +38,10 @@ SYMBOLS = (
     "nnp_create", "nnp_compute", "nnp_compute_host", "nnp_status", "nnp_destroy", "nnp_error_string",
     "nnp_launches_per_compute", "nnp_set_profiling", "nnp_get_stage_times", "nnp_stage_name", "nnp_get_work",
     "nnp_debug_pairs", "nnp_debug_aev", "nnp_debug_atomic_energies", "nnp_debug_daev", "nnp_n_features",
+    "nnp_create_from_file", "nnp_compute_fixed", "nnp_compute_async", "nnp_measure_peaks",
+    "nnp_coupling_create", "nnp_coupling_compute", "nnp_coupling_compute_fixed", "nnp_coupling_destroy",
 )
+FIXED_ONE = float(1 << 32)  # 64-bit fixed-point force format: round(F * 2^32)
 
 
 class NNPError(RuntimeError):
@@ -119,6 +122,25 @@ def load_library():
             getattr(lib, name).argtypes = [C.c_void_p, C.c_void_p]
         lib.nnp_n_features.restype = C.c_int
         lib.nnp_n_features.argtypes = [C.c_void_p]
+        lib.nnp_create_from_file.restype = C.c_int
+        lib.nnp_create_from_file.argtypes = [C.POINTER(C.c_void_p), C.c_char_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p,
+                                             C.c_int32, C.c_double, C.c_int32]
+        lib.nnp_compute_fixed.restype = C.c_int
+        lib.nnp_compute_fixed.argtypes = lib.nnp_compute.argtypes
+        lib.nnp_compute_async.restype = C.c_int
+        lib.nnp_compute_async.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
+                                          C.c_int32, C.c_void_p, C.c_void_p]
+        lib.nnp_measure_peaks.restype = C.c_int
+        lib.nnp_measure_peaks.argtypes = [C.c_void_p, C.c_int32]
+        lib.nnp_coupling_create.restype = C.c_int
+        lib.nnp_coupling_create.argtypes = [C.POINTER(C.c_void_p), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                            C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double,
+                                            C.c_double, C.c_double]
+        for name in ("nnp_coupling_compute", "nnp_coupling_compute_fixed"):
+            getattr(lib, name).restype = C.c_int
+            getattr(lib, name).argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+        lib.nnp_coupling_destroy.restype = None
+        lib.nnp_coupling_destroy.argtypes = [C.c_void_p]
         _lib = lib
     return _lib
 
@@ -189,7 +211,42 @@ class NNP:
         self.h = h
         self.n_features = int(self.lib.nnp_n_features(self.h))
 
+    @classmethod
+    def from_file(cls, path: str, atomic_numbers, mol_offsets=None, n_models_to_use: int = 0, length_scale: float = 1.0,
+                  flags: int = 0):
+        """nnp_create_from_file: a handle from a parameter file; atoms are named by atomic number."""
+        self = cls.__new__(cls)
+        self.lib = load_library()
+        z = np.ascontiguousarray(atomic_numbers, dtype=np.int32)
+        self.n_atoms = int(z.size)
+        off = None
+        self.n_molecules = 1
+        if mol_offsets is not None:
+            off = np.ascontiguousarray(mol_offsets, dtype=np.int32)
+            self.n_molecules = int(off.size - 1)
+        h = C.c_void_p()
+        rc = self.lib.nnp_create_from_file(C.byref(h), os.fsencode(path), self.n_atoms, z.ctypes.data if z.size else None,
+                                           self.n_molecules, off.ctypes.data if off is not None else None,
+                                           int(n_models_to_use), float(length_scale), int(flags))
+        _check(rc, "nnp_create_from_file")
+        self.h = h
+        self.n_features = int(self.lib.nnp_n_features(self.h))
+        self.n_models = int(n_models_to_use) if n_models_to_use else read_parameter_file_header(path)["n_models"]
+        return self
+
     # ---- the hot path
+    def compute_fixed(self, d_pos: int, pos_stride: int, d_atom_index, d_energy: int, d_force_fixed, force_stride: int,
+                      stream: int = 0):
+        """nnp_compute_fixed: forces added as round(F * 2^32) into an int64 buffer with integer atomics."""
+        _check(self.lib.nnp_compute_fixed(self.h, d_pos, pos_stride, d_atom_index, d_energy, d_force_fixed, force_stride,
+                                          stream or None), "nnp_compute_fixed")
+
+    def compute_async(self, d_pos: int, pos_stride: int, d_atom_index, d_energy: int, d_force, force_stride: int,
+                      fixed: bool, wait_event=None, done_event=None):
+        """nnp_compute_async: on the library's own stream, ordered by CUDA events (raw cudaEvent_t values)."""
+        _check(self.lib.nnp_compute_async(self.h, d_pos, pos_stride, d_atom_index, d_energy, d_force, force_stride,
+                                          1 if fixed else 0, wait_event, done_event), "nnp_compute_async")
+
     def compute(self, d_pos: int, pos_stride: int, d_atom_index, d_energy: int, d_force, force_stride: int,
                 stream: int = 0):
         """nnp_compute with raw device addresses (ints)."""
@@ -280,3 +337,89 @@ class NNP:
             self.destroy()
         except Exception:
             pass
+
+
+def measure_peaks():
+    """nnp_measure_peaks: dict of what the device sustains (FP32 FFMA, tcgen05 TF32, L2 reads, DRAM reads)."""
+    lib = load_library()
+    out = np.zeros(4, dtype=np.float64)
+    _check(lib.nnp_measure_peaks(out.ctypes.data, 4), "nnp_measure_peaks")
+    return {"fp32_ffma_tflops": float(out[0]), "tf32_tcgen05_tflops": float(out[1]), "l2_read_gbs": float(out[2]),
+            "dram_read_gbs": float(out[3])}
+
+
+class Coupling:
+    """One nnp_coupling handle: the NNP-MM coupling term of mechanical embedding (Eq. 4)."""
+
+    def __init__(self, nnp_rows, q_nnp, sigma_nnp, eps_nnp, mm_rows, q_mm, sigma_mm, eps_mm, coulomb_const: float,
+                 cutoff: float = 0.0, length_scale: float = 1.0):
+        self.lib = load_library()
+        i32 = lambda v: np.ascontiguousarray(v, dtype=np.int32)
+        f32 = lambda v: np.ascontiguousarray(v, dtype=np.float32)
+        a = [i32(nnp_rows), f32(q_nnp), f32(sigma_nnp), f32(eps_nnp), i32(mm_rows), f32(q_mm), f32(sigma_mm), f32(eps_mm)]
+        self.n_nnp, self.n_mm = int(a[0].size), int(a[4].size)
+        p = [x.ctypes.data if x.size else None for x in a]
+        h = C.c_void_p()
+        _check(self.lib.nnp_coupling_create(C.byref(h), self.n_nnp, p[0], p[1], p[2], p[3], self.n_mm, p[4], p[5], p[6],
+                                            p[7], float(coulomb_const), float(cutoff), float(length_scale)),
+               "nnp_coupling_create")
+        self.h = h
+
+    def compute(self, d_pos: int, pos_stride: int, d_energy, d_force, force_stride: int, stream: int = 0, fixed: bool = False):
+        fn = self.lib.nnp_coupling_compute_fixed if fixed else self.lib.nnp_coupling_compute
+        _check(fn(self.h, d_pos, pos_stride, d_energy, d_force, force_stride, stream or None), "nnp_coupling_compute")
+
+    def destroy(self):
+        if getattr(self, "h", None) is not None and self.h:
+            self.lib.nnp_coupling_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+# ------------------------------------------------------------------------------------------------
+# parameter files (format: csrc/params_file.cu).  Pure byte marshalling: nothing of the method is computed here.
+PARAM_MAGIC = b"NNPB200P"
+
+
+def write_parameter_file(path: str, params, weights, biases, atomic_numbers, self_energy=None, energy_scale=None):
+    """Write an ANI-style parameter set (any species order: `atomic_numbers[s]` is the element of species s)."""
+    S = int(params.n_species)
+    M = len(weights)
+    dims = np.ascontiguousarray(params.layer_dims, dtype="<i4")
+    L = dims.shape[1] - 1
+    z = np.ascontiguousarray(atomic_numbers, dtype="<i4")
+    assert z.size == S
+    se = np.zeros(S, "<f8") if self_energy is None else np.ascontiguousarray(self_energy, dtype="<f8")
+    f4 = lambda v: np.ascontiguousarray(v, dtype="<f4")
+    with open(path, "wb") as f:
+        f.write(PARAM_MAGIC)
+        f.write(np.array([1, S, M, L], "<i4").tobytes())
+        f.write(f4([params.rc_radial, params.rc_angular, params.eta_r, params.eta_a, params.zeta, params.cos_scale,
+                    params.celu_alpha]).tobytes())
+        f.write(np.array([params.shf_r.size, params.shf_a.size, params.shf_z.size], "<i4").tobytes())
+        f.write(np.array([params.energy_scale if energy_scale is None else energy_scale], "<f8").tobytes())
+        f.write(z.tobytes())
+        for v in (params.shf_r, params.shf_a, params.shf_z):
+            f.write(f4(v).tobytes())
+        f.write(dims.tobytes())
+        f.write(se.tobytes())
+        for m in range(M):
+            for e in range(S):
+                for l in range(L):
+                    w = f4(weights[m][e][l])
+                    assert w.shape == (dims[e, l + 1], dims[e, l])
+                    f.write(w.tobytes())
+                    b = np.zeros(dims[e, l + 1], "<f4") if biases is None else f4(biases[m][e][l])
+                    f.write(b.tobytes())
+
+
+def read_parameter_file_header(path: str):
+    with open(path, "rb") as f:
+        assert f.read(8) == PARAM_MAGIC
+        version, S, M, L = np.frombuffer(f.read(16), "<i4")
+    return {"version": int(version), "n_species": int(S), "n_models": int(M), "n_layers": int(L)}

@@ -709,7 +709,7 @@ constexpr int FIN_WARPS = FIN_THREADS / 32;
 
 __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(
     const int* __restrict__ nbr_r, const int* __restrict__ cnt_r, const float* __restrict__ phi, int N, int capR,
-    const int* __restrict__ atom_index, float* __restrict__ force, int force_stride, float fscale,
+    const int* __restrict__ atom_index, void* __restrict__ force, int force_stride, int fixed, float fscale,
     int n_force_blocks, const double* __restrict__ eatom, const int* __restrict__ sortpos,
     const int* __restrict__ species, const int* __restrict__ mol_off, int n_mol, int M,
     const double* __restrict__ self_energy, double escale, double* __restrict__ energy,
@@ -744,10 +744,21 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(
     fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
     if (lane == 0) {
       const int row = atom_index ? atom_index[a] : a;
-      float* f = force + (size_t)row * force_stride;
-      f[0] += fscale * fx;
-      f[1] += fscale * fy;
-      f[2] += fscale * fz;
+      if (fixed) {
+        // 64-bit fixed point (2^32 per force unit, the accumulation format of GPU MD engines): integer atomic adds
+        // commute, so MM kernels running CONCURRENTLY may add into the same buffer and the sum has the same bits in
+        // any order (NNP and MM concurrently instead of sequentially)
+        unsigned long long* f = reinterpret_cast<unsigned long long*>(force) + (size_t)row * force_stride;
+        const double sc = (double)fscale * 4294967296.0;
+        atomicAdd(f + 0, (unsigned long long)__double2ll_rn(sc * (double)fx));
+        atomicAdd(f + 1, (unsigned long long)__double2ll_rn(sc * (double)fy));
+        atomicAdd(f + 2, (unsigned long long)__double2ll_rn(sc * (double)fz));
+      } else {  // plain read-modify-write: safe only when every other adder is ordered with this stream
+        float* f = reinterpret_cast<float*>(force) + (size_t)row * force_stride;
+        f[0] += fscale * fx;
+        f[1] += fscale * fy;
+        f[2] += fscale * fz;
+      }
     }
   } else {
     // energy blocks: a CTA sums a chunk of a molecule (thread-strided atoms, warp tree, then the warps in order).  A
@@ -865,14 +876,14 @@ void launch_aev_backward(nnp_handle* h, cudaStream_t s) {
   }
 }
 
-void launch_finish(nnp_handle* h, const int* d_atom_index, double* d_energy, float* d_force, int force_stride,
+void launch_finish(nnp_handle* h, const int* d_atom_index, double* d_energy, void* d_force, int force_stride, int fixed,
                    cudaStream_t s) {
   if (h->N == 0) return;
   const int nfb = (h->N + FIN_WARPS - 1) / FIN_WARPS;
   const int neb = h->n_eblocks;
   const float fscale = (float)(h->energy_scale * h->length_scale);
   launch_kernel(h->pdl_now, finish_kernel, dim3(nfb + neb), dim3(FIN_THREADS), 0, s, h->d_nbr_r, h->d_cnt_r, h->d_phi,
-                h->N, h->capR, d_atom_index, d_force, force_stride, fscale, nfb, h->d_eatom, h->d_sortpos, h->d_species,
+                h->N, h->capR, d_atom_index, d_force, force_stride, fixed, fscale, nfb, h->d_eatom, h->d_sortpos, h->d_species,
                 h->d_mol_off, h->n_mol, h->M, h->d_self_energy, h->energy_scale, d_energy,
                 (const EnergyBlock*)h->d_eblocks, h->n_eblocks, h->d_epart, h->d_ecount);
 }

@@ -1,0 +1,239 @@
+// NNP-MM coupling term of mechanical embedding (Eq. 4) on the device:
+//   V = sum_{i in NNP} sum_{j in MM} [ kc q_i q_j / r_ij + 4 eps_ij ((sigma_ij/r_ij)^12 - (sigma_ij/r_ij)^6) ],
+// forces on the atoms of BOTH regions added into the caller's force buffer (the same buffer nnp_compute adds
+// into).  Readings C1-C4 of DESIGN.md: Lorentz-Berthelot mixing, caller-supplied Coulomb constant, optional
+// inclusive plain cutoff on D2 = (dx dx + dy dy) + dz dz evaluated in binary64 without contraction (the same
+// predicate as the neighbour search, so the pair set equals the oracle's), no periodic images.
+//
+// The NNP region is small (48-75 atoms in the paper's systems) and the MM region large, so the
+// work is O(N_NNP N_MM) distance tests of which a few per cent pass a 9 A cutoff.  Two launches, no float atomics,
+// fixed summation orders (bit-identical reruns):
+//   coupling_mm_kernel   one thread per MM atom j, NNP atoms staged in shared memory: F_j and the pair energies
+//   coupling_nnp_kernel  one CTA per NNP atom i, threads stride over the MM atoms: F_i; CTA 0 also adds the
+//                        per-CTA energy partials of the first kernel in index order
+// Every pair inside the cutoff is therefore evaluated twice, which costs less than a float-atomic-free transpose
+// of the pair forces.  Arithmetic is FP64 (the work is tiny; B200 has full-rate FP64 FMA) so that parity with the
+// float64 oracle is at rounding level; the force increments are rounded once when they are added to the buffer.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include <new>
+#include <vector>
+
+#include "nnp.h"
+
+namespace {
+
+constexpr int CP_THREADS = 256;
+
+struct CpAtom {  // an atom of either list: row in the caller's buffers and its parameters
+  int row;
+  float q, sigma, eps;
+};
+
+struct CpArgs {
+  const CpAtom* nnp;
+  const CpAtom* mm;
+  int n_nnp, n_mm;
+  double kc, rc2, length_scale;  // rc2 <= 0: no cutoff
+};
+
+__device__ __forceinline__ void load_pos(const float* pos, int stride, int row, double ls, double& x, double& y, double& z) {
+  const float* p = pos + (size_t)row * stride;
+  // caller length unit -> A with one f32 multiply, as nnp_compute does, so a caller working in nm sees the same bits
+  const float fl = (float)ls;
+  x = (double)(p[0] * fl); y = (double)(p[1] * fl); z = (double)(p[2] * fl);
+}
+
+// pair (NNP atom a, MM atom b) with d = r_b - r_a: energy and dV/dr / r ("g": F_b = -g d, F_a = +g d)
+__device__ __forceinline__ bool pair_terms(const CpArgs& A, double dx, double dy, double dz, float qa, float sa, float ea,
+                                           float qb, float sb, float eb, double& v, double& g) {
+  const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+  if (A.rc2 > 0.0 && d2 > A.rc2) return false;
+  const double r = sqrt(d2), inv = 1.0 / r;
+  const double sigma = 0.5 * ((double)sa + (double)sb);
+  const double eps = sqrt((double)ea * (double)eb);
+  const double s = sigma * inv, s2 = s * s, s6 = s2 * s2 * s2, s12 = s6 * s6;
+  const double vc = A.kc * (double)qa * (double)qb * inv;
+  v = vc + 4.0 * eps * (s12 - s6);
+  g = (-vc + 4.0 * eps * (-12.0 * s12 + 6.0 * s6)) * inv * inv;  // (dV/dr) / r
+  return true;
+}
+
+__device__ __forceinline__ double block_sum(double v, double* red) {  // fixed tree; result valid in thread 0
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  const int w = threadIdx.x >> 5;
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) red[w] = v;
+  __syncthreads();
+  double t = 0.0;
+  if (threadIdx.x == 0)
+    for (int k = 0; k < CP_THREADS / 32; ++k) t += red[k];
+  return t;
+}
+
+// add a force increment (output energy unit per caller length unit) into the caller's buffer
+__device__ __forceinline__ void add_force(void* buf, int stride, int row, int fixed, double fx, double fy, double fz) {
+  if (fixed) {  // 64-bit fixed point, 2^32 per unit: integer atomics commute, so concurrent adders give the same bits
+    unsigned long long* f = reinterpret_cast<unsigned long long*>(buf) + (size_t)row * stride;
+    atomicAdd(f + 0, (unsigned long long)__double2ll_rn(fx * 4294967296.0));
+    atomicAdd(f + 1, (unsigned long long)__double2ll_rn(fy * 4294967296.0));
+    atomicAdd(f + 2, (unsigned long long)__double2ll_rn(fz * 4294967296.0));
+  } else {
+    float* f = reinterpret_cast<float*>(buf) + (size_t)row * stride;
+    f[0] += (float)fx; f[1] += (float)fy; f[2] += (float)fz;
+  }
+}
+
+__global__ void __launch_bounds__(CP_THREADS) coupling_mm_kernel(const __grid_constant__ CpArgs A, const float* __restrict__ pos,
+                                                                  int pos_stride, void* force, int force_stride, int fixed,
+                                                                  double* __restrict__ e_part) {
+  __shared__ double sx[CP_THREADS], sy[CP_THREADS], sz[CP_THREADS];
+  __shared__ float sq[CP_THREADS], ss[CP_THREADS], se[CP_THREADS];
+  __shared__ double red[CP_THREADS / 32];
+  const int j = blockIdx.x * CP_THREADS + threadIdx.x;
+  const bool live = j < A.n_mm;
+  CpAtom b = live ? A.mm[j] : CpAtom{0, 0.f, 0.f, 0.f};
+  double bx = 0, by = 0, bz = 0;
+  if (live) load_pos(pos, pos_stride, b.row, A.length_scale, bx, by, bz);
+  double fx = 0, fy = 0, fz = 0, e = 0;
+  for (int i0 = 0; i0 < A.n_nnp; i0 += CP_THREADS) {
+    const int n = min(CP_THREADS, A.n_nnp - i0);
+    __syncthreads();
+    if ((int)threadIdx.x < n) {
+      const CpAtom a = A.nnp[i0 + threadIdx.x];
+      load_pos(pos, pos_stride, a.row, A.length_scale, sx[threadIdx.x], sy[threadIdx.x], sz[threadIdx.x]);
+      sq[threadIdx.x] = a.q; ss[threadIdx.x] = a.sigma; se[threadIdx.x] = a.eps;
+    }
+    __syncthreads();
+    if (live)
+      for (int i = 0; i < n; ++i) {  // NNP atoms in index order
+        const double dx = bx - sx[i], dy = by - sy[i], dz = bz - sz[i];
+        double v, g;
+        if (pair_terms(A, dx, dy, dz, sq[i], ss[i], se[i], b.q, b.sigma, b.eps, v, g)) {
+          e += v;
+          fx -= g * dx; fy -= g * dy; fz -= g * dz;
+        }
+      }
+  }
+  if (live && force && (fx != 0.0 || fy != 0.0 || fz != 0.0))
+    add_force(force, force_stride, b.row, fixed, fx * A.length_scale, fy * A.length_scale, fz * A.length_scale);
+  const double t = block_sum(e, red);
+  if (threadIdx.x == 0) e_part[blockIdx.x] = t;
+}
+
+__global__ void __launch_bounds__(CP_THREADS) coupling_nnp_kernel(const __grid_constant__ CpArgs A, const float* __restrict__ pos,
+                                                                   int pos_stride, void* force, int force_stride, int fixed,
+                                                                   const double* __restrict__ e_part, int n_part,
+                                                                   double* __restrict__ energy) {
+  __shared__ double red[CP_THREADS / 32];
+  const int i = blockIdx.x;
+  if (i < A.n_nnp) {
+    const CpAtom a = A.nnp[i];
+    double ax, ay, az;
+    load_pos(pos, pos_stride, a.row, A.length_scale, ax, ay, az);
+    double fx = 0, fy = 0, fz = 0;
+    for (int j = threadIdx.x; j < A.n_mm; j += CP_THREADS) {
+      const CpAtom b = A.mm[j];
+      double bx, by, bz;
+      load_pos(pos, pos_stride, b.row, A.length_scale, bx, by, bz);
+      const double dx = bx - ax, dy = by - ay, dz = bz - az;
+      double v, g;
+      if (pair_terms(A, dx, dy, dz, a.q, a.sigma, a.eps, b.q, b.sigma, b.eps, v, g)) {
+        fx += g * dx; fy += g * dy; fz += g * dz;
+      }
+    }
+    const double tx = block_sum(fx, red), ty = block_sum(fy, red), tz = block_sum(fz, red);
+    if (threadIdx.x == 0 && force)
+      add_force(force, force_stride, a.row, fixed, tx * A.length_scale, ty * A.length_scale, tz * A.length_scale);
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0 && energy) {
+    double t = 0.0;
+    for (int k = 0; k < n_part; ++k) t += e_part[k];
+    *energy = t;
+  }
+}
+
+}  // namespace
+
+struct nnp_coupling {
+  int device = 0;
+  CpArgs args;
+  CpAtom *d_nnp = nullptr, *d_mm = nullptr;
+  double* d_epart = nullptr;
+  int n_part = 0;
+};
+
+extern "C" void nnp_coupling_destroy(nnp_coupling* c) {
+  if (!c) return;
+  cudaSetDevice(c->device);
+  cudaDeviceSynchronize();
+  if (c->d_nnp) cudaFree(c->d_nnp);
+  if (c->d_mm) cudaFree(c->d_mm);
+  if (c->d_epart) cudaFree(c->d_epart);
+  delete c;
+}
+
+extern "C" int nnp_coupling_create(nnp_coupling** out, int32_t n_nnp, const int32_t* nnp_rows_host, const float* q_nnp_host,
+                                   const float* sigma_nnp_host, const float* eps_nnp_host, int32_t n_mm,
+                                   const int32_t* mm_rows_host, const float* q_mm_host, const float* sigma_mm_host,
+                                   const float* eps_mm_host, double coulomb_const, double cutoff, double length_scale) {
+  if (!out) return NNP_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (n_nnp < 0 || n_mm < 0 || !(length_scale > 0.0)) return NNP_ERR_INVALID_ARG;
+  if (n_nnp > 0 && (!nnp_rows_host || !q_nnp_host || !sigma_nnp_host || !eps_nnp_host)) return NNP_ERR_INVALID_ARG;
+  if (n_mm > 0 && (!mm_rows_host || !q_mm_host || !sigma_mm_host || !eps_mm_host)) return NNP_ERR_INVALID_ARG;
+  for (int i = 0; i < n_nnp; ++i)
+    if (nnp_rows_host[i] < 0 || eps_nnp_host[i] < 0.f) return NNP_ERR_INVALID_ARG;
+  for (int j = 0; j < n_mm; ++j)
+    if (mm_rows_host[j] < 0 || eps_mm_host[j] < 0.f) return NNP_ERR_INVALID_ARG;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return NNP_ERR_CUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return NNP_ERR_CUDA;
+  if (prop.major != 10) return NNP_ERR_UNSUPPORTED_ARCH;
+  nnp_coupling* c = new (std::nothrow) nnp_coupling();
+  if (!c) return NNP_ERR_ALLOC;
+  c->device = dev;
+  std::vector<CpAtom> a(n_nnp), b(n_mm);
+  for (int i = 0; i < n_nnp; ++i) a[i] = CpAtom{nnp_rows_host[i], q_nnp_host[i], sigma_nnp_host[i], eps_nnp_host[i]};
+  for (int j = 0; j < n_mm; ++j) b[j] = CpAtom{mm_rows_host[j], q_mm_host[j], sigma_mm_host[j], eps_mm_host[j]};
+  c->n_part = (n_mm + CP_THREADS - 1) / CP_THREADS;
+  bool ok = cudaMalloc((void**)&c->d_nnp, sizeof(CpAtom) * (size_t)(n_nnp > 0 ? n_nnp : 1)) == cudaSuccess &&
+            cudaMalloc((void**)&c->d_mm, sizeof(CpAtom) * (size_t)(n_mm > 0 ? n_mm : 1)) == cudaSuccess &&
+            cudaMalloc((void**)&c->d_epart, sizeof(double) * (size_t)(c->n_part > 0 ? c->n_part : 1)) == cudaSuccess;
+  if (ok && n_nnp) ok = cudaMemcpy(c->d_nnp, a.data(), sizeof(CpAtom) * (size_t)n_nnp, cudaMemcpyHostToDevice) == cudaSuccess;
+  if (ok && n_mm) ok = cudaMemcpy(c->d_mm, b.data(), sizeof(CpAtom) * (size_t)n_mm, cudaMemcpyHostToDevice) == cudaSuccess;
+  if (!ok) {
+    nnp_coupling_destroy(c);
+    return NNP_ERR_ALLOC;
+  }
+  c->args = CpArgs{c->d_nnp, c->d_mm, n_nnp, n_mm, coulomb_const, cutoff > 0.0 ? cutoff * cutoff : 0.0, length_scale};
+  *out = c;
+  return NNP_OK;
+}
+
+static int coupling_enqueue(nnp_coupling* c, const float* d_pos, int ps, double* d_energy, void* d_force, int fs, int fixed,
+                            cudaStream_t s) {
+  if (!c || !d_pos || ps < 3 || (d_force && fs < 3)) return NNP_ERR_INVALID_ARG;
+  if (c->args.n_mm > 0)
+    coupling_mm_kernel<<<c->n_part, CP_THREADS, 0, s>>>(c->args, d_pos, ps, d_force, fs, fixed, c->d_epart);
+  coupling_nnp_kernel<<<c->args.n_nnp > 0 ? c->args.n_nnp : 1, CP_THREADS, 0, s>>>(c->args, d_pos, ps, d_force, fs, fixed,
+                                                                                   c->d_epart, c->args.n_mm > 0 ? c->n_part : 0,
+                                                                                   d_energy);
+  return cudaGetLastError() == cudaSuccess ? NNP_OK : NNP_ERR_CUDA;
+}
+
+extern "C" int nnp_coupling_compute(nnp_coupling* c, const float* d_pos, int32_t pos_stride_floats, double* d_energy,
+                                    float* d_force_accum, int32_t force_stride_floats, void* cuda_stream) {
+  return coupling_enqueue(c, d_pos, pos_stride_floats, d_energy, d_force_accum, force_stride_floats, 0,
+                          (cudaStream_t)cuda_stream);
+}
+
+extern "C" int nnp_coupling_compute_fixed(nnp_coupling* c, const float* d_pos, int32_t pos_stride_floats, double* d_energy,
+                                          int64_t* d_force_fixed, int32_t force_stride_int64, void* cuda_stream) {
+  return coupling_enqueue(c, d_pos, pos_stride_floats, d_energy, d_force_fixed, force_stride_int64, 1,
+                          (cudaStream_t)cuda_stream);
+}

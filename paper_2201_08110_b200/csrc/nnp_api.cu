@@ -63,7 +63,9 @@ extern "C" void nnp_destroy(nnp_handle* h) {
   cudaSetDevice(h->device);
   if (h->last_stream) cudaStreamSynchronize(h->last_stream);
   cudaDeviceSynchronize();
-  if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+  for (auto& g : h->graphs)
+    if (g.exec) cudaGraphExecDestroy(g.exec);
+  if (h->own_stream) cudaStreamDestroy(h->own_stream);
   for (auto e : h->events) cudaEventDestroy(e);
   void* ptrs[] = {h->d_eblocks, h->d_epart, h->d_ecount, h->d_mol_range, h->d_species, h->d_mol_off, h->d_mol_id, h->d_sortpos, h->d_perm, h->d_grp_off, h->d_self_energy,
                   h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_aev, h->d_daev, h->d_phi,
@@ -817,7 +819,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
 
 // enqueue the launch chain A1..A8 on `s`; with `ev` record an event before the first and after each stage
 static void enqueue_chain(nnp_handle* h, const float* d_pos, int ps, const int* d_idx, double* d_energy,
-                          float* d_force, int fs, cudaStream_t s, bool ev) {
+                          void* d_force, int fs, int fixed, cudaStream_t s, bool ev) {
   int k = 0;
   auto mark = [&]() {
     if (ev) cudaEventRecord(h->events[k], s);
@@ -833,7 +835,7 @@ static void enqueue_chain(nnp_handle* h, const float* d_pos, int ps, const int* 
     if (h->use_mid) { mid_launch(h->smid, s, pdl); mark(); }
     for (auto& g : h->sbwd) { small_launch_bwd(g, s, pdl); mark(); }
     launch_aev_backward(h, s); mark();
-    launch_finish(h, d_idx, d_energy, d_force, fs, s); mark();
+    launch_finish(h, d_idx, d_energy, d_force, fs, fixed, s); mark();
     return;
   }
   if (h->use_umma) {
@@ -848,32 +850,37 @@ static void enqueue_chain(nnp_handle* h, const float* d_pos, int ps, const int* 
     for (auto& g : h->bwd) { launch_gemm(g, s); mark(); }
   }
   launch_aev_backward(h, s); mark();
-  launch_finish(h, d_idx, d_energy, d_force, fs, s); mark();
+  launch_finish(h, d_idx, d_energy, d_force, fs, fixed, s); mark();
 }
 
-extern "C" int nnp_compute(nnp_handle* h, const float* d_pos, int32_t pos_stride_floats,
-                           const int32_t* d_atom_index, double* d_energy, float* d_force_accum,
-                           int32_t force_stride_floats, void* cuda_stream) {
+static int compute_impl(nnp_handle* h, const float* d_pos, int ps, const int* d_atom_index, double* d_energy, void* d_force,
+                        int fs, int fixed, cudaStream_t s) {
   if (!h) return NNP_ERR_INVALID_ARG;
   if (h->N == 0) {  // no atoms: every (empty) molecule has energy 0; d_energy is WRITTEN as documented
-    if (d_energy) CK(cudaMemsetAsync(d_energy, 0, sizeof(double) * (size_t)h->n_mol, (cudaStream_t)cuda_stream));
-    h->last_stream = (cudaStream_t)cuda_stream;
+    if (d_energy) CK(cudaMemsetAsync(d_energy, 0, sizeof(double) * (size_t)h->n_mol, s));
+    h->last_stream = s;
     return NNP_OK;
   }
-  if (!d_pos || pos_stride_floats < 3 || (d_force_accum && force_stride_floats < 3)) return NNP_ERR_INVALID_ARG;
-  cudaStream_t s = (cudaStream_t)cuda_stream;
+  if (!d_pos || ps < 3 || (d_force && fs < 3)) return NNP_ERR_INVALID_ARG;
   h->last_stream = s;
   if (h->profiling || (h->flags & NNP_FLAG_NO_GRAPH)) {
-    enqueue_chain(h, d_pos, pos_stride_floats, d_atom_index, d_energy, d_force_accum, force_stride_floats, s,
-                  h->profiling);
+    enqueue_chain(h, d_pos, ps, d_atom_index, d_energy, d_force, fs, fixed, s, h->profiling);
     return cudaGetLastError() == cudaSuccess ? NNP_OK : NNP_ERR_CUDA;
   }
-  const bool same = h->graph_exec && h->g_pos == d_pos && h->g_idx == d_atom_index && h->g_energy == d_energy &&
-                    h->g_force == d_force_accum && h->g_ps == pos_stride_floats && h->g_fs == force_stride_floats;
-  if (!same) {
-    if (h->graph_exec) {
-      cudaGraphExecDestroy(h->graph_exec);
-      h->graph_exec = nullptr;
+  nnp_handle::GraphSlot* slot = nullptr;
+  for (auto& g : h->graphs)
+    if (g.exec && g.pos == d_pos && g.idx == d_atom_index && g.energy == d_energy && g.force == d_force && g.ps == ps &&
+        g.fs == fs && g.fixed == fixed)
+      slot = &g;
+  if (!slot) {
+    slot = &h->graphs[0];  // a free entry, else the least recently used one
+    for (auto& g : h->graphs) {
+      if (!g.exec) { slot = &g; break; }
+      if (g.used < slot->used) slot = &g;
+    }
+    if (slot->exec) {
+      cudaGraphExecDestroy(slot->exec);
+      slot->exec = nullptr;
     }
     cudaStream_t cs;
     CK(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
@@ -882,20 +889,48 @@ extern "C" int nnp_compute(nnp_handle* h, const float* d_pos, int32_t pos_stride
       cudaStreamDestroy(cs);
       return NNP_ERR_CUDA;
     }
-    enqueue_chain(h, d_pos, pos_stride_floats, d_atom_index, d_energy, d_force_accum, force_stride_floats, cs, false);
+    enqueue_chain(h, d_pos, ps, d_atom_index, d_energy, d_force, fs, fixed, cs, false);
     cudaError_t e = cudaStreamEndCapture(cs, &graph);
     cudaStreamDestroy(cs);
     if (e != cudaSuccess || !graph) return NNP_ERR_CUDA;
-    e = cudaGraphInstantiate(&h->graph_exec, graph, 0);
+    e = cudaGraphInstantiate(&slot->exec, graph, 0);
     cudaGraphDestroy(graph);
     if (e != cudaSuccess) {
-      h->graph_exec = nullptr;
+      slot->exec = nullptr;
       return NNP_ERR_CUDA;
     }
-    h->g_pos = d_pos; h->g_idx = d_atom_index; h->g_energy = d_energy; h->g_force = d_force_accum;
-    h->g_ps = pos_stride_floats; h->g_fs = force_stride_floats;
+    slot->pos = d_pos; slot->idx = d_atom_index; slot->energy = d_energy; slot->force = d_force;
+    slot->ps = ps; slot->fs = fs; slot->fixed = fixed;
   }
-  CK(cudaGraphLaunch(h->graph_exec, s));
+  slot->used = ++h->graph_clock;
+  CK(cudaGraphLaunch(slot->exec, s));
+  return NNP_OK;
+}
+
+extern "C" int nnp_compute(nnp_handle* h, const float* d_pos, int32_t pos_stride_floats,
+                           const int32_t* d_atom_index, double* d_energy, float* d_force_accum,
+                           int32_t force_stride_floats, void* cuda_stream) {
+  return compute_impl(h, d_pos, pos_stride_floats, d_atom_index, d_energy, d_force_accum, force_stride_floats, 0,
+                      (cudaStream_t)cuda_stream);
+}
+
+extern "C" int nnp_compute_fixed(nnp_handle* h, const float* d_pos, int32_t pos_stride_floats,
+                                 const int32_t* d_atom_index, double* d_energy, int64_t* d_force_fixed,
+                                 int32_t force_stride_int64, void* cuda_stream) {
+  return compute_impl(h, d_pos, pos_stride_floats, d_atom_index, d_energy, d_force_fixed, force_stride_int64, 1,
+                      (cudaStream_t)cuda_stream);
+}
+
+extern "C" int nnp_compute_async(nnp_handle* h, const float* d_pos, int32_t pos_stride_floats,
+                                 const int32_t* d_atom_index, double* d_energy, void* d_force, int32_t force_stride,
+                                 int32_t force_is_fixed64, void* wait_event, void* done_event) {
+  if (!h) return NNP_ERR_INVALID_ARG;
+  if (!h->own_stream) CK(cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking));
+  if (wait_event) CK(cudaStreamWaitEvent(h->own_stream, (cudaEvent_t)wait_event, 0));
+  const int rc = compute_impl(h, d_pos, pos_stride_floats, d_atom_index, d_energy, d_force, force_stride,
+                              force_is_fixed64 ? 1 : 0, h->own_stream);
+  if (rc != NNP_OK) return rc;
+  if (done_event) CK(cudaEventRecord((cudaEvent_t)done_event, h->own_stream));
   return NNP_OK;
 }
 

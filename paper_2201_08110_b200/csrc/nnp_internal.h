@@ -294,13 +294,20 @@ struct nnp_handle {
   // host staging for nnp_compute_host
   float *d_hpos = nullptr, *d_hforce = nullptr;
   double* d_henergy = nullptr;
-  // graph
-  cudaGraphExec_t graph_exec = nullptr;
-  const void* g_pos = nullptr;
-  const void* g_idx = nullptr;
-  void *g_energy = nullptr, *g_force = nullptr;
-  int g_ps = 0, g_fs = 0;
+  // graphs: one instantiated graph per distinct argument tuple, a small LRU (an engine that double-buffers its
+  // positions or forces alternates between two of them at no cost)
+  struct GraphSlot {
+    cudaGraphExec_t exec = nullptr;
+    const void* pos = nullptr;
+    const void* idx = nullptr;
+    void *energy = nullptr, *force = nullptr;
+    int ps = 0, fs = 0, fixed = 0;
+    unsigned long long used = 0;
+  };
+  GraphSlot graphs[4];
+  unsigned long long graph_clock = 0;
   cudaStream_t last_stream = nullptr;
+  cudaStream_t own_stream = nullptr;  // nnp_compute_async: library-owned stream
   // profiling
   bool profiling = false;
   std::vector<cudaEvent_t> events;
@@ -318,7 +325,7 @@ void launch_aev_forward(nnp_handle* h, const float* d_pos, int pos_stride, const
 void launch_aev_backward(nnp_handle* h, cudaStream_t s);
 void launch_gemm(const GemmLaunch& g, cudaStream_t s);
 void launch_last_layer(nnp_handle* h, cudaStream_t s);
-void launch_finish(nnp_handle* h, const int* d_atom_index, double* d_energy, float* d_force, int force_stride,
+void launch_finish(nnp_handle* h, const int* d_atom_index, double* d_energy, void* d_force, int force_stride, int fixed,
                    cudaStream_t s);
 size_t aev_smem_bytes(const nnp_handle* h, bool backward);
 void build_gemm_tiles(const std::vector<GemmProblem>& probs, std::vector<GemmTile>& tiles);

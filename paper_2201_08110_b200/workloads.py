@@ -413,3 +413,41 @@ def coupling_system(n_mm: int = 30000, seed: int = BASE_SEED + 77, density: floa
     f32 = lambda lo, hi, n: rng.uniform(lo, hi, size=n).astype(np.float32)
     return CouplingSystem(pos, nnp_rows, mm_rows, f32(-0.6, 0.6, n_nnp), f32(1.0, 3.6, n_nnp), f32(0.01, 0.25, n_nnp),
                           f32(-0.9, 0.9, n_mm), f32(0.4, 3.6, n_mm), f32(0.0, 0.25, n_mm))
+
+
+# ------------------------------------------------------------------------------------------------
+# ANI-1x as a second parameter set (Table 4: "ANI-1x" on the 3BE9 ligand): 4 elements H, C, N, O ->
+# 4*16 + 10*32 = 384 features, its own AEV constants and narrower networks.  Values: the published ANI-1x
+# hyper-parameters; trained weights are not in this container (seeded Xavier weights stand in, as for ANI-2x).
+ANI1X_ATOMIC_NUMBERS = (1, 6, 7, 8)
+ANI2X_ATOMIC_NUMBERS = (1, 6, 7, 8, 9, 16, 17)
+
+
+def ani1x_params() -> AniParams:
+    f32 = np.float32
+    hidden = {"H": (160, 128, 96), "C": (144, 112, 96), "N": (128, 112, 96), "O": (128, 112, 96)}
+    n_feat = 4 * 16 + 10 * 32
+    dims = np.array([[n_feat, *hidden[s], 1] for s in ("H", "C", "N", "O")], dtype=np.int32)
+    return AniParams(
+        n_species=4,
+        rc_radial=f32(5.2),
+        rc_angular=f32(3.5),
+        eta_r=f32(16.0),
+        shf_r=(0.9 + 0.26875 * np.arange(16, dtype=np.float64)).astype(f32),
+        eta_a=f32(8.0),
+        zeta=f32(32.0),
+        shf_a=(0.9 + 0.65 * np.arange(4, dtype=np.float64)).astype(f32),
+        shf_z=((2.0 * np.arange(8, dtype=np.float64) + 1.0) * math.pi / 16.0).astype(f32),
+        cos_scale=f32(0.95),
+        celu_alpha=f32(0.1),
+        layer_dims=dims,
+        energy_scale=627.5094740631,
+    )
+
+
+def ani1x_ligand(n: int = 48, n_models: int = 8) -> Workload:
+    """A 3BE9-ligand-sized region (48 atoms) of H/C/N/O at 50/30/10/10 % in a ball of radius 6 A."""
+    b = BASE_SEED + 60
+    pos = place_in_ball(np.random.default_rng(b), n, 6.0)
+    spc = make_species(n, (0.5, 0.3, 0.1, 0.1), b + 1)
+    return Workload(f"ani1x_ligand{n}", 0, pos, spc, np.array([0, n], np.int32), n_models, 100, b + 2, b + 3, ani1x_params())
