@@ -200,6 +200,10 @@ const char *nnp_stage_name(nnp_handle *h, int32_t stage);
  * what[0] = weight bytes the MLP layers must read once, what[1] = MLP flops (2 per MAC, forward +
  * input-gradient backward), what[2] = AEV bytes (write+read), what[3] = layer-1 weight bytes. */
 int nnp_get_work(nnp_handle *h, double *what_host, int32_t n);
+/* Per stage (index as in nnp_stage_name): for a tensor-engine launch the flops it actually issues (2 per MAC of the
+ * valid rows x atoms of every contraction box it runs; boxes of structural zeros are skipped and not counted) and the
+ * atom-tile width chosen for it; 0 / 0 for other stages.  Either pointer may be NULL. */
+int nnp_get_stage_work(nnp_handle *h, int32_t stage, double *issued_flops_host, int32_t *atom_tile_host);
 
 /*
  * nnp_measure_peaks (measurement only): micro-benchmarks on the current device; peaks_host f64[n], n <= 4:

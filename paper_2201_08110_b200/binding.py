@@ -38,7 +38,7 @@ SYMBOLS = (
     "nnp_create", "nnp_compute", "nnp_compute_host", "nnp_status", "nnp_destroy", "nnp_error_string",
     "nnp_launches_per_compute", "nnp_set_profiling", "nnp_get_stage_times", "nnp_stage_name", "nnp_get_work",
     "nnp_debug_pairs", "nnp_debug_aev", "nnp_debug_atomic_energies", "nnp_debug_daev", "nnp_n_features",
-    "nnp_create_from_file", "nnp_compute_fixed", "nnp_compute_async", "nnp_measure_peaks",
+    "nnp_get_stage_work", "nnp_create_from_file", "nnp_compute_fixed", "nnp_compute_async", "nnp_measure_peaks",
     "nnp_coupling_create", "nnp_coupling_compute", "nnp_coupling_compute_fixed", "nnp_coupling_destroy",
 )
 FIXED_ONE = float(1 << 32)  # 64-bit fixed-point force format: round(F * 2^32)
@@ -122,6 +122,8 @@ def load_library():
             getattr(lib, name).argtypes = [C.c_void_p, C.c_void_p]
         lib.nnp_n_features.restype = C.c_int
         lib.nnp_n_features.argtypes = [C.c_void_p]
+        lib.nnp_get_stage_work.restype = C.c_int
+        lib.nnp_get_stage_work.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_int32)]
         lib.nnp_create_from_file.restype = C.c_int
         lib.nnp_create_from_file.argtypes = [C.POINTER(C.c_void_p), C.c_char_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p,
                                              C.c_int32, C.c_double, C.c_int32]
@@ -297,6 +299,17 @@ class NNP:
         _check(self.lib.nnp_get_stage_times(self.h, ms.ctypes.data, n.value, C.byref(n)), "nnp_get_stage_times")
         names = [self.lib.nnp_stage_name(self.h, k).decode() for k in range(n.value)]
         return dict(zip(names, ms.tolist()))
+
+    def stage_work(self):
+        """{stage name: (flops issued by a tensor-engine launch, its atom-tile width)}; (0, 0) for other stages."""
+        n = C.c_int32()
+        _check(self.lib.nnp_get_stage_times(self.h, None, 0, C.byref(n)), "nnp_get_stage_times")
+        out = {}
+        for k in range(n.value):
+            fl, tile = C.c_double(), C.c_int32()
+            _check(self.lib.nnp_get_stage_work(self.h, k, C.byref(fl), C.byref(tile)), "nnp_get_stage_work")
+            out[self.lib.nnp_stage_name(self.h, k).decode()] = (fl.value, tile.value)
+        return out
 
     def work(self):
         w = np.zeros(4, dtype=np.float64)

@@ -744,7 +744,7 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(
     fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
     if (lane == 0) {
       const int row = atom_index ? atom_index[a] : a;
-      if (fixed) {
+      if (fixed & 1) {
         // 64-bit fixed point (2^32 per force unit, the accumulation format of GPU MD engines): integer atomic adds
         // commute, so MM kernels running CONCURRENTLY may add into the same buffer and the sum has the same bits in
         // any order (NNP and MM concurrently instead of sequentially)
@@ -753,6 +753,11 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(
         atomicAdd(f + 0, (unsigned long long)__double2ll_rn(sc * (double)fx));
         atomicAdd(f + 1, (unsigned long long)__double2ll_rn(sc * (double)fy));
         atomicAdd(f + 2, (unsigned long long)__double2ll_rn(sc * (double)fz));
+      } else if (fixed & 2) {  // nnp_compute_host: the buffer is the library's own, forces are WRITTEN
+        float* f = reinterpret_cast<float*>(force) + (size_t)row * force_stride;
+        f[0] = fscale * fx;
+        f[1] = fscale * fy;
+        f[2] = fscale * fz;
       } else {  // plain read-modify-write: safe only when every other adder is ordered with this stream
         float* f = reinterpret_cast<float*>(force) + (size_t)row * force_stride;
         f[0] += fscale * fx;

@@ -8,11 +8,10 @@
 // The NNP region is small (48-75 atoms in the paper's systems) and the MM region large, so the
 // work is O(N_NNP N_MM) distance tests of which a few per cent pass a 9 A cutoff.  Two launches, no float atomics,
 // fixed summation orders (bit-identical reruns):
-//   coupling_mm_kernel   one thread per MM atom j, NNP atoms staged in shared memory: F_j and the pair energies
-//   coupling_nnp_kernel  one CTA per NNP atom i, threads stride over the MM atoms: F_i; CTA 0 also adds the
-//                        per-CTA energy partials of the first kernel in index order
-// Every pair inside the cutoff is therefore evaluated twice, which costs less than a float-atomic-free transpose
-// of the pair forces.  Arithmetic is FP64 (the work is tiny; B200 has full-rate FP64 FMA) so that parity with the
+//   coupling_mm_kernel   one thread per MM atom j, NNP atoms staged in shared memory: F_j, the pair energies, and the
+//                        reaction on every NNP atom reduced over the warp (shuffles) and the CTA (warp order)
+//   coupling_nnp_kernel  adds the per-CTA partials of F_i and of the energy in CTA order
+// Arithmetic is FP64 (the work is tiny; B200 has full-rate FP64 FMA) so that parity with the
 // float64 oracle is at rounding level; the force increments are rounded once when they are added to the buffer.
 #include <cuda_runtime.h>
 #include <math.h>
@@ -87,36 +86,62 @@ __device__ __forceinline__ void add_force(void* buf, int stride, int row, int fi
   }
 }
 
+constexpr int CP_CHUNK = 64;  // NNP atoms staged per pass
+
+// One thread per MM atom j, NNP atoms staged in shared memory CP_CHUNK at a time.  F_j is accumulated by the thread
+// and added to the buffer (every j belongs to one thread).  The reaction on NNP atom i is reduced over the warp with
+// shuffles -- only for the (i, warp) combinations that have a pair inside the cutoff, which a 9 A cutoff makes rare --
+// then over the CTA's warps in warp order, and written as the CTA's partial f_part[blockIdx][i][3]; the second kernel
+// adds the partials in CTA order.  No float atomics; every sum has a fixed order.
 __global__ void __launch_bounds__(CP_THREADS) coupling_mm_kernel(const __grid_constant__ CpArgs A, const float* __restrict__ pos,
                                                                   int pos_stride, void* force, int force_stride, int fixed,
-                                                                  double* __restrict__ e_part) {
-  __shared__ double sx[CP_THREADS], sy[CP_THREADS], sz[CP_THREADS];
-  __shared__ float sq[CP_THREADS], ss[CP_THREADS], se[CP_THREADS];
+                                                                  double* __restrict__ e_part, double* __restrict__ f_part) {
+  __shared__ double sx[CP_CHUNK], sy[CP_CHUNK], sz[CP_CHUNK];
+  __shared__ float sq[CP_CHUNK], ss[CP_CHUNK], se[CP_CHUNK];
+  __shared__ double wpart[CP_THREADS / 32][CP_CHUNK][3];
   __shared__ double red[CP_THREADS / 32];
   const int j = blockIdx.x * CP_THREADS + threadIdx.x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const bool live = j < A.n_mm;
   CpAtom b = live ? A.mm[j] : CpAtom{0, 0.f, 0.f, 0.f};
   double bx = 0, by = 0, bz = 0;
   if (live) load_pos(pos, pos_stride, b.row, A.length_scale, bx, by, bz);
   double fx = 0, fy = 0, fz = 0, e = 0;
-  for (int i0 = 0; i0 < A.n_nnp; i0 += CP_THREADS) {
-    const int n = min(CP_THREADS, A.n_nnp - i0);
+  for (int i0 = 0; i0 < A.n_nnp; i0 += CP_CHUNK) {
+    const int n = min(CP_CHUNK, A.n_nnp - i0);
     __syncthreads();
     if ((int)threadIdx.x < n) {
       const CpAtom a = A.nnp[i0 + threadIdx.x];
       load_pos(pos, pos_stride, a.row, A.length_scale, sx[threadIdx.x], sy[threadIdx.x], sz[threadIdx.x]);
       sq[threadIdx.x] = a.q; ss[threadIdx.x] = a.sigma; se[threadIdx.x] = a.eps;
     }
+    for (int k = threadIdx.x; k < (CP_THREADS / 32) * CP_CHUNK * 3; k += CP_THREADS) (&wpart[0][0][0])[k] = 0.0;
     __syncthreads();
-    if (live)
-      for (int i = 0; i < n; ++i) {  // NNP atoms in index order
-        const double dx = bx - sx[i], dy = by - sy[i], dz = bz - sz[i];
-        double v, g;
-        if (pair_terms(A, dx, dy, dz, sq[i], ss[i], se[i], b.q, b.sigma, b.eps, v, g)) {
-          e += v;
-          fx -= g * dx; fy -= g * dy; fz -= g * dz;
-        }
+    for (int i = 0; i < n; ++i) {  // NNP atoms in index order
+      const double dx = bx - sx[i], dy = by - sy[i], dz = bz - sz[i];
+      double v = 0.0, g = 0.0;
+      const bool hit = live && pair_terms(A, dx, dy, dz, sq[i], ss[i], se[i], b.q, b.sigma, b.eps, v, g);
+      if (__ballot_sync(0xffffffffu, hit) == 0u) continue;
+      double gx = hit ? g * dx : 0.0, gy = hit ? g * dy : 0.0, gz = hit ? g * dz : 0.0;
+      if (hit) {
+        e += v;
+        fx -= gx; fy -= gy; fz -= gz;
       }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        gx += __shfl_xor_sync(0xffffffffu, gx, o);
+        gy += __shfl_xor_sync(0xffffffffu, gy, o);
+        gz += __shfl_xor_sync(0xffffffffu, gz, o);
+      }
+      if (lane == 0) { wpart[warp][i][0] = gx; wpart[warp][i][1] = gy; wpart[warp][i][2] = gz; }
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < n * 3; k += CP_THREADS) {
+      const int i = k / 3, c = k - 3 * i;
+      double t = 0.0;
+      for (int w = 0; w < CP_THREADS / 32; ++w) t += wpart[w][i][c];
+      f_part[((size_t)blockIdx.x * A.n_nnp + i0 + i) * 3 + c] = t;
+    }
   }
   if (live && force && (fx != 0.0 || fy != 0.0 || fz != 0.0))
     add_force(force, force_stride, b.row, fixed, fx * A.length_scale, fy * A.length_scale, fz * A.length_scale);
@@ -124,35 +149,35 @@ __global__ void __launch_bounds__(CP_THREADS) coupling_mm_kernel(const __grid_co
   if (threadIdx.x == 0) e_part[blockIdx.x] = t;
 }
 
-__global__ void __launch_bounds__(CP_THREADS) coupling_nnp_kernel(const __grid_constant__ CpArgs A, const float* __restrict__ pos,
-                                                                   int pos_stride, void* force, int force_stride, int fixed,
-                                                                   const double* __restrict__ e_part, int n_part,
+// forces on the NNP atoms: one warp per atom adds the CTA partials of the first kernel (lanes stride over the CTAs,
+// then a fixed shuffle tree: the same order in every run); the energy partials likewise by warp 0 of CTA 0
+__global__ void __launch_bounds__(CP_THREADS) coupling_nnp_kernel(const __grid_constant__ CpArgs A, void* force, int force_stride,
+                                                                   int fixed, const double* __restrict__ e_part,
+                                                                   const double* __restrict__ f_part, int n_part,
                                                                    double* __restrict__ energy) {
-  __shared__ double red[CP_THREADS / 32];
-  const int i = blockIdx.x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int i = blockIdx.x * (CP_THREADS / 32) + warp;
   if (i < A.n_nnp) {
-    const CpAtom a = A.nnp[i];
-    double ax, ay, az;
-    load_pos(pos, pos_stride, a.row, A.length_scale, ax, ay, az);
-    double fx = 0, fy = 0, fz = 0;
-    for (int j = threadIdx.x; j < A.n_mm; j += CP_THREADS) {
-      const CpAtom b = A.mm[j];
-      double bx, by, bz;
-      load_pos(pos, pos_stride, b.row, A.length_scale, bx, by, bz);
-      const double dx = bx - ax, dy = by - ay, dz = bz - az;
-      double v, g;
-      if (pair_terms(A, dx, dy, dz, a.q, a.sigma, a.eps, b.q, b.sigma, b.eps, v, g)) {
-        fx += g * dx; fy += g * dy; fz += g * dz;
-      }
+    double tx = 0.0, ty = 0.0, tz = 0.0;
+    for (int k = lane; k < n_part; k += 32) {
+      const double* p = f_part + ((size_t)k * A.n_nnp + i) * 3;
+      tx += p[0]; ty += p[1]; tz += p[2];
     }
-    const double tx = block_sum(fx, red), ty = block_sum(fy, red), tz = block_sum(fz, red);
-    if (threadIdx.x == 0 && force)
-      add_force(force, force_stride, a.row, fixed, tx * A.length_scale, ty * A.length_scale, tz * A.length_scale);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      tx += __shfl_xor_sync(0xffffffffu, tx, o);
+      ty += __shfl_xor_sync(0xffffffffu, ty, o);
+      tz += __shfl_xor_sync(0xffffffffu, tz, o);
+    }
+    if (lane == 0 && force)
+      add_force(force, force_stride, A.nnp[i].row, fixed, tx * A.length_scale, ty * A.length_scale, tz * A.length_scale);
   }
-  if (blockIdx.x == 0 && threadIdx.x == 0 && energy) {
-    double t = 0.0;
-    for (int k = 0; k < n_part; ++k) t += e_part[k];
-    *energy = t;
+  if (blockIdx.x == 0 && warp == 0 && energy) {
+    double s = 0.0;
+    for (int k = lane; k < n_part; k += 32) s += e_part[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) *energy = s;
   }
 }
 
@@ -162,7 +187,7 @@ struct nnp_coupling {
   int device = 0;
   CpArgs args;
   CpAtom *d_nnp = nullptr, *d_mm = nullptr;
-  double* d_epart = nullptr;
+  double *d_epart = nullptr, *d_fpart = nullptr;
   int n_part = 0;
 };
 
@@ -173,6 +198,7 @@ extern "C" void nnp_coupling_destroy(nnp_coupling* c) {
   if (c->d_nnp) cudaFree(c->d_nnp);
   if (c->d_mm) cudaFree(c->d_mm);
   if (c->d_epart) cudaFree(c->d_epart);
+  if (c->d_fpart) cudaFree(c->d_fpart);
   delete c;
 }
 
@@ -203,7 +229,8 @@ extern "C" int nnp_coupling_create(nnp_coupling** out, int32_t n_nnp, const int3
   c->n_part = (n_mm + CP_THREADS - 1) / CP_THREADS;
   bool ok = cudaMalloc((void**)&c->d_nnp, sizeof(CpAtom) * (size_t)(n_nnp > 0 ? n_nnp : 1)) == cudaSuccess &&
             cudaMalloc((void**)&c->d_mm, sizeof(CpAtom) * (size_t)(n_mm > 0 ? n_mm : 1)) == cudaSuccess &&
-            cudaMalloc((void**)&c->d_epart, sizeof(double) * (size_t)(c->n_part > 0 ? c->n_part : 1)) == cudaSuccess;
+            cudaMalloc((void**)&c->d_epart, sizeof(double) * (size_t)(c->n_part > 0 ? c->n_part : 1)) == cudaSuccess &&
+            cudaMalloc((void**)&c->d_fpart, sizeof(double) * 3 * (size_t)(c->n_part > 0 ? c->n_part : 1) * (size_t)(n_nnp > 0 ? n_nnp : 1)) == cudaSuccess;
   if (ok && n_nnp) ok = cudaMemcpy(c->d_nnp, a.data(), sizeof(CpAtom) * (size_t)n_nnp, cudaMemcpyHostToDevice) == cudaSuccess;
   if (ok && n_mm) ok = cudaMemcpy(c->d_mm, b.data(), sizeof(CpAtom) * (size_t)n_mm, cudaMemcpyHostToDevice) == cudaSuccess;
   if (!ok) {
@@ -219,10 +246,10 @@ static int coupling_enqueue(nnp_coupling* c, const float* d_pos, int ps, double*
                             cudaStream_t s) {
   if (!c || !d_pos || ps < 3 || (d_force && fs < 3)) return NNP_ERR_INVALID_ARG;
   if (c->args.n_mm > 0)
-    coupling_mm_kernel<<<c->n_part, CP_THREADS, 0, s>>>(c->args, d_pos, ps, d_force, fs, fixed, c->d_epart);
-  coupling_nnp_kernel<<<c->args.n_nnp > 0 ? c->args.n_nnp : 1, CP_THREADS, 0, s>>>(c->args, d_pos, ps, d_force, fs, fixed,
-                                                                                   c->d_epart, c->args.n_mm > 0 ? c->n_part : 0,
-                                                                                   d_energy);
+    coupling_mm_kernel<<<c->n_part, CP_THREADS, 0, s>>>(c->args, d_pos, ps, d_force, fs, fixed, c->d_epart, c->d_fpart);
+  const int nb = (c->args.n_nnp + CP_THREADS / 32 - 1) / (CP_THREADS / 32);
+  coupling_nnp_kernel<<<nb > 0 ? nb : 1, CP_THREADS, 0, s>>>(c->args, d_force, fs, fixed, c->d_epart, c->d_fpart,
+                                                            c->args.n_mm > 0 ? c->n_part : 0, d_energy);
   return cudaGetLastError() == cudaSuccess ? NNP_OK : NNP_ERR_CUDA;
 }
 

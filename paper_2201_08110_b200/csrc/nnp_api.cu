@@ -63,13 +63,14 @@ extern "C" void nnp_destroy(nnp_handle* h) {
   cudaSetDevice(h->device);
   if (h->last_stream) cudaStreamSynchronize(h->last_stream);
   cudaDeviceSynchronize();
+  if (h->h_hout) cudaFreeHost(h->h_hout);
   for (auto& g : h->graphs)
     if (g.exec) cudaGraphExecDestroy(g.exec);
   if (h->own_stream) cudaStreamDestroy(h->own_stream);
   for (auto e : h->events) cudaEventDestroy(e);
   void* ptrs[] = {h->d_eblocks, h->d_epart, h->d_ecount, h->d_mol_range, h->d_species, h->d_mol_off, h->d_mol_id, h->d_sortpos, h->d_perm, h->d_grp_off, h->d_self_energy,
                   h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_aev, h->d_daev, h->d_phi,
-                  h->d_eatom, h->d_status, h->d_W, h->d_b, h->d_hpos, h->d_hforce, h->d_henergy,
+                  h->d_eatom, h->d_status, h->d_W, h->d_b, h->d_hpos, h->d_hout,
                   h->d_aev_lo, h->d_Whi, h->d_Wlo, h->d_WThi, h->d_WTlo};
   for (void* p : ptrs)
     if (p) cudaFree(p);
@@ -323,8 +324,11 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       dev_alloc(&h->d_nbr_a, (size_t)N * h->capA) || dev_alloc(&h->d_cnt_r, (size_t)N) ||
       dev_alloc(&h->d_cnt_a, (size_t)N) || dev_alloc(&h->d_aev, (size_t)N * n_feat) ||
       dev_alloc(&h->d_daev, (size_t)h->n_parts * N * n_feat) || dev_alloc(&h->d_phi, (size_t)N * h->capR * 3) ||
-      dev_alloc(&h->d_eatom, (size_t)N * M) || dev_alloc(&h->d_status, 1) || dev_alloc(&h->d_hpos, (size_t)N * 3) ||
-      dev_alloc(&h->d_hforce, (size_t)N * 3) || dev_alloc(&h->d_henergy, (size_t)n_molecules))
+      dev_alloc(&h->d_eatom, (size_t)N * M) || dev_alloc(&h->d_status, 1) || dev_alloc(&h->d_hpos, (size_t)N * 3))
+    return fail(NNP_ERR_ALLOC);
+  h->hout_force_off = sizeof(double) * (size_t)n_molecules;
+  h->hout_bytes = h->hout_force_off + sizeof(float) * 3 * (size_t)N;
+  if (dev_alloc(&h->d_hout, h->hout_bytes) || cudaHostAlloc((void**)&h->h_hout, std::max<size_t>(h->hout_bytes, 1), cudaHostAllocDefault) != cudaSuccess)
     return fail(NNP_ERR_ALLOC);
   if (h->use_umma && dev_alloc(&h->d_aev_lo, (size_t)N * n_feat)) return fail(NNP_ERR_ALLOC);
   // latency-bound sizes only: in a large batch the serial row build inside every centre's CTA costs more than the
@@ -808,6 +812,16 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   }
   h->stage_names.push_back("aev_bwd");
   h->stage_names.push_back("finish");
+  h->stage_issued.assign(h->stage_names.size(), 0.0);
+  h->stage_tile.assign(h->stage_names.size(), 0);
+  if (h->use_umma)
+    for (size_t k = 0; k < h->stage_names.size(); ++k)
+      for (auto* v : {&h->ufwd, &h->ubwd})
+        for (auto& g : *v)
+          if (g.name == h->stage_names[k]) {
+            h->stage_issued[k] = g.issued_flops;
+            h->stage_tile[k] = g.tile;
+          }
   h->n_launches = N > 0 ? (int)h->stage_names.size() + (h->use_cells ? 4 : 0) : 0;  // cell path: 5 kernels in "nbr"
   h->events.resize(h->stage_names.size() + 1);
   for (auto& e : h->events)
@@ -942,15 +956,16 @@ extern "C" int nnp_compute_host(nnp_handle* h, const float* pos_host, double* en
     return NNP_OK;
   }
   cudaStream_t s = (cudaStream_t)cuda_stream;
+  // three stream operations and one synchronisation: positions in, the graph (forces WRITTEN into the library's
+  // block, so no memset), energies + forces out in one copy to a pinned block
   CK(cudaMemcpyAsync(h->d_hpos, pos_host, sizeof(float) * 3 * (size_t)h->N, cudaMemcpyHostToDevice, s));
-  CK(cudaMemsetAsync(h->d_hforce, 0, sizeof(float) * 3 * (size_t)h->N, s));
-  int rc = nnp_compute(h, h->d_hpos, 3, nullptr, h->d_henergy, h->d_hforce, 3, cuda_stream);
+  int rc = compute_impl(h, h->d_hpos, 3, nullptr, reinterpret_cast<double*>(h->d_hout),
+                        h->d_hout + h->hout_force_off, 3, 2, s);
   if (rc != NNP_OK) return rc;
-  if (energy_host)
-    CK(cudaMemcpyAsync(energy_host, h->d_henergy, sizeof(double) * (size_t)h->n_mol, cudaMemcpyDeviceToHost, s));
-  if (force_host)
-    CK(cudaMemcpyAsync(force_host, h->d_hforce, sizeof(float) * 3 * (size_t)h->N, cudaMemcpyDeviceToHost, s));
+  CK(cudaMemcpyAsync(h->h_hout, h->d_hout, h->hout_bytes, cudaMemcpyDeviceToHost, s));
   CK(cudaStreamSynchronize(s));
+  if (energy_host) memcpy(energy_host, h->h_hout, sizeof(double) * (size_t)h->n_mol);
+  if (force_host) memcpy(force_host, h->h_hout + h->hout_force_off, sizeof(float) * 3 * (size_t)h->N);
   return NNP_OK;
 }
 
@@ -992,6 +1007,13 @@ extern "C" int nnp_get_stage_times(nnp_handle* h, float* ms_host, int32_t capaci
 extern "C" const char* nnp_stage_name(nnp_handle* h, int32_t stage) {
   if (!h || stage < 0 || stage >= (int)h->stage_names.size()) return "";
   return h->stage_names[stage].c_str();
+}
+
+extern "C" int nnp_get_stage_work(nnp_handle* h, int32_t stage, double* issued_flops_host, int32_t* atom_tile_host) {
+  if (!h || stage < 0 || stage >= (int)h->stage_names.size()) return NNP_ERR_INVALID_ARG;
+  if (issued_flops_host) *issued_flops_host = h->stage_issued[stage];
+  if (atom_tile_host) *atom_tile_host = h->stage_tile[stage];
+  return NNP_OK;
 }
 
 extern "C" int nnp_get_work(nnp_handle* h, double* what_host, int32_t n) {

@@ -292,8 +292,12 @@ struct nnp_handle {
   int n_parts = 1;                   // dE/dAEV is produced as n_parts partial sums (per model at small N)
   LastLayerArgs last;
   // host staging for nnp_compute_host
-  float *d_hpos = nullptr, *d_hforce = nullptr;
-  double* d_henergy = nullptr;
+  // nnp_compute_host: device staging (positions; energies then forces in ONE block, so one copy brings both back)
+  // and a pinned host block of the same layout
+  float* d_hpos = nullptr;
+  unsigned char* d_hout = nullptr;
+  unsigned char* h_hout = nullptr;
+  size_t hout_bytes = 0, hout_force_off = 0;
   // graphs: one instantiated graph per distinct argument tuple, a small LRU (an engine that double-buffers its
   // positions or forces alternates between two of them at no cost)
   struct GraphSlot {
@@ -312,6 +316,8 @@ struct nnp_handle {
   bool profiling = false;
   std::vector<cudaEvent_t> events;
   std::vector<std::string> stage_names;
+  std::vector<double> stage_issued;  // tensor-engine stages: 2 x MACs actually issued (structural zeros skipped)
+  std::vector<int> stage_tile;       // tensor-engine stages: atom-tile width chosen for the launch
   int n_launches = 0;
   double work[4] = {0, 0, 0, 0};
 };

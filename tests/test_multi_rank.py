@@ -68,7 +68,19 @@ def _worker(rank, world, port, q):
         gathered = [None] * world
         dist.all_gather_object(gathered, (sh.mol_lo, sh.atom_lo, mine["E"], mine["F"]))
         t_max = multi.max_over_ranks(10.0 + rank, dist)
+        # ensemble sharding of ONE molecule: this rank's networks, then the one SUM all-reduce
+        W3, B3 = wl.make_weights(p, 3, seed=12, random_biases=True)
+        se = np.array([-0.5, -38.0, -54.7])
+        m_lo, m_hi = multi.shard_models(3, world, rank)  # 2 + 1 networks: unequal parts
+        Wp, Bp = multi.slice_models(W3, B3, m_lo, m_hi)
+        part = AniOracle(p, Wp, Bp, self_energy=se).energy_forces(mols[1].positions, mols[1].species)
+        E_all, F_all = multi.combine_ensemble_parts(part["E"], part["F"], m_hi - m_lo, 3, dist)
+        whole = AniOracle(p, W3, B3, self_energy=se).energy_forces(mols[1].positions, mols[1].species)
+        ens_ok = (np.allclose(E_all, whole["E"], rtol=1e-13, atol=1e-9) and np.allclose(F_all, whole["F"], rtol=0, atol=1e-10))
+        flags = [None] * world
+        dist.all_gather_object(flags, bool(ens_ok))
         if rank == 0:
+            assert all(flags), "ensemble-sharded result differs from the whole ensemble"
             full = orc.energy_forces(pos, spc, off)
             E = np.concatenate([g[2] for g in sorted(gathered, key=lambda g: g[0])])
             F = np.concatenate([g[3] for g in sorted(gathered, key=lambda g: g[1])])
@@ -92,3 +104,15 @@ def test_two_rank_gloo_sharded_batch_matches_unsharded():
         pr.join(timeout=180)
         assert pr.exitcode == 0
     assert q.get(timeout=10) is True
+
+
+def test_shard_models_and_single_part_identity():
+    assert [multi.shard_models(8, 4, r) for r in range(4)] == [(0, 2), (2, 4), (4, 6), (6, 8)]
+    assert [multi.shard_models(8, 3, r) for r in range(3)] == [(0, 3), (3, 6), (6, 8)]
+    with pytest.raises(ValueError):
+        multi.shard_models(1, 2, 0)
+    E, F = np.array([1.5, -2.0]), np.arange(12, dtype=np.float32).reshape(4, 3)
+    E2, F2 = multi.combine_ensemble_parts(E, F, 8, 8)
+    assert np.array_equal(E, E2) and np.array_equal(F, F2) and F2.dtype == np.float32
+    with pytest.raises(ValueError):
+        multi.combine_ensemble_parts(E, F, 4, 8)
