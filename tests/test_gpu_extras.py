@@ -233,3 +233,55 @@ def test_measured_peaks_are_plausible():
     assert 30.0 < pk["fp32_ffma_tflops"] < 90.0
     assert 300.0 < pk["tf32_tcgen05_tflops"] < 1400.0
     assert pk["l2_read_gbs"] > pk["dram_read_gbs"] > 2000.0
+
+
+def _gpu_ef(nnp, pos, n_mol):
+    p = torch.from_numpy(np.ascontiguousarray(pos)).to(DEV)
+    E = torch.zeros(n_mol, dtype=torch.float64, device=DEV)
+    F = torch.zeros((pos.shape[0], 3), dtype=torch.float32, device=DEV)
+    nnp.compute_torch(p, E, F); nnp.check()
+    return E, F
+
+
+def test_molecule_shards_equal_the_unsharded_batch():
+    """SURVEY 8(e), molecules: what rank r of 2 computes for its slice of a configs[2]-like batch is what the
+    unsharded handle computes for those molecules (molecules never interact).  Not bit for bit: a handle chooses its
+    GEMM tiling from its own element-group sizes, so FP32 summation orders differ between the two handles."""
+    from paper_2201_08110_b200 import multi
+
+    w = wl.config3(n_mol=24)
+    W, B = w.weights()
+    whole = NNP(w.params, W, B, w.species, w.mol_offsets)
+    E0, F0 = _gpu_ef(whole, w.positions, w.n_molecules)
+    for rank in range(2):
+        sh = multi.shard_molecules(w.mol_offsets, 2, rank)
+        part = NNP(w.params, W, B, w.species[sh.atom_lo:sh.atom_hi], sh.mol_offsets)
+        E, F = _gpu_ef(part, w.positions[sh.atom_lo:sh.atom_hi], sh.mol_hi - sh.mol_lo)
+        sizes = torch.from_numpy(np.diff(sh.mol_offsets).astype(np.float64)).to(DEV)
+        assert ((E - E0[sh.mol_lo:sh.mol_hi]).abs() / sizes).max().item() <= 2e-6
+        assert (F - F0[sh.atom_lo:sh.atom_hi]).abs().max().item() <= 2e-4
+        part.destroy()
+    whole.destroy()
+
+
+def test_ensemble_shards_combine_to_the_whole_ensemble():
+    """SURVEY 8(e), one large molecule: the networks split 3 + 3 + 2 over three handles; the weighted sum that
+    multi.combine_ensemble_parts all-reduces equals the 8-network result to rounding."""
+    from paper_2201_08110_b200 import multi
+
+    w = wl.config4()
+    W, B = w.weights()
+    whole = NNP(w.params, W, B, w.species)
+    E0, F0 = _gpu_ef(whole, w.positions, 1)
+    buf = None
+    for rank in range(3):
+        lo, hi = multi.shard_models(w.n_models, 3, rank)
+        Wp, Bp = multi.slice_models(W, B, lo, hi)
+        part = NNP(w.params, Wp, Bp, w.species)
+        E, F = _gpu_ef(part, w.positions, 1)
+        contrib = torch.cat([E, F.double().reshape(-1)]) * ((hi - lo) / w.n_models)  # what the SUM all-reduce adds up
+        buf = contrib if buf is None else buf + contrib
+        part.destroy()
+    assert abs(buf[0].item() - E0.item()) / w.n_atoms <= 2e-6
+    assert (buf[1:].reshape(-1, 3) - F0.double()).abs().max().item() <= 2e-4
+    whole.destroy()
