@@ -198,60 +198,76 @@ __device__ __forceinline__ void split4(const float4 v, float4& h, float4& l) {
 }
 __device__ __forceinline__ void drain_sync() { asm volatile("bar.sync 1, %0;" ::"n"(U_DRAIN_THREADS) : "memory"); }
 
-// epilogue of `na` atoms (rows of the staging tile [atom][128 features]) by the 256 drain threads: bias + CELU /
-// x CELU' / scale, four consecutive features of one atom per thread and step (16-byte loads and stores), four steps
-// in flight.  Global row of staging row r is a0 + r.
+// store one float4 of results: split into the hi / lo planes when a tensor launch consumes it
+__device__ __forceinline__ void store_out(const UmmaItem& t, size_t o, const float4 x) {
+  if (t.C_lo) {
+    float4 h, l;
+    split4(x, h, l);
+    st4(t.C + o, h);
+    st4(t.C_lo + o, l);
+  } else {
+    st4(t.C + o, x);
+  }
+}
+
+// epilogue of `na` <= 64 atoms (rows of the staging tile [atom][128 features]) by the 256 drain threads: bias + CELU /
+// x CELU' / scale, four consecutive features of one atom per thread and step (16-byte loads and stores).  A thread
+// has at most 8 steps; the backward epilogue issues ALL its global loads (h of the layer below, two planes) before
+// the first use, so a round costs one memory latency instead of one per step.  Global row of staging row r is a0 + r.
 __device__ __forceinline__ void epilogue_rows(const UmmaItem& t, const float* staging, int a0, int na, int dt) {
-  constexpr int U = 4;
+  constexpr int U = 8;  // 64 atoms x 32 feature groups / 256 threads
   const int n_vec = na * 32;
   const int g = dt & 31;          // the thread's feature group is the same in every step (256 % 32 == 0)
   if (4 * g >= t.f_valid) return;
-  float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
-  if (t.epi == EPI_BIAS_CELU && t.bias) b = ld4(t.bias + 4 * g);
-  for (int base = dt; base < n_vec; base += U * U_DRAIN_THREADS) {
-    float4 v[U], d[U];
-    bool ok[U];
+  const int r0 = dt >> 5;         // rows r0, r0 + 8, ...
+  if (t.epi == EPI_MUL_DCELU) {
+    float4 d[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
-      const int idx = base + u * U_DRAIN_THREADS;
-      ok[u] = idx < n_vec;
-      const int r = idx >> 5;
-      v[u] = ok[u] ? ld4(staging + r * 128 + 4 * g) : make_float4(0.f, 0.f, 0.f, 0.f);
-      if (t.epi == EPI_MUL_DCELU) {  // h of the layer below (hi + lo is exact), for CELU'
-        d[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (ok[u]) {
-          const size_t o = (size_t)(a0 + r) * t.ldaux + 4 * g;
-          d[u] = ld4(t.aux + o);
-          if (t.aux_lo) {
-            const float4 l = ld4(t.aux_lo + o);
-            d[u].x += l.x; d[u].y += l.y; d[u].z += l.z; d[u].w += l.w;
-          }
-        }
+      const int r = r0 + 8 * u;
+      d[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (r * 32 < n_vec) d[u] = ld4(t.aux + (size_t)(a0 + r) * t.ldaux + 4 * g);
+    }
+    if (t.aux_lo) {
+      float4 l[U];
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int r = r0 + 8 * u;
+        l[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (r * 32 < n_vec) l[u] = ld4(t.aux_lo + (size_t)(a0 + r) * t.ldaux + 4 * g);
       }
+#pragma unroll
+      for (int u = 0; u < U; ++u) { d[u].x += l[u].x; d[u].y += l[u].y; d[u].z += l[u].z; d[u].w += l[u].w; }  // exact
     }
 #pragma unroll
     for (int u = 0; u < U; ++u) {
-      if (!ok[u]) continue;
-      const int r = (base + u * U_DRAIN_THREADS) >> 5;
-      float4 x = v[u];
-      if (t.epi == EPI_BIAS_CELU) {
-        x.x = celu_f(x.x + b.x, t.alpha, t.inv_alpha); x.y = celu_f(x.y + b.y, t.alpha, t.inv_alpha);
-        x.z = celu_f(x.z + b.z, t.alpha, t.inv_alpha); x.w = celu_f(x.w + b.w, t.alpha, t.inv_alpha);
-      } else if (t.epi == EPI_MUL_DCELU) {
-        x.x *= dcelu_from_h(d[u].x, t.inv_alpha); x.y *= dcelu_from_h(d[u].y, t.inv_alpha);
-        x.z *= dcelu_from_h(d[u].z, t.inv_alpha); x.w *= dcelu_from_h(d[u].w, t.inv_alpha);
-      } else {
-        x.x *= t.scale; x.y *= t.scale; x.z *= t.scale; x.w *= t.scale;
-      }
-      const size_t o = (size_t)(a0 + r) * t.ldc + 4 * g;
-      if (t.C_lo) {
-        float4 h, l;
-        split4(x, h, l);
-        st4(t.C + o, h);
-        st4(t.C_lo + o, l);
-      } else {
-        st4(t.C + o, x);
-      }
+      const int r = r0 + 8 * u;
+      if (r * 32 >= n_vec) continue;
+      float4 x = ld4(staging + r * 128 + 4 * g);
+      x.x *= dcelu_from_h(d[u].x, t.inv_alpha); x.y *= dcelu_from_h(d[u].y, t.inv_alpha);
+      x.z *= dcelu_from_h(d[u].z, t.inv_alpha); x.w *= dcelu_from_h(d[u].w, t.inv_alpha);
+      store_out(t, (size_t)(a0 + r) * t.ldc + 4 * g, x);
+    }
+  } else if (t.epi == EPI_BIAS_CELU) {
+    float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (t.bias) b = ld4(t.bias + 4 * g);
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int r = r0 + 8 * u;
+      if (r * 32 >= n_vec) continue;
+      float4 x = ld4(staging + r * 128 + 4 * g);
+      x.x = celu_f(x.x + b.x, t.alpha, t.inv_alpha); x.y = celu_f(x.y + b.y, t.alpha, t.inv_alpha);
+      x.z = celu_f(x.z + b.z, t.alpha, t.inv_alpha); x.w = celu_f(x.w + b.w, t.alpha, t.inv_alpha);
+      store_out(t, (size_t)(a0 + r) * t.ldc + 4 * g, x);
+    }
+  } else {
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int r = r0 + 8 * u;
+      if (r * 32 >= n_vec) continue;
+      float4 x = ld4(staging + r * 128 + 4 * g);
+      x.x *= t.scale; x.y *= t.scale; x.z *= t.scale; x.w *= t.scale;
+      st4(t.C + (size_t)(a0 + r) * t.ldc + 4 * g, x);
     }
   }
 }
