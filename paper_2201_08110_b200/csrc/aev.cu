@@ -217,7 +217,7 @@ size_t aev_smem_bytes(const nnp_handle* h, bool backward) {
   const int CH = trip_chunk(h, backward);
   if (!backward) {
     fl += (size_t)(h->n_feat - h->aev.n_radial);                       // angular part of the row
-    fl += (size_t)(h->aev.n_shf_z + h->aev.n_shf_a) * CH;              // F1 / F2 factors of a pass
+    fl += (size_t)(h->aev.n_shf_z + h->aev.n_shf_a) * (CH + 1);        // F1 / F2 factors of a pass (row pitch CH + 1)
   } else {
     fl += (size_t)h->aev.n_radial + (size_t)n_pairs * ang_row_pad(h);  // dE/dAEV row (angular blocks padded)
     fl += (size_t)2 * 3 * h->capR;                                     // radial + angular pair gradients
@@ -376,8 +376,12 @@ __global__ void __launch_bounds__(AEV_THREADS, 6) aev_forward_kernel(
   const CentreTab t = carve_tab(smem, capR, capA, c.S);
   const int n_ang = c.n_feat - c.n_radial;
   float* row = t.rest;                 // [n_ang]
-  float* bF1 = row + n_ang;            // [n_shf_z][CH]
-  float* bF2 = bF1 + c.n_shf_z * CH;   // [n_shf_a][CH]
+  // row pitch CH + 1: in the column sums below the lanes of a warp read the same triplet of DIFFERENT rows (one per
+  // (ShfA, ShfZ) sub-term); with a pitch that is a multiple of 32 those were 4- and 8-way bank conflicts (ncu: 55 % of
+  // the kernel's shared-memory wavefronts)
+  const int CHP = CH + 1;
+  float* bF1 = row + n_ang;            // [n_shf_z][CHP]
+  float* bF2 = bF1 + c.n_shf_z * CHP;  // [n_shf_a][CHP]
   pdl_trigger();
   pdl_wait();
   float4* mp = reinterpret_cast<float4*>(smem) + mp_off4;  // [max molecule size]: the molecule's positions (fused path)
@@ -440,7 +444,7 @@ __global__ void __launch_bounds__(AEV_THREADS, 6) aev_forward_kernel(
       for (int iz = 0; iz < NZ; ++iz) {
         if (iz < c.n_shf_z) {
           const float u = 0.5f + 0.5f * ((cc * c.cos_z[iz] + ss * c.sin_z[iz]) + (cc * c.cos_z_lo[iz] + ss * c.sin_z_lo[iz]));
-          bF1[iz * CH + tl] = pow_split(u, c.zeta_int, c.zeta_frac);
+          bF1[iz * CHP + tl] = pow_split(u, c.zeta_int, c.zeta_frac);
         }
       }
       const float w = 2.0f * (t.fca[qa] * t.fca[qb]);
@@ -450,7 +454,7 @@ __global__ void __launch_bounds__(AEV_THREADS, 6) aev_forward_kernel(
         if (ia < c.n_shf_a) {
           const float shfa = c.shf_a[ia];
           const float d = 0.5f * (((ra - shfa) + (rb - shfa)) + rl);
-          bF2[ia * CH + tl] = w * gauss(d, c.ka_hi, c.ka_lo);
+          bF2[ia * CHP + tl] = w * gauss(d, c.ka_hi, c.ka_lo);
         }
       }
     }
@@ -463,8 +467,8 @@ __global__ void __launch_bounds__(AEV_THREADS, 6) aev_forward_kernel(
       const int st = t.pair_st[p];
       const int s = st >> 8, u = st & 255;
       const int a0 = t.sp_off[s], a1 = t.sp_off[s + 1], b0 = t.sp_off[u], b1 = t.sp_off[u + 1];
-      const float* f1 = bF1 + iz * CH;
-      const float* f2 = bF2 + ia * CH;
+      const float* f1 = bF1 + iz * CHP;
+      const float* f2 = bF2 + ia * CHP;
       float acc = 0.0f;
       for (int a = a0; a < a1; ++a) {
         const int base = trip_row_start(a, na) - a - 1 - c0;  // local index of (a, b) is base + b
