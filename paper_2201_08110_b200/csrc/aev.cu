@@ -847,7 +847,7 @@ void launch_aev_forward(nnp_handle* h, const float* d_pos, int pos_stride, const
   if (h->N == 0) return;
   const int blocks = h->N;
   const size_t smem0 = aev_smem_bytes(h, false);
-  const size_t smem = smem0 + (h->fuse_nbr ? 256 * sizeof(float4) : 0);  // + the molecule's positions (<= 256 atoms)
+  const size_t smem = smem0 + (h->fuse_nbr ? 512 * sizeof(float4) : 0);  // + the molecule's positions (<= 512 atoms)
   const int mp_off4 = (int)(smem0 / sizeof(float4));
   const NbrArgs nb = nbr_args(h, d_pos, pos_stride, d_atom_index);
   const int fused = h->fuse_nbr ? 1 : 0;
@@ -898,7 +898,7 @@ void launch_finish(nnp_handle* h, const int* d_atom_index, double* d_energy, voi
 }
 
 int aev_set_smem_attributes(nnp_handle* h) {
-  const int fb = (int)(aev_smem_bytes(h, false) + 256 * sizeof(float4)), bb = (int)aev_smem_bytes(h, true);
+  const int fb = (int)(aev_smem_bytes(h, false) + 512 * sizeof(float4)), bb = (int)aev_smem_bytes(h, true);
   cudaError_t e[6];
   e[0] = cudaFuncSetAttribute(aev_forward_kernel<4, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, fb);
   e[1] = cudaFuncSetAttribute(aev_forward_kernel<NNP_MAX_SHF_Z, NNP_MAX_SHF_A>,

@@ -333,7 +333,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   if (h->use_umma && dev_alloc(&h->d_aev_lo, (size_t)N * n_feat)) return fail(NNP_ERR_ALLOC);
   // latency-bound sizes only: in a large batch the serial row build inside every centre's CTA costs more than the
   // launch it saves (configs[2]: +36 us in the AEV forward against a 12 us neighbour kernel)
-  h->fuse_nbr = N > 0 && N <= 512 && !h->use_cells && max_mol <= 256 && !(cfg->flags & NNP_FLAG_NO_NBR_FUSION);
+  h->fuse_nbr = N > 0 && N <= 512 && !h->use_cells && max_mol <= 512 && !(cfg->flags & NNP_FLAG_NO_NBR_FUSION);
   if (h->use_cells && cells_alloc(h) != 0) return fail(NNP_ERR_ALLOC);
   {  // energy reduction blocks: chunks of <= 2048 atoms
     const int ECH = 2048;
