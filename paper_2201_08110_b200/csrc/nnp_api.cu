@@ -193,8 +193,14 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     for (int i = mol_off[m]; i < mol_off[m + 1]; ++i) mol_id[i] = m;
     max_mol = std::max(max_mol, mol_off[m + 1] - mol_off[m]);
   }
-  h->capR = cfg->max_radial_neighbors > 0 ? cfg->max_radial_neighbors : std::min(std::max(max_mol - 1, 1), 256);
-  h->capA = cfg->max_angular_neighbors > 0 ? cfg->max_angular_neighbors : std::min(std::max(max_mol - 1, 1), 128);
+  // Row capacities of the neighbour lists.  A molecule of n atoms has at most n - 1 neighbours; for large molecules the
+  // default assumes condensed matter (<= 0.11 atoms/A^3 gives ~61 atoms inside 5.1 A and ~20 inside 3.5 A; configs[4]
+  // peaks at 90 / 39): 160 radial and 80 angular slots.  The capacities size the per-centre shared-memory tables of the
+  // AEV kernels (occupancy) and the pair-gradient buffer; a denser system sets NNP_ERR_CAPACITY, which nnp_status
+  // reports, and is served by max_radial_neighbors / max_angular_neighbors.
+  const int dflt_r = max_mol >= 1024 ? 160 : 256, dflt_a = max_mol >= 1024 ? 80 : 128;
+  h->capR = cfg->max_radial_neighbors > 0 ? cfg->max_radial_neighbors : std::min(std::max(max_mol - 1, 1), dflt_r);
+  h->capA = cfg->max_angular_neighbors > 0 ? cfg->max_angular_neighbors : std::min(std::max(max_mol - 1, 1), dflt_a);
   if (h->capA > h->capR) h->capA = h->capR;
   // A1 engine: all pairs inside a molecule at ligand sizes, cell binning for large molecules
   h->use_cells = N > 0 && !(cfg->flags & NNP_FLAG_NO_CELLS) && (max_mol >= 1024 || (cfg->flags & NNP_FLAG_FORCE_CELLS));
