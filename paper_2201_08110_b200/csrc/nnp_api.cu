@@ -64,13 +64,14 @@ extern "C" void nnp_destroy(nnp_handle* h) {
   if (h->last_stream) cudaStreamSynchronize(h->last_stream);
   cudaDeviceSynchronize();
   if (h->h_hout) cudaFreeHost(h->h_hout);
+  if (h->h_hpos) cudaFreeHost(h->h_hpos);
   for (auto& g : h->graphs)
     if (g.exec) cudaGraphExecDestroy(g.exec);
   if (h->own_stream) cudaStreamDestroy(h->own_stream);
   for (auto e : h->events) cudaEventDestroy(e);
   void* ptrs[] = {h->d_eblocks, h->d_epart, h->d_ecount, h->d_mol_range, h->d_species, h->d_mol_off, h->d_mol_id, h->d_sortpos, h->d_perm, h->d_grp_off, h->d_self_energy,
                   h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_aev, h->d_daev, h->d_phi,
-                  h->d_eatom, h->d_status, h->d_W, h->d_b, h->d_hpos, h->d_hout,
+                  h->d_eatom, h->d_status, h->d_W, h->d_b,
                   h->d_aev_lo, h->d_Whi, h->d_Wlo, h->d_WThi, h->d_WTlo};
   for (void* p : ptrs)
     if (p) cudaFree(p);
@@ -330,12 +331,16 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
       dev_alloc(&h->d_nbr_a, (size_t)N * h->capA) || dev_alloc(&h->d_cnt_r, (size_t)N) ||
       dev_alloc(&h->d_cnt_a, (size_t)N) || dev_alloc(&h->d_aev, (size_t)N * n_feat) ||
       dev_alloc(&h->d_daev, (size_t)h->n_parts * N * n_feat) || dev_alloc(&h->d_phi, (size_t)N * h->capR * 3) ||
-      dev_alloc(&h->d_eatom, (size_t)N * M) || dev_alloc(&h->d_status, 1) || dev_alloc(&h->d_hpos, (size_t)N * 3))
+      dev_alloc(&h->d_eatom, (size_t)N * M) || dev_alloc(&h->d_status, 1))
     return fail(NNP_ERR_ALLOC);
   h->hout_force_off = sizeof(double) * (size_t)n_molecules;
   h->hout_bytes = h->hout_force_off + sizeof(float) * 3 * (size_t)N;
-  if (dev_alloc(&h->d_hout, h->hout_bytes) || cudaHostAlloc((void**)&h->h_hout, std::max<size_t>(h->hout_bytes, 1), cudaHostAllocDefault) != cudaSuccess)
+  if (cudaHostAlloc((void**)&h->h_hout, std::max<size_t>(h->hout_bytes, 8), cudaHostAllocMapped) != cudaSuccess ||
+      cudaHostAlloc((void**)&h->h_hpos, std::max<size_t>(sizeof(float) * 3 * (size_t)N, 4), cudaHostAllocMapped) != cudaSuccess ||
+      cudaHostGetDevicePointer((void**)&h->d_hout_alias, h->h_hout, 0) != cudaSuccess ||
+      cudaHostGetDevicePointer((void**)&h->d_hpos_alias, h->h_hpos, 0) != cudaSuccess)
     return fail(NNP_ERR_ALLOC);
+  memset(h->h_hout, 0, std::max<size_t>(h->hout_bytes, 8));
   if (h->use_umma && dev_alloc(&h->d_aev_lo, (size_t)N * n_feat)) return fail(NNP_ERR_ALLOC);
   // latency-bound sizes only: in a large batch the serial row build inside every centre's CTA costs more than the
   // launch it saves (configs[2]: +36 us in the AEV forward against a 12 us neighbour kernel)
@@ -962,13 +967,14 @@ extern "C" int nnp_compute_host(nnp_handle* h, const float* pos_host, double* en
     return NNP_OK;
   }
   cudaStream_t s = (cudaStream_t)cuda_stream;
-  // three stream operations and one synchronisation: positions in, the graph (forces WRITTEN into the library's
-  // block, so no memset), energies + forces out in one copy to a pinned block
-  CK(cudaMemcpyAsync(h->d_hpos, pos_host, sizeof(float) * 3 * (size_t)h->N, cudaMemcpyHostToDevice, s));
-  int rc = compute_impl(h, h->d_hpos, 3, nullptr, reinterpret_cast<double*>(h->d_hout),
-                        h->d_hout + h->hout_force_off, 3, 2, s);
+  // Zero-copy staging: the positions go into a pinned block of the library (a host memcpy of 12 N bytes) that the
+  // first kernel reads through its device alias, and the finish kernel WRITES energies and forces straight into a
+  // second pinned block; the call is then one graph launch and one stream synchronisation -- no copy engine
+  // operations, no memset (each costs 2-4 us of launch latency at ligand sizes).
+  memcpy(h->h_hpos, pos_host, sizeof(float) * 3 * (size_t)h->N);
+  int rc = compute_impl(h, h->d_hpos_alias, 3, nullptr, reinterpret_cast<double*>(h->d_hout_alias),
+                        h->d_hout_alias + h->hout_force_off, 3, 2, s);
   if (rc != NNP_OK) return rc;
-  CK(cudaMemcpyAsync(h->h_hout, h->d_hout, h->hout_bytes, cudaMemcpyDeviceToHost, s));
   CK(cudaStreamSynchronize(s));
   if (energy_host) memcpy(energy_host, h->h_hout, sizeof(double) * (size_t)h->n_mol);
   if (force_host) memcpy(force_host, h->h_hout + h->hout_force_off, sizeof(float) * 3 * (size_t)h->N);

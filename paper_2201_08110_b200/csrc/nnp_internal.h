@@ -292,11 +292,12 @@ struct nnp_handle {
   int n_parts = 1;                   // dE/dAEV is produced as n_parts partial sums (per model at small N)
   LastLayerArgs last;
   // host staging for nnp_compute_host
-  // nnp_compute_host: device staging (positions; energies then forces in ONE block, so one copy brings both back)
-  // and a pinned host block of the same layout
-  float* d_hpos = nullptr;
-  unsigned char* d_hout = nullptr;
+  // nnp_compute_host: pinned, device-mapped host blocks (positions in; energies then forces out) and their device
+  // aliases: the kernels read / write them directly
+  float* h_hpos = nullptr;
+  const float* d_hpos_alias = nullptr;
   unsigned char* h_hout = nullptr;
+  unsigned char* d_hout_alias = nullptr;
   size_t hout_bytes = 0, hout_force_off = 0;
   // graphs: one instantiated graph per distinct argument tuple, a small LRU (an engine that double-buffers its
   // positions or forces alternates between two of them at no cost)

@@ -510,3 +510,33 @@ def test_ensemble_of_identical_models_equals_single():
     assert np.abs(r1["F"] - r8["F"]).max() <= 1e-4
     one.destroy()
     eight.destroy()
+
+
+@pytest.mark.parametrize("case", ["molecules", "water"])
+@pytest.mark.parametrize("seed,scale_w", [(901, 1.0), (902, 1.0), (903, 1.5)])
+def test_tensor_engine_energy_headroom(case, seed, scale_w):
+    """the tcgen05 path must keep its margin on other weight draws and on larger weights, not only on the
+    configs' seed: its energy error may exceed that of the exact-product FP32 FFMA engine (same AEV, same oracle) by
+    at most 2e-6 kcal/mol per atom, and the compensation of the truncating accumulate must
+    leave no bias larger than that."""
+    w = wl.config3(n_mol=40) if case == "molecules" else wl.config5(n_mol=700)
+    W, B = wl.make_weights(w.params, w.n_models, seed=seed)
+    if scale_w != 1.0:
+        W = [[[a * np.float32(scale_w) for a in e] for e in m] for m in W]
+    ref = AniOracle(w.params, W, B).energy_forces(w.positions, w.species, w.mol_offsets, want_intermediates=True)
+    sizes = np.maximum(np.diff(w.mol_offsets), 1)
+    err, bias = {}, {}
+    for name, flags in (("tensor", 0), ("ffma", ENGINES["ffma"])):
+        nnp = NNP(w.params, W, B, w.species, w.mol_offsets, flags=flags)
+        gpu = gpu_eval(nnp, w.positions, n_mol=w.n_molecules, stages=True)
+        err[name] = float((np.abs(gpu["E"] - ref["E"]) / sizes).max())
+        bias[name] = float(((gpu["e_atom"].mean(axis=0) - ref["e_atom"].mean(axis=0)) * w.params.energy_scale).mean())
+        # 1e-3 kcal/mol/A is stated for ANI-2x-like weights (max |F| ~ 50-100); larger weights scale the forces and
+        # their rounding error alike (x1.5 per layer => x5): the same 1e-5 relative to the largest force
+        assert np.abs(gpu["F"] - ref["F"]).max() <= max(F_TOL, 1e-5 * np.abs(ref["F"]).max())
+        nnp.destroy()
+    print(f"[parity] headroom {case} seed={seed} x{scale_w}: max|dE|/N tensor {err['tensor']:.2e} ffma {err['ffma']:.2e}; "
+          f"mean de_i tensor {bias['tensor']:+.2e} ffma {bias['ffma']:+.2e}")
+    e_tol = E_TOL_PER_ATOM * scale_w ** 4  # the network output scales with the product of the four layers' weights
+    assert err["tensor"] <= e_tol
+    assert err["tensor"] <= err["ffma"] + 0.2 * e_tol and abs(bias["tensor"] - bias["ffma"]) <= 0.2 * e_tol
