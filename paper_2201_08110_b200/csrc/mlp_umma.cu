@@ -165,11 +165,11 @@ __device__ __forceinline__ void tmem_add(uint32_t taddr, float* acc, uint32_t co
 // CT columns starting at taddr (CT = 8, 16, 32 or 64)
 template <int CT>
 __device__ __forceinline__ void tmem_add_cols(uint32_t taddr, float* acc, uint32_t comp) {
-  if constexpr (CT <= 16) {
+  if constexpr (CT <= 32) {
     tmem_add<CT>(taddr, acc, comp);
-  } else {  // 16 columns at a time: the staging registers count against the 112 of a thread
+  } else {  // 32 columns per load: fewer load / wait round trips per slot than 16, and the staging registers still fit
 #pragma unroll
-    for (int g = 0; g < CT / 16; ++g) tmem_add<16>(taddr + 16 * g, acc + 16 * g, comp);
+    for (int g = 0; g < CT / 32; ++g) tmem_add<32>(taddr + 32 * g, acc + 32 * g, comp);
   }
 }
 
