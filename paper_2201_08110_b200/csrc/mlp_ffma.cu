@@ -222,6 +222,10 @@ __global__ void __launch_bounds__(128) last_layer_kernel(const __grid_constant__
   float* hl = a.act_lo ? a.act_lo + hoff : nullptr;  // tensor engine: activations are stored split (hi, lo planes)
   const float* wv = a.W + a.w_off[e] + (size_t)m * H;
   double acc = 0.0;
+  if (a.act_full) {  // tensor engine: delta was written by the forward epilogue; only the energy is left
+    const float* hf = a.act_full + hoff;
+    for (int o = lane; o < H; o += 32) acc += (double)wv[o] * (double)hf[o];
+  } else
   for (int o = lane; o < H; o += 32) {
     const float hv = hl ? h[o] + hl[o] : h[o], ww = wv[o];  // hi + lo is exact
     acc += (double)ww * (double)hv;

@@ -248,6 +248,25 @@ __device__ __forceinline__ void epilogue_rows(const UmmaItem& t, const float* st
       x.z *= dcelu_from_h(d[u].z, t.inv_alpha); x.w *= dcelu_from_h(d[u].w, t.inv_alpha);
       store_out(t, (size_t)(a0 + r) * t.ldc + 4 * g, x);
     }
+  } else if (t.epi == EPI_BIAS_CELU_LAST) {
+    // last hidden layer: h as ONE plane for the energy kernel, and the start of the backward pass
+    // delta = w_last * CELU'(h) as the split operand of the first backward GEMM (h is not read again as an operand)
+    float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (t.bias) b = ld4(t.bias + 4 * g);
+    const float4 wl = ld4(t.w_last + 4 * g);
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int r = r0 + 8 * u;
+      if (r * 32 >= n_vec) continue;
+      float4 x = ld4(staging + r * 128 + 4 * g);
+      x.x = celu_f(x.x + b.x, t.alpha, t.inv_alpha); x.y = celu_f(x.y + b.y, t.alpha, t.inv_alpha);
+      x.z = celu_f(x.z + b.z, t.alpha, t.inv_alpha); x.w = celu_f(x.w + b.w, t.alpha, t.inv_alpha);
+      const size_t o = (size_t)(a0 + r) * t.ldc + 4 * g;
+      st4(t.C_full + o, x);
+      x.x = wl.x * dcelu_from_h(x.x, t.inv_alpha); x.y = wl.y * dcelu_from_h(x.y, t.inv_alpha);
+      x.z = wl.z * dcelu_from_h(x.z, t.inv_alpha); x.w = wl.w * dcelu_from_h(x.w, t.inv_alpha);
+      store_out(t, o, x);
+    }
   } else if (t.epi == EPI_BIAS_CELU) {
     float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
     if (t.bias) b = ld4(t.bias + 4 * g);
@@ -591,6 +610,8 @@ static void plan_items(UmmaPlan& pl, const std::vector<UmmaProblem>& probs, cons
         t.aux = p.aux ? p.aux + (size_t)a0 * p.ldaux + f0 : nullptr;
         t.aux_lo = p.aux_lo ? p.aux_lo + (size_t)a0 * p.ldaux + f0 : nullptr;
         t.ldaux = p.ldaux;
+        t.C_full = p.C_full ? p.C_full + (size_t)a0 * p.ldc + f0 : nullptr;
+        t.w_last = p.w_last ? p.w_last + f0 : nullptr;
         t.scale = p.scale; t.alpha = p.alpha; t.inv_alpha = p.inv_alpha;
         pl.items.push_back(t);
         pl.cost.push_back((long long)nkb * box_cycles(nt) + 1500);

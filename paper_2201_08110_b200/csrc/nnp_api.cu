@@ -72,7 +72,7 @@ extern "C" void nnp_destroy(nnp_handle* h) {
   void* ptrs[] = {h->d_eblocks, h->d_epart, h->d_ecount, h->d_mol_range, h->d_species, h->d_mol_off, h->d_mol_id, h->d_sortpos, h->d_perm, h->d_grp_off, h->d_self_energy,
                   h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_aev, h->d_daev, h->d_phi,
                   h->d_eatom, h->d_status, h->d_W, h->d_b,
-                  h->d_aev_lo, h->d_Whi, h->d_Wlo, h->d_WThi, h->d_WTlo};
+                  h->d_aev_lo, h->d_Whi, h->d_Wlo, h->d_WThi, h->d_WTlo, h->d_act_full};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (int l = 0; l < NNP_MAX_LAYERS; ++l) {
@@ -380,6 +380,12 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     }
     if (dev_alloc(&h->d_act[l], (size_t)o)) return fail(NNP_ERR_ALLOC);
     if (h->use_umma && dev_alloc(&h->d_act_lo[l], (size_t)o)) return fail(NNP_ERR_ALLOC);
+    // the last hidden layer's forward launch writes delta_{L-1} in its epilogue when it is a per-model problem
+    // (L - 1 >= 2): its h is kept as one plane for the energies
+    if (h->use_umma && l == L - 1 && L - 1 >= 2) {
+      if (dev_alloc(&h->d_act_full, (size_t)o)) return fail(NNP_ERR_ALLOC);
+      h->fuse_delta = true;
+    }
   }
 
   // ---- MLP launches (grouped GEMMs), shapes fixed at create time
@@ -540,15 +546,20 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
             p.epi = EPI_BIAS_CELU;
             probs.push_back(p);
           } else if (pass == 0) {
+            const bool last = h->fuse_delta && l == L - 1;
             for (int m = 0; m < M; ++m) {
               UmmaProblem q = p;
+              if (last) {
+                q.C_full = h->d_act_full + h->act_off[l][e] + (size_t)m * nout;
+                q.w_last = h->d_W + h->w_off[e * L + L - 1] + (size_t)m * nout;
+              }
               q.F = nout; q.K = nin;
               q.a_c0 = 0; q.a_c1 = m * nout; q.b_c0 = m * nin; q.b_c1 = 0;
               q.C = h->d_act[l] + h->act_off[l][e] + (size_t)m * nout;
               q.C_lo = h->d_act_lo[l] + h->act_off[l][e] + (size_t)m * nout;
               q.ldc = M * nout;
               q.bias = h->d_b + h->b_off[e * L + l - 1] + (size_t)m * nout;
-              q.epi = EPI_BIAS_CELU;
+              q.epi = last ? EPI_BIAS_CELU_LAST : EPI_BIAS_CELU;
               probs.push_back(q);
             }
           } else if (l > 1) {
@@ -798,7 +809,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     }
     LastLayerArgs& la = h->last;
     memset(&la, 0, sizeof(la));
-    la.act = h->d_act[L - 1]; la.act_lo = h->d_act_lo[L - 1]; la.W = h->d_W; la.bias = h->d_b; la.e_out = h->d_eatom;
+    la.act = h->d_act[L - 1]; la.act_lo = h->d_act_lo[L - 1]; la.act_full = h->fuse_delta ? h->d_act_full : nullptr; la.W = h->d_W; la.bias = h->d_b; la.e_out = h->d_eatom;
     for (int e = 0; e <= S; ++e) la.grp_off[e] = h->grp_off[e];
     for (int e = 0; e < S; ++e) {
       la.act_off[e] = ao[e]; la.w_off[e] = wo2[e]; la.b_off[e] = bo2[e]; la.H[e] = Hs[e];

@@ -77,7 +77,7 @@ struct GemmProblem {
   float alpha;  // CELU alpha
   float inv_alpha;
 };
-enum { EPI_BIAS_CELU = 0, EPI_MUL_DCELU = 1, EPI_SCALE = 2 };
+enum { EPI_BIAS_CELU = 0, EPI_MUL_DCELU = 1, EPI_SCALE = 2, EPI_BIAS_CELU_LAST = 3 };
 
 struct GemmTile {
   int prob, m0, n0, cfg;
@@ -118,6 +118,10 @@ struct UmmaItem {            // one tile of one GEMM, as the persistent CTAs con
   const float* bias;         // [f] or null
   const float* aux;          // aux[a * ldaux + f]: activations h (hi plane) for EPI_MUL_DCELU (may alias C)
   const float* aux_lo;       // lo plane of h (may alias C_lo), or null
+  // EPI_BIAS_CELU_LAST (forward through the last hidden layer): h goes to C_full as ONE plane (the 1-output layer's
+  // FP64 dot product reads it) and C / C_lo receive delta = w_last * CELU'(h), the operand of the backward pass
+  float* C_full;
+  const float* w_last;       // [f] weights of the 1-output layer for this tile's features
   float scale, alpha, inv_alpha;
 };
 struct UmmaProblem {
@@ -132,6 +136,8 @@ struct UmmaProblem {
   const float* bias;
   const float* aux;
   const float* aux_lo;
+  float* C_full;
+  const float* w_last;
   float scale, alpha, inv_alpha;
 };
 struct UmmaLaunch {
@@ -226,6 +232,7 @@ struct EnergyBlock {  // one CTA of the energy reduction: atoms [a0, a1) of mole
 struct LastLayerArgs {
   float* act;          // [n_atoms_sorted][M][H] per element group (arena), overwritten with delta
   float* act_lo;       // tensor engine: lo plane of the same arena (h = act + act_lo; delta is written split), else null
+  const float* act_full;  // tensor engine with the fused delta: h of the last hidden layer as one plane (energies only)
   const float* W;      // arena
   const float* bias;   // arena
   double* e_out;       // [n_sorted][M]
@@ -281,6 +288,8 @@ struct nnp_handle {
   // activations: act[l] for l = 1..L-1
   float* d_act[NNP_MAX_LAYERS] = {nullptr};
   float* d_act_lo[NNP_MAX_LAYERS] = {nullptr};  // tensor engine: lo planes
+  float* d_act_full = nullptr;                  // tensor engine: h_{L-1} as one plane (see EPI_BIAS_CELU_LAST)
+  bool fuse_delta = false;
   std::vector<long long> act_off[NNP_MAX_LAYERS];  // [S] float offsets
   // MLP launches
   std::vector<GemmLaunch> fwd, bwd;  // fwd: layers 1..L-1; bwd: layers L-1..1
