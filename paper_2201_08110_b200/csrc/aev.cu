@@ -187,34 +187,26 @@ __device__ __forceinline__ float gauss(float d, float khi, float klo) {
 }
 
 constexpr int AEV_THREADS = 256;  // one CTA per centre atom: 256 threads at latency-bound sizes, 128 at large N
-constexpr int TAB_FIELDS = 10;    // per radial slot: ux uy uz rhi rlo fcr dfcr fca dfca spec
+constexpr int TAB_FIELDS = 11;    // per radial slot: ux uy uz rhi rlo fcr dfcr fca dfca spec rord
 // triplets of a centre processed per pass through shared memory: small enough that 6-8 CTAs share an SM (the
 // phases of a centre are latency-bound, other centres fill the gaps), measured on configs[2] and configs[4]
 constexpr int TRIP_CHUNK_FWD = 256;
-constexpr int TRIP_CHUNK_BWD = 512;
+constexpr int TRIP_CHUNK_BWD = 512;  // upper bound; trip_chunk() halves it when that lets one more CTA share the SM
 
-// triplets per pass: enough for every centre of this handle, a multiple of 32, bounded
-static int trip_chunk(const nnp_handle* h, bool backward) {
-  const long long t = (long long)h->capA * (h->capA - 1) / 2;
-  long long c = (t + 31) / 32 * 32;
-  if (c < 32) c = 32;
-  const int cap = backward ? TRIP_CHUNK_BWD : TRIP_CHUNK_FWD;
-  if (c > cap) c = cap;
-  return (int)c;
-}
+static int trip_chunk(const nnp_handle* h, bool backward);
 static int ang_row_pad(const nnp_handle* h) {  // floats per padded angular block of the staged dE/dAEV row
   return h->aev.n_sub + 4;
 }
 
-// shared memory (floats): table | asl[capA] | sp_off[S+1] | pair_st[n_pairs] | tmp[2 capA] | pres[n_pairs+1] | kernel part
+// shared memory (floats): table | asl[capA] | sp_off[S+1] | pair_st[n_pairs] | tmp[2 capA] | pres[n_pairs+1] |
+// r_off[S+1] | kernel part
 static size_t aev_common_floats(const nnp_handle* h) {
   const int S = h->S;
-  return (size_t)TAB_FIELDS * h->capR + 3 * (size_t)h->capA + (S + 1) + (size_t)S * (S + 1) + 1;
+  return (size_t)TAB_FIELDS * h->capR + 3 * (size_t)h->capA + 2 * (S + 1) + (size_t)S * (S + 1) + 1;
 }
-size_t aev_smem_bytes(const nnp_handle* h, bool backward) {
+static size_t aev_smem_bytes_ch(const nnp_handle* h, bool backward, int CH) {
   size_t fl = aev_common_floats(h);
   const int n_pairs = h->S * (h->S + 1) / 2;
-  const int CH = trip_chunk(h, backward);
   if (!backward) {
     fl += (size_t)(h->n_feat - h->aev.n_radial);                       // angular part of the row
     fl += (size_t)(h->aev.n_shf_z + h->aev.n_shf_a) * (CH + 1);        // F1 / F2 factors of a pass (row pitch CH + 1)
@@ -225,10 +217,40 @@ size_t aev_smem_bytes(const nnp_handle* h, bool backward) {
   }
   return ((fl + 3) & ~(size_t)3) * 4 + 16;
 }
+// shape of the backward launch: threads per centre CTA and triplets per pass (see aev_block_threads)
+static void aev_bwd_shape(const nnp_handle* h, int* threads, int* chunk) {
+  const long long t = (long long)h->capA * (h->capA - 1) / 2;
+  const long long c = std::max<long long>(32, (t + 31) / 32 * 32);
+  const int big = (int)std::min<long long>(c, TRIP_CHUNK_BWD), small = (int)std::min<long long>(c, TRIP_CHUNK_BWD / 2);
+  *threads = AEV_THREADS;
+  *chunk = big;
+  if (h->N < 2048) return;
+#ifdef AEV_BWD_FORCE_THREADS
+  *threads = AEV_BWD_FORCE_THREADS;
+  *chunk = AEV_BWD_FORCE_CHUNK < big ? AEV_BWD_FORCE_CHUNK : big;
+  return;
+#endif
+  const size_t sm_bytes = 227 * 1024;
+  if ((aev_smem_bytes_ch(h, true, big) + 1024) * 8 <= sm_bytes) { *threads = 128; return; }
+  if ((aev_smem_bytes_ch(h, true, small) + 1024) * 8 <= sm_bytes) { *threads = 128; *chunk = small; }
+}
+// triplets per pass: enough for every centre of this handle, a multiple of 32, bounded
+static int trip_chunk(const nnp_handle* h, bool backward) {
+  if (backward) {
+    int th, ch;
+    aev_bwd_shape(h, &th, &ch);
+    return ch;
+  }
+  const long long t = (long long)h->capA * (h->capA - 1) / 2;
+  return (int)std::min<long long>(std::max<long long>(32, (t + 31) / 32 * 32), TRIP_CHUNK_FWD);
+}
+size_t aev_smem_bytes(const nnp_handle* h, bool backward) { return aev_smem_bytes_ch(h, backward, trip_chunk(h, backward)); }
 
 struct CentreTab {
   float *ux, *uy, *uz, *rhi, *rlo, *fcr, *dfcr, *fca, *dfca;
   int* spec;
+  int* rord;     // radial slots grouped by species (stable within a species)
+  int* r_off;    // [S+1] first position in rord of every species
   int* asl;      // angular neighbours: radial slots, sorted by species (stable)
   int* sp_off;   // [S+1] first position in asl of every species
   int* pair_st;  // [n_pairs] (s << 8) | t of every species-pair block, s <= t
@@ -242,12 +264,14 @@ __device__ __forceinline__ CentreTab carve_tab(float* smem, int capR, int capA, 
   t.ux = smem; t.uy = t.ux + capR; t.uz = t.uy + capR; t.rhi = t.uz + capR; t.rlo = t.rhi + capR;
   t.fcr = t.rlo + capR; t.dfcr = t.fcr + capR; t.fca = t.dfcr + capR; t.dfca = t.fca + capR;
   t.spec = reinterpret_cast<int*>(t.dfca + capR);
-  t.asl = t.spec + capR;
+  t.rord = t.spec + capR;
+  t.asl = t.rord + capR;
   t.sp_off = t.asl + capA;
   t.pair_st = t.sp_off + (S + 1);
   t.tmp = t.pair_st + S * (S + 1) / 2;
   t.pres = t.tmp + 2 * capA;
-  const int used = TAB_FIELDS * capR + 3 * capA + (S + 1) + S * (S + 1) + 1;
+  t.r_off = t.pres + S * (S + 1) / 2 + 1;
+  const int used = TAB_FIELDS * capR + 3 * capA + 2 * (S + 1) + S * (S + 1) + 1;
   t.rest = smem + ((used + 3) & ~3);
   return t;
 }
@@ -293,6 +317,30 @@ __device__ __forceinline__ void build_tab(const CentreTab& t, int i, int nr, int
     for (int u = s; u < c.S; ++u) t.pair_st[p++] = (s << 8) | u;
   }
   __syncthreads();
+  if (want_pres) {
+    // radial slots grouped by species, list order kept within a species (ballot compaction, one warp per species):
+    // a radial column then visits the neighbours of ITS species only, in the order the full loop would add them
+    const int lane = threadIdx.x & 31;
+    for (int s = threadIdx.x >> 5; s < c.S; s += (int)(blockDim.x >> 5)) {
+      int less = 0;
+      for (int q0 = 0; q0 < nr; q0 += 32) {
+        const int q = q0 + lane;
+        less += __popc(__ballot_sync(FULL, q < nr && t.spec[q] < s));
+      }
+      int pos = less;
+      for (int q0 = 0; q0 < nr; q0 += 32) {
+        const int q = q0 + lane;
+        const bool m = q < nr && t.spec[q] == s;
+        const unsigned b = __ballot_sync(FULL, m);
+        if (m) t.rord[pos + __popc(b & ((1u << lane) - 1u))] = q;
+        pos += __popc(b);
+      }
+      if (lane == 0) {
+        t.r_off[s] = less;
+        if (s == c.S - 1) t.r_off[c.S] = pos;
+      }
+    }
+  }
   // the angular slots and their species, staged once (the sort below reads them na times)
   for (int q = threadIdx.x; q < na; q += blockDim.x) {
     const int slot = nbr_a[(size_t)i * capA + q];
@@ -364,8 +412,11 @@ __device__ __forceinline__ void trip_decode(int t, int na, int& a, int& b) {
 //                    species.  Fixed order, no atomics.
 // NZ / NA are the register-array bounds (n_shf_z <= NZ, n_shf_a <= NA).
 // ------------------------------------------------------------------------------------------------
+// 4 CTAs of 256 threads (8 of 128 at large N) per SM: 64 registers per thread.  A bound of 6 (40 registers) spilled in
+// the backward kernel and measured 8-11 % slower at configs[4]; shared memory, not registers, limits residency there.
+constexpr int AEV_MINB = 4;
 template <int NZ, int NA>
-__global__ void __launch_bounds__(AEV_THREADS, 6) aev_forward_kernel(
+__global__ void __launch_bounds__(AEV_THREADS, AEV_MINB) aev_forward_kernel(
     const float4* __restrict__ pos4, const int* __restrict__ nbr_r, const int* __restrict__ nbr_a,
     const int* __restrict__ cnt_r, const int* __restrict__ cnt_a, const int* __restrict__ sortpos, int N,
     const __grid_constant__ AevConst c, int capR, int capA, int CH, float* __restrict__ aev, float* __restrict__ aev_lo,
@@ -414,11 +465,12 @@ __global__ void __launch_bounds__(AEV_THREADS, 6) aev_forward_kernel(
     const int s = col / c.n_shf_r, k = col % c.n_shf_r;
     const float shf = c.shf_r[k];
     float acc = 0.0f;
+    const int p1 = t.r_off[s + 1];
 #pragma unroll 4
-    for (int q = 0; q < nr; ++q) {  // predicated (no branch): the exponentials of consecutive neighbours overlap
+    for (int p = t.r_off[s]; p < p1; ++p) {  // the neighbours of species s, in list order
+      const int q = t.rord[p];
       const float d = (t.rhi[q] - shf) + t.rlo[q];
-      const float v = 0.25f * gauss(d, c.kr_hi, c.kr_lo) * t.fcr[q];
-      acc += t.spec[q] == s ? v : 0.0f;
+      acc += 0.25f * gauss(d, c.kr_hi, c.kr_lo) * t.fcr[q];
     }
     if (out_lo) {
       const float hi = __uint_as_float((__float_as_uint(acc) + 0x1000u) & 0xFFFFE000u);
@@ -510,7 +562,7 @@ __device__ __forceinline__ float warp_sum(float v) {
 // MULTI: dE/dAEV arrives as several partial rows (ligand sizes, one per model); a separate instantiation so that its
 // wider load batch does not cost the large-system instantiation registers (occupancy)
 template <int NZ, int NA, bool MULTI>
-__global__ void __launch_bounds__(AEV_THREADS, MULTI ? 4 : 6) aev_backward_kernel(
+__global__ void __launch_bounds__(AEV_THREADS, MULTI ? 4 : AEV_MINB) aev_backward_kernel(
     const float4* __restrict__ pos4, const int* __restrict__ nbr_r, const int* __restrict__ nbr_a,
     const int* __restrict__ cnt_r, const int* __restrict__ cnt_a, const int* __restrict__ sortpos, int N,
     const __grid_constant__ AevConst c, int capR, int capA, int CH, const float* __restrict__ daev, int n_parts,
@@ -531,7 +583,9 @@ __global__ void __launch_bounds__(AEV_THREADS, MULTI ? 4 : 6) aev_backward_kerne
   const int nr = cnt_r[i], na = cnt_a[i];
   const float* gin = daev + (size_t)sortpos[i] * c.n_feat;
   // dE/dAEV row = fixed-order sum of the partial rows.  All loads of a pass (KC columns x 8 partial rows per thread)
-  // are issued before the first add: one memory latency per pass instead of one per partial row
+  // are issued before the first add: one memory latency per pass instead of one per partial row.  (Loading only the
+  // columns this centre can touch -- after the table is built -- saves 9 % of the instructions and LOSES 5 % of the
+  // time at configs[4]: the row load then sits on the centre's dependency chain instead of under the table build.)
   if (n_parts == 1) {  // large systems: one row, keep as many columns in flight as possible
     for (int fb = 0; fb < c.n_feat; fb += 8 * (int)blockDim.x) {
       float x[8];
@@ -840,7 +894,10 @@ static bool aev_small_shape(const nnp_handle* h) { return h->aev.n_shf_z <= 4 &&
 // backward: 33 KB per CTA, 6 per SM either way, where the wider CTA wins; measured both ways)
 static int aev_block_threads(const nnp_handle* h, bool backward) {
   if (h->N < 2048) return AEV_THREADS;
-  return (!backward || aev_smem_bytes(h, true) * 10 <= 227 * 1024) ? 128 : AEV_THREADS;
+  if (!backward) return 128;
+  int th, ch;
+  aev_bwd_shape(h, &th, &ch);
+  return th;
 }
 
 void launch_aev_forward(nnp_handle* h, const float* d_pos, int pos_stride, const int* d_atom_index, cudaStream_t s) {
