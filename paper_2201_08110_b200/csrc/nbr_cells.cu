@@ -159,21 +159,28 @@ __global__ void __launch_bounds__(GRID_THREADS) cell_scan_kernel(const CellGrid*
   if (threadIdx.x == 0) cell_start[n] = carry;
 }
 
+// atoms in cell order: index, position and molecule side by side, so that the sweep below reads three coalesced,
+// INDEPENDENT streams (index -> molecule -> position was a chain of three dependent gathers per candidate batch)
 __global__ void __launch_bounds__(256) cell_fill_kernel(int N, const int* __restrict__ cell_of,
                                                         const int* __restrict__ cell_rank,
-                                                        const int* __restrict__ cell_start, int* __restrict__ cell_atoms) {
+                                                        const int* __restrict__ cell_start, const float4* __restrict__ pos4,
+                                                        const int* __restrict__ mol_id, int* __restrict__ cell_atoms,
+                                                        float4* __restrict__ cell_pos4, int* __restrict__ cell_mol) {
   pdl_trigger();
   pdl_wait();
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
-  cell_atoms[cell_start[cell_of[i]] + cell_rank[i]] = i;
+  const int dst = cell_start[cell_of[i]] + cell_rank[i];
+  cell_atoms[dst] = i;
+  cell_pos4[dst] = pos4[i];
+  cell_mol[dst] = mol_id[i];
 }
 
 // warp per centre; dynamic shared memory: [NBRC_WARPS][2][capR] ints (compacted row, sorted row)
 __global__ void __launch_bounds__(NBRC_WARPS * 32) nbr_cells_kernel(
     const float4* __restrict__ pos4, const int* __restrict__ mol_id, const CellGrid* __restrict__ grid,
-    const int* __restrict__ cell_of, const int* __restrict__ cell_start, const int* __restrict__ cell_atoms, int N,
-    double rc_r2, double rc_a2, int capR, int capA, int* __restrict__ nbr_r, int* __restrict__ nbr_a,
+    const int* __restrict__ cell_of, const int* __restrict__ cell_start, const int* __restrict__ cell_atoms,
+    const float4* __restrict__ cell_pos4, const int* __restrict__ cell_mol, int N, double rc_r2, double rc_a2, int capR, int capA, int* __restrict__ nbr_r, int* __restrict__ nbr_a,
     int* __restrict__ cnt_r, int* __restrict__ cnt_a, int* __restrict__ status) {
   extern __shared__ int rows_smem[];
   pdl_trigger();
@@ -189,35 +196,41 @@ __global__ void __launch_bounds__(NBRC_WARPS * 32) nbr_cells_kernel(
   const int ci = cell_of[i];
   const int cx = ci % g.nx, cy = (ci / g.nx) % g.ny, cz = ci / (g.nx * g.ny);
   const unsigned below = (1u << lane) - 1u;
-  int nr = 0;
-  for (int dz = -1; dz <= 1; ++dz) {
-    const int z = cz + dz;
-    if (z < 0 || z >= g.nz) continue;
-    for (int dy = -1; dy <= 1; ++dy) {
-      const int y = cy + dy;
-      if (y < 0 || y >= g.ny) continue;
-      // the (up to) three cells of an x-run are contiguous in the cell order, hence in cell_atoms
+  // the nine x-runs of the 27-cell neighbourhood (the up to three cells of a run are contiguous in the cell order):
+  // lane r < 9 fetches the atom range of run r, so the range lookups of all runs are one memory round trip
+  int my_s0 = 0, my_s1 = 0;
+  if (lane < 9) {
+    const int z = cz + lane / 3 - 1, y = cy + lane % 3 - 1;
+    if (z >= 0 && z < g.nz && y >= 0 && y < g.ny) {
       const int x0 = max(cx - 1, 0), x1 = min(cx + 1, g.nx - 1);
       const int c0 = (z * g.ny + y) * g.nx + x0;
-      const int s0 = cell_start[c0], s1 = cell_start[c0 + (x1 - x0) + 1];
-      for (int base = s0; base < s1; base += 32) {
-        const int idx = base + lane;
-        const int j = idx < s1 ? cell_atoms[idx] : -1;
-        bool in_r = false, in_a = false;
-        if (j >= 0 && j != i && mol_id[j] == m) {
-          const float4 pj = pos4[j];
-          const double dx = (double)pj.x - (double)pi.x;
-          const double dy2 = (double)pj.y - (double)pi.y;
-          const double dz2 = (double)pj.z - (double)pi.z;
-          const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy2, dy2)), __dmul_rn(dz2, dz2));
-          in_r = d2 <= rc_r2;
-          in_a = d2 <= rc_a2;
-        }
-        const unsigned br = __ballot_sync(FULLMASK, in_r);
-        const int slot = nr + __popc(br & below);
-        if (in_r && slot < capR) row[slot] = j | (in_a ? (int)0x80000000 : 0);
-        nr += __popc(br);
+      my_s0 = cell_start[c0];
+      my_s1 = cell_start[c0 + (x1 - x0) + 1];
+    }
+  }
+  int nr = 0;
+  for (int run = 0; run < 9; ++run) {
+    const int s0 = __shfl_sync(FULLMASK, my_s0, run), s1 = __shfl_sync(FULLMASK, my_s1, run);
+    for (int base = s0; base < s1; base += 32) {
+      const int idx = base + lane;
+      const bool live = idx < s1;
+      const int j = live ? cell_atoms[idx] : -1;
+      const int mj = live ? cell_mol[idx] : -1;
+      float4 pj = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (live) pj = cell_pos4[idx];
+      bool in_r = false, in_a = false;
+      if (live && j != i && mj == m) {
+        const double dx = (double)pj.x - (double)pi.x;
+        const double dy2 = (double)pj.y - (double)pi.y;
+        const double dz2 = (double)pj.z - (double)pi.z;
+        const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy2, dy2)), __dmul_rn(dz2, dz2));
+        in_r = d2 <= rc_r2;
+        in_a = d2 <= rc_a2;
       }
+      const unsigned br = __ballot_sync(FULLMASK, in_r);
+      const int slot = nr + __popc(br & below);
+      if (in_r && slot < capR) row[slot] = j | (in_a ? (int)0x80000000 : 0);
+      nr += __popc(br);
     }
   }
   __syncwarp();
@@ -257,6 +270,8 @@ int cells_alloc(nnp_handle* h) {
   if (cudaMalloc((void**)&h->d_cell_of, sizeof(int) * N) != cudaSuccess) return -1;
   if (cudaMalloc((void**)&h->d_cell_rank, sizeof(int) * N) != cudaSuccess) return -1;
   if (cudaMalloc((void**)&h->d_cell_atoms, sizeof(int) * N) != cudaSuccess) return -1;
+  if (cudaMalloc((void**)&h->d_cell_mol, sizeof(int) * N) != cudaSuccess) return -1;
+  if (cudaMalloc((void**)&h->d_cell_pos4, sizeof(float4) * N) != cudaSuccess) return -1;
   const size_t smem = (size_t)NBRC_WARPS * 2 * h->capR * sizeof(int);
   if (smem > 48 * 1024 &&
       cudaFuncSetAttribute((const void*)nbr_cells_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
@@ -265,7 +280,8 @@ int cells_alloc(nnp_handle* h) {
 }
 
 void cells_free(nnp_handle* h) {
-  void* ptrs[] = {h->d_cell_grid, h->d_cell_count, h->d_cell_start, h->d_cell_of, h->d_cell_rank, h->d_cell_atoms};
+  void* ptrs[] = {h->d_cell_grid, h->d_cell_count, h->d_cell_start, h->d_cell_of, h->d_cell_rank, h->d_cell_atoms,
+                  h->d_cell_mol,  h->d_cell_pos4};
   for (void* p : ptrs)
     if (p) cudaFree(p);
 }
@@ -283,10 +299,12 @@ void launch_neighbors_cells(nnp_handle* h, const float* d_pos, int pos_stride, c
   launch_kernel(pdl, cell_scan_kernel, dim3(1), dim3(GRID_THREADS), 0, s, (const CellGrid*)grid,
                 (const int*)h->d_cell_count, h->d_cell_start);
   launch_kernel(pdl, cell_fill_kernel, dim3((N + 255) / 256), dim3(256), 0, s, N, (const int*)h->d_cell_of,
-                (const int*)h->d_cell_rank, (const int*)h->d_cell_start, h->d_cell_atoms);
+                (const int*)h->d_cell_rank, (const int*)h->d_cell_start, (const float4*)h->d_pos4, (const int*)h->d_mol_id,
+                h->d_cell_atoms, h->d_cell_pos4, h->d_cell_mol);
   const size_t smem = (size_t)NBRC_WARPS * 2 * h->capR * sizeof(int);
   launch_kernel(pdl, nbr_cells_kernel, dim3((N + NBRC_WARPS - 1) / NBRC_WARPS), dim3(NBRC_WARPS * 32), smem, s,
                 (const float4*)h->d_pos4, (const int*)h->d_mol_id, (const CellGrid*)grid, (const int*)h->d_cell_of,
-                (const int*)h->d_cell_start, (const int*)h->d_cell_atoms, N, h->aev.rc_r2, h->aev.rc_a2, h->capR, h->capA,
+                (const int*)h->d_cell_start, (const int*)h->d_cell_atoms, (const float4*)h->d_cell_pos4,
+                (const int*)h->d_cell_mol, N, h->aev.rc_r2, h->aev.rc_a2, h->capR, h->capA,
                 h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_status);
 }

@@ -277,7 +277,8 @@ struct nnp_handle {
   bool fuse_nbr = false;  // small molecules: the AEV forward kernel builds the neighbour rows itself
   void* d_cell_grid = nullptr;
   int *d_cell_count = nullptr, *d_cell_start = nullptr, *d_cell_of = nullptr, *d_cell_rank = nullptr,
-      *d_cell_atoms = nullptr;
+      *d_cell_atoms = nullptr, *d_cell_mol = nullptr;  // cell_mol: molecule of every atom, in cell order
+  float4* d_cell_pos4 = nullptr;                        // positions (+ species) in cell order
   int* d_status = nullptr;
   // weights
   float *d_W = nullptr, *d_b = nullptr;
