@@ -566,7 +566,7 @@ __global__ void __launch_bounds__(AEV_THREADS, MULTI ? 4 : AEV_MINB) aev_backwar
     const float4* __restrict__ pos4, const int* __restrict__ nbr_r, const int* __restrict__ nbr_a,
     const int* __restrict__ cnt_r, const int* __restrict__ cnt_a, const int* __restrict__ sortpos, int N,
     const __grid_constant__ AevConst c, int capR, int capA, int CH, const float* __restrict__ daev, int n_parts,
-    size_t part_stride, float* __restrict__ phi) {
+    size_t part_stride, unsigned long long live_boxes, float* __restrict__ phi) {
   extern __shared__ __align__(16) float smem[];
   const int i = blockIdx.x;
   const CentreTab t = carve_tab(smem, capR, capA, c.S);
@@ -582,55 +582,63 @@ __global__ void __launch_bounds__(AEV_THREADS, MULTI ? 4 : AEV_MINB) aev_backwar
   const float4 pi = pos4[i];
   const int nr = cnt_r[i], na = cnt_a[i];
   const float* gin = daev + (size_t)sortpos[i] * c.n_feat;
-  // dE/dAEV row = fixed-order sum of the partial rows.  All loads of a pass (KC columns x 8 partial rows per thread)
-  // are issued before the first add: one memory latency per pass instead of one per partial row.  (Loading only the
-  // columns this centre can touch -- after the table is built -- saves 9 % of the instructions and LOSES 5 % of the
-  // time at configs[4]: the row load then sits on the centre's dependency chain instead of under the table build.)
-  if (n_parts == 1) {  // large systems: one row, keep as many columns in flight as possible
-    for (int fb = 0; fb < c.n_feat; fb += 8 * (int)blockDim.x) {
-      float x[8];
-#pragma unroll
-      for (int k = 0; k < 8; ++k) {
-        const int f = fb + k * (int)blockDim.x + threadIdx.x;
-        x[k] = f < c.n_feat ? gin[f] : 0.0f;
+  // dE/dAEV row = fixed-order sum of the partial rows, staged in shared memory (angular blocks padded).  A warp takes
+  // 32-column boxes of the row; the boxes that hold only structural zeros (species that do not occur in the system:
+  // `live_boxes`, the mask layer 1 skips by) are never read below and are not loaded (water: 8 of 32 boxes).  All
+  // loads of a pass are issued before the first add: one memory latency per pass, not one per partial row.
+  // (Loading only the columns THIS centre touches -- known after the table is built -- saves more instructions and
+  // LOSES 5 % of the time at configs[4]: the row load then sits on the centre's dependency chain.)
+  {
+    const int nbox = (c.n_feat + 31) >> 5;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+    const unsigned long long live = live_boxes ? live_boxes : ~0ull;
+    const int sub_shift = (c.n_sub & (c.n_sub - 1)) == 0 ? __ffs(c.n_sub) - 1 : -1;  // n_sub = 32 for ANI-1x / ANI-2x
+    auto put = [&](int f, float v) {
+      if (f < c.n_radial) {
+        g[f] = v;
+      } else {
+        const int fa = f - c.n_radial;
+        const int blk = sub_shift >= 0 ? fa >> sub_shift : fa / c.n_sub;
+        gang[blk * bpad + (fa - blk * c.n_sub)] = v;
       }
+    };
+    constexpr int KB = MULTI ? 4 : 8;  // boxes per warp and pass
+    for (int b0 = warp; b0 < nbox; b0 += KB * nw) {
+      if (!MULTI) {  // large systems: one row
+        float x[KB];
 #pragma unroll
-      for (int k = 0; k < 8; ++k) {
-        const int f = fb + k * (int)blockDim.x + threadIdx.x;
-        if (f < c.n_radial) g[f] = x[k];
-        else if (f < c.n_feat) {
-          const int fa = f - c.n_radial, blk = fa / c.n_sub;
-          gang[blk * bpad + (fa - blk * c.n_sub)] = x[k];
+        for (int k = 0; k < KB; ++k) {
+          const int bx = b0 + k * nw, f = bx * 32 + lane;
+          x[k] = (bx < nbox && ((live >> bx) & 1ull) && f < c.n_feat) ? gin[f] : 0.0f;
         }
-      }
-    }
-  }
-  constexpr int KC = MULTI ? 4 : 2;  // columns per thread and pass: KC x 8 loads in flight before the first add
-  for (int fb = 0; n_parts > 1 && fb < c.n_feat; fb += KC * (int)blockDim.x) {
-    float acc[KC];
 #pragma unroll
-    for (int k = 0; k < KC; ++k) acc[k] = 0.0f;
-    for (int p0 = 0; p0 < n_parts; p0 += 8) {
-      float x[KC][8];
+        for (int k = 0; k < KB; ++k) {
+          const int bx = b0 + k * nw, f = bx * 32 + lane;
+          if (bx < nbox && ((live >> bx) & 1ull) && f < c.n_feat) put(f, x[k]);
+        }
+      } else {
+        float acc[KB];
 #pragma unroll
-      for (int k = 0; k < KC; ++k) {
-        const int f = fb + k * (int)blockDim.x + threadIdx.x;
+        for (int k = 0; k < KB; ++k) acc[k] = 0.0f;
+        for (int p0 = 0; p0 < n_parts; p0 += 8) {
+          float x[KB][8];
 #pragma unroll
-        for (int u = 0; u < 8; ++u)
-          x[k][u] = (f < c.n_feat && p0 + u < n_parts) ? gin[(size_t)(p0 + u) * part_stride + f] : 0.0f;
-      }
+          for (int k = 0; k < KB; ++k) {
+            const int bx = b0 + k * nw, f = bx * 32 + lane;
+            const bool on = bx < nbox && ((live >> bx) & 1ull) && f < c.n_feat;
 #pragma unroll
-      for (int k = 0; k < KC; ++k)
+            for (int u = 0; u < 8; ++u) x[k][u] = (on && p0 + u < n_parts) ? gin[(size_t)(p0 + u) * part_stride + f] : 0.0f;
+          }
 #pragma unroll
-        for (int u = 0; u < 8; ++u) acc[k] += x[k][u];
-    }
+          for (int k = 0; k < KB; ++k)
 #pragma unroll
-    for (int k = 0; k < KC; ++k) {
-      const int f = fb + k * (int)blockDim.x + threadIdx.x;
-      if (f < c.n_radial) g[f] = acc[k];
-      else if (f < c.n_feat) {
-        const int fa = f - c.n_radial, blk = fa / c.n_sub;
-        gang[blk * bpad + (fa - blk * c.n_sub)] = acc[k];
+            for (int u = 0; u < 8; ++u) acc[k] += x[k][u];
+        }
+#pragma unroll
+        for (int k = 0; k < KB; ++k) {
+          const int bx = b0 + k * nw, f = bx * 32 + lane;
+          if (bx < nbox && ((live >> bx) & 1ull) && f < c.n_feat) put(f, acc[k]);
+        }
       }
     }
   }
@@ -927,7 +935,7 @@ static void launch_aev_backward_t(nnp_handle* h, cudaStream_t s) {
   launch_kernel(h->pdl_now, aev_backward_kernel<NZ, NA, MULTI>, dim3(h->N), dim3(aev_block_threads(h, true)), aev_smem_bytes(h, true), s,
                 (const float4*)h->d_pos4, (const int*)h->d_nbr_r, (const int*)h->d_nbr_a, (const int*)h->d_cnt_r,
                 (const int*)h->d_cnt_a, (const int*)h->d_sortpos, h->N, h->aev, h->capR, h->capA, trip_chunk(h, true),
-                (const float*)h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->d_phi);
+                (const float*)h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->aev_live_boxes, h->d_phi);
 }
 
 void launch_aev_backward(nnp_handle* h, cudaStream_t s) {

@@ -499,6 +499,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     }
     if (!any_dead) l1_kmask = l1_fmask = 0;  // nothing to skip
   }
+  h->aev_live_boxes = l1_kmask;  // the AEV backward kernel loads only these 32-column boxes of a dE/dAEV row
   if (h->use_umma) {
     // tcgen05 engine: D[f][a] = sum_k W[f][k] X[a][k].  Layer 1 forward runs all models of an element as ONE
     // problem (their weight rows are contiguous and they share the AEV input): F = M*H1 is a multiple of 128.

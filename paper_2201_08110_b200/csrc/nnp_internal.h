@@ -278,6 +278,7 @@ struct nnp_handle {
   void* d_cell_grid = nullptr;
   int *d_cell_count = nullptr, *d_cell_start = nullptr, *d_cell_of = nullptr, *d_cell_rank = nullptr,
       *d_cell_atoms = nullptr, *d_cell_mol = nullptr;  // cell_mol: molecule of every atom, in cell order
+  unsigned long long aev_live_boxes = 0;  // 32-column boxes of the AEV that are not structural zeros (0: all)
   float4* d_cell_pos4 = nullptr;                        // positions (+ species) in cell order
   int* d_status = nullptr;
   // weights
