@@ -22,6 +22,7 @@ NNP_FLAG_NO_PDL = 32
 NNP_FLAG_NO_CELLS = 64
 NNP_FLAG_FORCE_CELLS = 128
 NNP_FLAG_NO_FWD1 = 256
+NNP_FLAG_NO_SWEEP_REVERSAL = 512
 NNP_FLAG_NO_NBR_FUSION = 1024
 NNP_FLAG_NO_ZERO_SKIP = 2048
 ERRORS = {

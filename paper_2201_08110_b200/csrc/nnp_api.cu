@@ -592,7 +592,8 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
         }
         UmmaLaunch ul;
         ul.name = (pass == 0 ? "mlp_fwd_l" : "mlp_bwd_l") + std::to_string(l);
-        if (umma_build_launch(ul, probs, aops, bops, prop.multiProcessorCount)) {
+        const bool reverse = !(cfg->flags & NNP_FLAG_NO_SWEEP_REVERSAL) && ((pass * (L - 1) + li) & 1) == 0;
+        if (umma_build_launch(ul, probs, aops, bops, prop.multiProcessorCount, reverse)) {
           umma_free_launch(ul);
           return fail(NNP_ERR_CUDA);
         }

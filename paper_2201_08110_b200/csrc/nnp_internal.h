@@ -151,7 +151,7 @@ struct UmmaLaunch {
 };
 int umma_init();
 int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, const std::vector<UmmaOperand>& aops,
-                      const std::vector<UmmaOperand>& bops, int num_sms);
+                      const std::vector<UmmaOperand>& bops, int num_sms, bool reverse = false);
 void umma_launch(const UmmaLaunch& L, cudaStream_t s, bool pdl);
 void umma_free_launch(UmmaLaunch& L);
 

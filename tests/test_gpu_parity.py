@@ -16,7 +16,8 @@ from oracle.ani_oracle import AniOracle  # noqa: E402
 from paper_2201_08110_b200 import workloads as wl  # noqa: E402
 from paper_2201_08110_b200.binding import (NNP, NNP_FLAG_FORCE_CELLS, NNP_FLAG_NO_CELLS, NNP_FLAG_NO_GRAPH,  # noqa: E402
                                             NNP_FLAG_NO_FWD1, NNP_FLAG_NO_MID, NNP_FLAG_NO_NBR_FUSION, NNP_FLAG_NO_PDL, NNP_FLAG_NO_SMALL,
-                                            NNP_FLAG_NO_UMMA, NNP_FLAG_NO_ZERO_SKIP, NNPError)
+                                            NNP_FLAG_NO_UMMA, NNP_FLAG_NO_ZERO_SKIP, NNP_FLAG_NO_SWEEP_REVERSAL,
+                                            NNPError)
 
 # MLP engines: ligand-size weight-streaming FFMA (default at these sizes; with the fused middle launch or
 # one launch per layer), tcgen05 3xTF32 (default at large sizes), grouped FFMA GEMMs (the engine of shapes the
@@ -314,6 +315,18 @@ def test_structural_zero_skipping_changes_nothing():
     assert np.abs(ra["F"] - rb["F"]).max() <= 2e-4
     assert np.abs(ra["dG"][:, live] - rb["dG"][:, live]).max() <= 1e-6
     assert np.any(rb["dG"][:, ~live] != 0.0) and np.all(ra["dG"][:, 896:] == 0.0)  # tile 7 (columns 896..1007) is dead
+    a.destroy(); b.destroy()
+
+
+def test_sweep_direction_of_tensor_launches_changes_nothing():
+    """Consecutive tensor-engine launches sweep the (element, model) blocks in opposite directions (L2 reuse); the
+    schedule does not touch the arithmetic of a tile: same bits as with every launch in the same direction."""
+    w = wl.config4()
+    W, B = w.weights()
+    a = NNP(w.params, W, B, w.species)
+    b = NNP(w.params, W, B, w.species, flags=NNP_FLAG_NO_SWEEP_REVERSAL)
+    ra, rb = gpu_eval(a, w.positions), gpu_eval(b, w.positions)
+    assert np.array_equal(ra["E"], rb["E"]) and np.array_equal(ra["F"], rb["F"])
     a.destroy(); b.destroy()
 
 
