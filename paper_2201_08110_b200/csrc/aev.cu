@@ -645,26 +645,25 @@ __global__ void __launch_bounds__(AEV_THREADS, MULTI ? 4 : AEV_MINB) aev_backwar
   for (int f = threadIdx.x; f < 3 * nr; f += blockDim.x) pha[f] = 0.0f;
   build_tab(t, i, nr, na, pi, pos4, nbr_r, nbr_a, capR, capA, c, false);
 
-  // ---- radial: dT/dr = 0.25 e (f_C' - 2 eta (r - Shf) f_C); a group of lanes per neighbour
+  // ---- radial: dT/dr = 0.25 e (f_C' - 2 eta (r - Shf) f_C); four lanes per neighbour, each takes every fourth
+  // shift (a 16-lane group per neighbour spent half of its instructions in the shuffle tree)
   {
-    const int glanes = c.n_shf_r <= 16 ? 16 : 32;
-    const int groups = blockDim.x / glanes;
-    const int grp = threadIdx.x / glanes, k = threadIdx.x % glanes;
-    for (int q0 = 0; q0 < nr; q0 += groups) {
-      const int q = q0 + grp;
+    const int q4 = threadIdx.x >> 2, l4 = threadIdx.x & 3, per_pass = blockDim.x >> 2;
+    for (int q0 = 0; q0 < nr; q0 += per_pass) {
+      const int q = q0 + q4;
       float v = 0.0f;
-      if (q < nr && k < c.n_shf_r) {
-        const float d = (t.rhi[q] - c.shf_r[k]) + t.rlo[q];
-        const float ex = 0.25f * gauss(d, c.kr_hi, c.kr_lo);
-        const float dT = ex * (t.dfcr[q] - 2.0f * c.eta_r * d * t.fcr[q]);
-        v = g[t.spec[q] * c.n_shf_r + k] * dT;
+      if (q < nr) {
+        const float rh = t.rhi[q], rl = t.rlo[q], fc = t.fcr[q], dfc = t.dfcr[q];
+        const float* gs = g + t.spec[q] * c.n_shf_r;
+        for (int k = l4; k < c.n_shf_r; k += 4) {
+          const float d = (rh - c.shf_r[k]) + rl;
+          const float ex = 0.25f * gauss(d, c.kr_hi, c.kr_lo);
+          v = fmaf(gs[k], ex * (dfc - 2.0f * c.eta_r * d * fc), v);
+        }
       }
-      for (int o = glanes >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
-      if (q < nr && k == 0) {
-        phr[3 * q + 0] = v * t.ux[q];
-        phr[3 * q + 1] = v * t.uy[q];
-        phr[3 * q + 2] = v * t.uz[q];
-      }
+      v += __shfl_xor_sync(FULL, v, 1);
+      v += __shfl_xor_sync(FULL, v, 2);
+      if (q < nr && l4 < 3) phr[3 * q + l4] = v * (l4 == 0 ? t.ux[q] : l4 == 1 ? t.uy[q] : t.uz[q]);
     }
   }
 
