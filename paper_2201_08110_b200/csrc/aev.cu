@@ -526,6 +526,7 @@ __global__ void __launch_bounds__(AEV_THREADS, AEV_MINB) aev_forward_kernel(
         const int base = trip_row_start(a, na) - a - 1 - c0;  // local index of (a, b) is base + b
         const int lo = max(s == u ? a + 1 : b0, -base);
         const int hi = min(b1, cn - base);
+#pragma unroll 4
         for (int b = lo; b < hi; ++b) acc = fmaf(f1[base + b], f2[base + b], acc);
       }
       row[f] += acc;
