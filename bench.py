@@ -199,14 +199,28 @@ def stage_rooflines(w, nnp, stages, config, peaks):
     elif tensor:
         ceiling = peaks["tf32x3_ceiling_tflops"]
         tsrc = "measured: nnp_measure_peaks tcgen05 kind::tf32 rate / 3 (3xTF32 issues 3 MMAs per useful MAC)"
+        abytes = nnp.stage_bytes()
         for l in range(1, L):
             for st in (f"mlp_fwd_l{l}", f"mlp_bwd_l{l}"):
                 fl, tile = issued.get(st, (0.0, 0))
-                add(st, "gemm_umma_kernel", "tensor", fl, "TFLOP/s", ceiling, tsrc,
-                    "flops actually issued (structural-zero boxes skipped, padding excluded)",
-                    {"dense_nominal_flops": 2.0 * mac[l], "issued_fraction": fl / (2.0 * mac[l]) if mac[l] else None,
-                     "atom_tile": tile, "frac_of_tf32_peak": None if stages.get(st, 0) <= 0 else
-                     fl / (stages[st] * 1e-6) / 1e12 / peaks["tf32_tcgen05_tflops"]})
+                by = abytes.get(st, 0.0)
+                if stages.get(st, 0) <= 0:
+                    continue
+                t = stages[st] * 1e-6
+                tfrac = fl / t / 1e12 / ceiling
+                hfrac = by / t / 1e9 / peaks["hbm_copy_gbs"]
+                extra = {"dense_nominal_flops": 2.0 * mac[l], "issued_fraction": fl / (2.0 * mac[l]) if mac[l] else None,
+                         "atom_tile": tile, "frac_of_tf32_peak": fl / t / 1e12 / peaks["tf32_tcgen05_tflops"],
+                         "tensor_frac": tfrac, "hbm_frac": hfrac, "issued_flops": fl, "algorithmic_bytes": by}
+                # a launch is bound by whichever of its two rooflines it is closer to: the hidden-layer launches of a
+                # large system stream split activation planes that do not fit L2
+                if hfrac > tfrac and by > 126e6:  # below the L2 size the planes of a launch never leave the L2
+                    add(st, "gemm_umma_kernel", "hbm", by, "GB/s", peaks["hbm_copy_gbs"], peaks["hbm_copy_source"],
+                        "algorithmic bytes (nnp_get_stage_bytes): operand planes, output planes and epilogue reads, each once",
+                        extra)
+                else:
+                    add(st, "gemm_umma_kernel", "tensor", fl, "TFLOP/s", ceiling, tsrc,
+                        "flops actually issued (structural-zero boxes skipped, padding excluded)", extra)
     else:  # grouped FP32 FFMA GEMMs (shapes outside the tensor engine)
         for l in range(1, L):
             for st in (f"mlp_fwd_l{l}", f"mlp_bwd_l{l}"):

@@ -205,6 +205,11 @@ int nnp_get_work(nnp_handle *h, double *what_host, int32_t n);
  * valid rows x atoms of every contraction box it runs; boxes of structural zeros are skipped and not counted) and the
  * atom-tile width chosen for it; 0 / 0 for other stages.  Either pointer may be NULL. */
 int nnp_get_stage_work(nnp_handle *h, int32_t stage, double *issued_flops_host, int32_t *atom_tile_host);
+/* Per stage: ALGORITHMIC bytes of a tensor-engine launch -- every operand plane it reads counted once (weights and
+ * activations, hi and lo planes, only the contraction boxes it runs), the planes it writes once, and the activations
+ * its epilogue reads once; 0 for other stages.  The hidden-layer launches of a large system move more bytes per flop
+ * than the layer-1 launches and are bound by this number, not by the tensor pipe. */
+int nnp_get_stage_bytes(nnp_handle *h, int32_t stage, double *bytes_host);
 
 /*
  * nnp_measure_peaks (measurement only): micro-benchmarks on the current device; peaks_host f64[n], n <= 4:

@@ -39,7 +39,7 @@ SYMBOLS = (
     "nnp_create", "nnp_compute", "nnp_compute_host", "nnp_status", "nnp_destroy", "nnp_error_string",
     "nnp_launches_per_compute", "nnp_set_profiling", "nnp_get_stage_times", "nnp_stage_name", "nnp_get_work",
     "nnp_debug_pairs", "nnp_debug_aev", "nnp_debug_atomic_energies", "nnp_debug_daev", "nnp_n_features",
-    "nnp_get_stage_work", "nnp_create_from_file", "nnp_compute_fixed", "nnp_compute_async", "nnp_measure_peaks",
+    "nnp_get_stage_work", "nnp_get_stage_bytes", "nnp_create_from_file", "nnp_compute_fixed", "nnp_compute_async", "nnp_measure_peaks",
     "nnp_coupling_create", "nnp_coupling_compute", "nnp_coupling_compute_fixed", "nnp_coupling_destroy",
 )
 FIXED_ONE = float(1 << 32)  # 64-bit fixed-point force format: round(F * 2^32)
@@ -125,6 +125,8 @@ def load_library():
         lib.nnp_n_features.argtypes = [C.c_void_p]
         lib.nnp_get_stage_work.restype = C.c_int
         lib.nnp_get_stage_work.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_int32)]
+        lib.nnp_get_stage_bytes.restype = C.c_int
+        lib.nnp_get_stage_bytes.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double)]
         lib.nnp_create_from_file.restype = C.c_int
         lib.nnp_create_from_file.argtypes = [C.POINTER(C.c_void_p), C.c_char_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p,
                                              C.c_int32, C.c_double, C.c_int32]
@@ -310,6 +312,17 @@ class NNP:
             fl, tile = C.c_double(), C.c_int32()
             _check(self.lib.nnp_get_stage_work(self.h, k, C.byref(fl), C.byref(tile)), "nnp_get_stage_work")
             out[self.lib.nnp_stage_name(self.h, k).decode()] = (fl.value, tile.value)
+        return out
+
+    def stage_bytes(self):
+        """{stage name: algorithmic bytes of a tensor-engine launch (operands, outputs, epilogue reads, each once)}."""
+        n = C.c_int32()
+        _check(self.lib.nnp_get_stage_times(self.h, None, 0, C.byref(n)), "nnp_get_stage_times")
+        out = {}
+        for k in range(n.value):
+            b = C.c_double()
+            _check(self.lib.nnp_get_stage_bytes(self.h, k, C.byref(b)), "nnp_get_stage_bytes")
+            out[self.lib.nnp_stage_name(self.h, k).decode()] = b.value
         return out
 
     def work(self):

@@ -342,6 +342,7 @@ struct UmmaPlan {
   int np_max = 16;
   long long makespan = 0;
   double flops = 0;
+  double bytes = 0;  // algorithmic: every operand / output plane of a problem once
 };
 
 static void plan_items(UmmaPlan& pl, const std::vector<UmmaProblem>& probs, const std::vector<UmmaOperand>& bops, int cap,
@@ -359,6 +360,17 @@ static void plan_items(UmmaPlan& pl, const std::vector<UmmaProblem>& probs, cons
     unsigned long long kmask = nkb_all <= 64 ? p.kmask : 0ull;
     if (nkb_all < 64) kmask &= (1ull << nkb_all) - 1ull;
     const int nkb = kmask ? __builtin_popcountll(kmask) : nkb_all;
+    {
+      // algorithmic bytes of the problem: both operands (hi and lo planes, the contraction boxes that are run, clipped
+      // to K), the output planes and what the epilogue reads, each once; dead feature tiles excluded
+      int f_live = 0;
+      for (int f0 = 0; f0 < p.F; f0 += 128)
+        if (!(p.fmask && f0 / 128 < 64 && !((p.fmask >> (f0 / 128)) & 1ull))) f_live += std::min(128, p.F - f0);
+      const double k_live = std::min<double>(p.K, 32.0 * nkb);
+      const double out_planes = (p.C_lo ? 2.0 : 1.0) + (p.C_full ? 1.0 : 0.0);
+      const double aux_planes = p.aux ? (p.aux_lo ? 2.0 : 1.0) : 0.0;
+      pl.bytes += 4.0 * (2.0 * k_live * ((double)f_live + p.n_atoms) + (out_planes + aux_planes) * (double)p.n_atoms * f_live);
+    }
     for (int f0 = 0; f0 < p.F; f0 += 128) {
       if (p.fmask && f0 / 128 < 64 && !((p.fmask >> (f0 / 128)) & 1ull)) continue;
       for (int a0 = 0; a0 < p.n_atoms; a0 += nt) {
@@ -455,6 +467,7 @@ int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, cons
   L.grid = n ? (int)G : 0;
   L.tile = np_max;
   L.issued_flops = best.flops;
+  L.algo_bytes = best.bytes;
   P->b_box_bytes = np_max * 128;
   P->stage_bytes = 2 * A_BOX_BYTES + 2 * P->b_box_bytes;
   const size_t bar_bytes = (2 * U_MAX_STAGES + 2 * U_MAX_SLOTS) * 8 + 16;

@@ -838,6 +838,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   h->stage_names.push_back("finish");
   h->stage_issued.assign(h->stage_names.size(), 0.0);
   h->stage_tile.assign(h->stage_names.size(), 0);
+  h->stage_bytes.assign(h->stage_names.size(), 0.0);
   if (h->use_umma)
     for (size_t k = 0; k < h->stage_names.size(); ++k)
       for (auto* v : {&h->ufwd, &h->ubwd})
@@ -845,6 +846,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
           if (g.name == h->stage_names[k]) {
             h->stage_issued[k] = g.issued_flops;
             h->stage_tile[k] = g.tile;
+            h->stage_bytes[k] = g.algo_bytes;
           }
   h->n_launches = N > 0 ? (int)h->stage_names.size() + (h->use_cells ? 4 : 0) : 0;  // cell path: 5 kernels in "nbr"
   h->events.resize(h->stage_names.size() + 1);
@@ -1038,6 +1040,12 @@ extern "C" int nnp_get_stage_work(nnp_handle* h, int32_t stage, double* issued_f
   if (!h || stage < 0 || stage >= (int)h->stage_names.size()) return NNP_ERR_INVALID_ARG;
   if (issued_flops_host) *issued_flops_host = h->stage_issued[stage];
   if (atom_tile_host) *atom_tile_host = h->stage_tile[stage];
+  return NNP_OK;
+}
+
+extern "C" int nnp_get_stage_bytes(nnp_handle* h, int32_t stage, double* bytes_host) {
+  if (!h || !bytes_host || stage < 0 || stage >= (int)h->stage_names.size()) return NNP_ERR_INVALID_ARG;
+  *bytes_host = h->stage_bytes[stage];
   return NNP_OK;
 }
 

@@ -146,7 +146,8 @@ struct UmmaLaunch {
   int* d_cta_off = nullptr;
   int n_items = 0, grid = 0, tile = 0;
   size_t smem_bytes = 0;
-  double issued_flops = 0;  // 2 x MACs of the boxes actually run (padding and structural zeros excluded/included as issued)
+  double issued_flops = 0;
+  double algo_bytes = 0;   // operand planes read once + output planes written once + epilogue reads  // 2 x MACs of the boxes actually run (padding and structural zeros excluded/included as issued)
   std::string name;
 };
 int umma_init();
@@ -328,7 +329,7 @@ struct nnp_handle {
   bool profiling = false;
   std::vector<cudaEvent_t> events;
   std::vector<std::string> stage_names;
-  std::vector<double> stage_issued;  // tensor-engine stages: 2 x MACs actually issued (structural zeros skipped)
+  std::vector<double> stage_issued, stage_bytes;  // tensor-engine stages: 2 x MACs actually issued (structural zeros skipped)
   std::vector<int> stage_tile;       // tensor-engine stages: atom-tile width chosen for the launch
   int n_launches = 0;
   double work[4] = {0, 0, 0, 0};
