@@ -490,6 +490,10 @@ int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, cons
 
 void umma_launch(const UmmaLaunch& L, cudaStream_t s, bool pdl) {
   if (L.n_items == 0) return;
+  if (L.pair) {
+    umma2_launch(L, s, pdl);
+    return;
+  }
   launch_kernel(pdl, gemm_umma_kernel, dim3(L.grid), dim3(U_THREADS), L.smem_bytes, s,
                 *reinterpret_cast<const UmmaParams*>(L.params));
 }
@@ -503,6 +507,7 @@ int umma_init() {
 void umma_free_launch(UmmaLaunch& L) {
   if (L.d_items) cudaFree(L.d_items);
   if (L.d_cta_off) cudaFree(L.d_cta_off);
-  delete reinterpret_cast<UmmaParams*>(L.params);
+  if (L.pair) umma2_free_params(L);
+  else delete reinterpret_cast<UmmaParams*>(L.params);
   L.d_items = nullptr; L.d_cta_off = nullptr; L.params = nullptr;
 }

@@ -593,7 +593,10 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
         UmmaLaunch ul;
         ul.name = (pass == 0 ? "mlp_fwd_l" : "mlp_bwd_l") + std::to_string(l);
         const bool reverse = !(cfg->flags & NNP_FLAG_NO_SWEEP_REVERSAL) && ((pass * (L - 1) + li) & 1) == 0;
-        if (umma_build_launch(ul, probs, aops, bops, prop.multiProcessorCount, reverse)) {
+        // opt-in: the two layer-1 launches of large systems on CTA pairs (cta_group::2, 256 x 256 tiles)
+        const bool pair = l == 1 && (cfg->flags & NNP_FLAG_UMMA_PAIRS) && umma2_suits(probs) && umma2_init() == 0;
+        if (pair ? umma2_build_launch(ul, probs, aops, bops, prop.multiProcessorCount)
+                 : umma_build_launch(ul, probs, aops, bops, prop.multiProcessorCount, reverse)) {
           umma_free_launch(ul);
           return fail(NNP_ERR_CUDA);
         }

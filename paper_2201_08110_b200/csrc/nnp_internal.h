@@ -146,6 +146,7 @@ struct UmmaLaunch {
   int* d_cta_off = nullptr;
   int n_items = 0, grid = 0, tile = 0;
   size_t smem_bytes = 0;
+  bool pair = false;       // built by the CTA-pair engine (mlp_umma2.cu)
   double issued_flops = 0;
   double algo_bytes = 0;   // operand planes read once + output planes written once + epilogue reads  // 2 x MACs of the boxes actually run (padding and structural zeros excluded/included as issued)
   std::string name;
@@ -155,6 +156,13 @@ int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, cons
                       const std::vector<UmmaOperand>& bops, int num_sms, bool reverse = false);
 void umma_launch(const UmmaLaunch& L, cudaStream_t s, bool pdl);
 void umma_free_launch(UmmaLaunch& L);
+// CTA-pair variant (cta_group::2, 256 x 256 tiles): opt-in (NNP_FLAG_UMMA_PAIRS), measured slower
+int umma2_init();
+bool umma2_suits(const std::vector<UmmaProblem>& probs);
+int umma2_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, const std::vector<UmmaOperand>& aops,
+                       const std::vector<UmmaOperand>& bops, int num_sms);
+void umma2_launch(const UmmaLaunch& L, cudaStream_t s, bool pdl);
+void umma2_free_params(UmmaLaunch& L);
 
 // ---- ligand-size engine (mlp_small.cu): weight-streaming FFMA kernels, one CTA per item
 struct SmallFwdItem {       // out[a*ldc + r] = CELU(bias[r] + sum_k W[r*K + k] X[a*ldx + k]),  r < n_rows, a < n_atoms

@@ -16,7 +16,7 @@ from oracle.ani_oracle import AniOracle  # noqa: E402
 from paper_2201_08110_b200 import workloads as wl  # noqa: E402
 from paper_2201_08110_b200.binding import (NNP, NNP_FLAG_FORCE_CELLS, NNP_FLAG_NO_CELLS, NNP_FLAG_NO_GRAPH,  # noqa: E402
                                             NNP_FLAG_NO_FWD1, NNP_FLAG_NO_MID, NNP_FLAG_NO_NBR_FUSION, NNP_FLAG_NO_PDL, NNP_FLAG_NO_SMALL,
-                                            NNP_FLAG_NO_UMMA, NNP_FLAG_NO_ZERO_SKIP, NNP_FLAG_NO_SWEEP_REVERSAL,
+                                            NNP_FLAG_NO_UMMA, NNP_FLAG_NO_ZERO_SKIP, NNP_FLAG_NO_SWEEP_REVERSAL, NNP_FLAG_UMMA_PAIRS,
                                             NNPError)
 
 # MLP engines: ligand-size weight-streaming FFMA (default at these sizes; with the fused middle launch or
@@ -327,6 +327,21 @@ def test_sweep_direction_of_tensor_launches_changes_nothing():
     b = NNP(w.params, W, B, w.species, flags=NNP_FLAG_NO_SWEEP_REVERSAL)
     ra, rb = gpu_eval(a, w.positions), gpu_eval(b, w.positions)
     assert np.array_equal(ra["E"], rb["E"]) and np.array_equal(ra["F"], rb["F"])
+    a.destroy(); b.destroy()
+
+
+def test_cta_pair_engine_matches_the_one_cta_engine():
+    """Opt-in cta_group::2 engine for the layer-1 launches (256 x 256 tiles on CTA pairs): same operands, slots and
+    compensation as the default engine, so energies and forces agree to FP32 summation order -- and with the oracle
+    through the default engine's parity tests."""
+    w = wl.config5()
+    W, B = w.weights()
+    a = NNP(w.params, W, B, w.species)
+    b = NNP(w.params, W, B, w.species, flags=NNP_FLAG_UMMA_PAIRS)
+    ra, rb = gpu_eval(a, w.positions), gpu_eval(b, w.positions)
+    assert abs(ra["E"][0] - rb["E"][0]) / w.n_atoms <= 1e-6
+    assert np.abs(ra["F"] - rb["F"]).max() <= 1e-4
+    assert np.abs(rb["F"]).max() > 1.0
     a.destroy(); b.destroy()
 
 
