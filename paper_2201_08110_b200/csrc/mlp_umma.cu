@@ -57,9 +57,6 @@ struct UmmaParams {
   int n_slots;         // TMEM slot ring depth: 4 or 8
   int slot_shift;      // log2(n_slots)
   int comp;            // 1: add the expected truncation loss of a slot (one ulp away from zero, see tmem_add) back
-  // chained launch: tensor maps of every layer in device memory, [(layer * 4 + kind) * NNP_MAX_SPECIES + slot] with
-  // kind 0..3 = weights hi, weights lo, activations hi, activations lo; null: the arrays above
-  const CUtensorMap* gmaps;
 };
 
 __device__ __forceinline__ void drain_sync() { asm volatile("bar.sync 1, %0;" ::"n"(U_DRAIN_THREADS) : "memory"); }
@@ -137,11 +134,6 @@ __device__ __forceinline__ void drain_item(const UmmaItem& t, const UmmaParams& 
     if (na > 0) epilogue_rows<U_DRAIN_THREADS>(t, staging, h * CT, na, dt);
     drain_sync();
   }
-  if (t.sig) {  // chained launch: the output of this item is in memory -- tell its consumers
-    __threadfence();
-    drain_sync();
-    if (dt == 0) atomicAdd(t.sig, 1u);
-  }
 }
 
 __global__ void __launch_bounds__(U_THREADS, 1) gemm_umma_kernel(const __grid_constant__ UmmaParams P) {
@@ -191,28 +183,6 @@ __global__ void __launch_bounds__(U_THREADS, 1) gemm_umma_kernel(const __grid_co
       const CUtensorMap* al = &P.alo[amap];
       const CUtensorMap* bh = &P.bhi[bmap];
       const CUtensorMap* bl = &P.blo[bmap];
-      if (P.gmaps) {
-        const CUtensorMap* base = P.gmaps + (size_t)__shfl_sync(0xffffffffu, t.layer, 0) * 4 * NNP_MAX_SPECIES;
-        ah = base + amap;
-        al = base + NNP_MAX_SPECIES + amap;
-        bh = base + 2 * NNP_MAX_SPECIES + bmap;
-        bl = base + 3 * NNP_MAX_SPECIES + bmap;
-        // chained launch: the activation boxes of this item are the output of earlier items of this launch (other
-        // CTAs).  Wait until all of them have signalled (acquire), then order the TMA reads (async proxy) after it.
-        // The static schedule puts a consumer a whole step behind its producers, so this wait is normally over at once.
-        if (leader && t.dep) {
-          const unsigned int* dep = t.dep;
-          const unsigned int need = (unsigned int)t.dep_need;
-          unsigned int have;
-          for (;;) {
-            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(have) : "l"(dep) : "memory");
-            if (have >= need) break;
-            __nanosleep(200);
-          }
-          asm volatile("fence.proxy.async;" ::: "memory");
-        }
-        __syncwarp();
-      }
       const int a_c0 = __shfl_sync(0xffffffffu, t.a_c0, 0), a_c1 = __shfl_sync(0xffffffffu, t.a_c1, 0),
                 b_c0 = __shfl_sync(0xffffffffu, t.b_c0, 0), b_c1 = __shfl_sync(0xffffffffu, t.b_c1, 0),
                 nkb = __shfl_sync(0xffffffffu, t.nkb, 0);
@@ -369,7 +339,6 @@ struct UmmaPlan {
   std::vector<UmmaItem> items;
   std::vector<long long> cost;
   std::vector<int> tile_of_bmap;
-  std::vector<int> atile;  // per item: index of its atom tile within the element group
   int np_max = 16;
   long long makespan = 0;
   double flops = 0;
@@ -427,7 +396,6 @@ static void plan_items(UmmaPlan& pl, const std::vector<UmmaProblem>& probs, cons
         t.w_last = p.w_last ? p.w_last + f0 : nullptr;
         t.scale = p.scale; t.alpha = p.alpha; t.inv_alpha = p.inv_alpha;
         pl.items.push_back(t);
-        pl.atile.push_back(a0 / nt);
         pl.cost.push_back((long long)nkb * box_cycles(nt) + 1500);
         pl.flops += 2.0 * t.f_valid * t.n_valid * 32.0 * nkb;
       }
@@ -520,138 +488,6 @@ int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, cons
   return 0;
 }
 
-// ------------------------------------------------------------------------------------------------
-// Chained launch: the tensor launches of a step (forward layers 1..L-1, backward layers L-1..1, in that order) as ONE
-// persistent launch.  Layer d reads what layer d-1 wrote, per atom tile: an item of layer d for atom tile g may
-// start when all items of layer d-1 for tile g have signalled (one counter per (layer, tile)).  The static
-// schedule is a skewed wavefront over chunks of atom tiles -- step t runs layer d on chunk t-d -- so a consumer is
-// scheduled a whole step (all layers of one chunk, a few rounds of the machine) after its producers: the wait is
-// normally already satisfied, and what the producer wrote (a chunk's planes, tens of MB) is still in L2 when the
-// consumer's TMA loads ask for it, instead of making a round trip through HBM as between separate launches.
-// Deadlock-free: every CTA runs its items in schedule order, dependencies point backwards in that order, and all CTAs
-// of the grid are resident (one per SM).
-// ------------------------------------------------------------------------------------------------
-int umma_build_chain(UmmaLaunch& L, const std::vector<std::vector<UmmaProblem>>& probs,
-                     const std::vector<std::vector<UmmaOperand>>& aops, const std::vector<std::vector<UmmaOperand>>& bops,
-                     int num_sms) {
-  UmmaParams* P = new UmmaParams();
-  memset(P, 0, sizeof(*P));
-  L.params = P;
-  const int nl = (int)probs.size();
-  if (nl < 2 || (int)aops.size() != nl || (int)bops.size() != nl) return -1;
-  // tensor maps of every layer
-  std::vector<CUtensorMap> hm((size_t)nl * 4 * NNP_MAX_SPECIES);
-  memset(hm.data(), 0, hm.size() * sizeof(CUtensorMap));
-  for (int l = 0; l < nl; ++l) {
-    if (aops[l].size() > NNP_MAX_SPECIES || bops[l].size() > NNP_MAX_SPECIES) return -1;
-    for (size_t i = 0; i < aops[l].size(); ++i) {
-      const UmmaOperand& o = aops[l][i];
-      if (encode_map(&hm[((size_t)l * 4 + 0) * NNP_MAX_SPECIES + i], o.hi, o.rows, o.cols, o.ld, 128)) return -1;
-      if (encode_map(&hm[((size_t)l * 4 + 1) * NNP_MAX_SPECIES + i], o.lo, o.rows, o.cols, o.ld, 128)) return -1;
-    }
-    for (size_t i = 0; i < bops[l].size(); ++i) {
-      const UmmaOperand& o = bops[l][i];
-      if (encode_map(&hm[((size_t)l * 4 + 2) * NNP_MAX_SPECIES + i], o.hi, o.rows, o.cols, o.ld, 128)) return -1;
-      if (encode_map(&hm[((size_t)l * 4 + 3) * NNP_MAX_SPECIES + i], o.lo, o.rows, o.cols, o.ld, 128)) return -1;
-    }
-  }
-  if (cudaMalloc(&L.d_maps, hm.size() * sizeof(CUtensorMap)) != cudaSuccess) return -1;
-  cudaMemcpy(L.d_maps, hm.data(), hm.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice);
-  P->gmaps = reinterpret_cast<const CUtensorMap*>(L.d_maps);
-  // global atom-tile index: the element groups (activation map slots) one after the other, 128 atoms per tile
-  const size_t ns = bops[0].size();
-  std::vector<int> tile_base(ns + 1, 0);
-  for (size_t i = 0; i < ns; ++i) tile_base[i + 1] = tile_base[i] + (int)((bops[0][i].rows + 127) / 128);
-  const int T = tile_base[ns];
-  if (T == 0) return -1;
-  L.counter_bytes = (size_t)nl * T * sizeof(unsigned int);
-  if (cudaMalloc((void**)&L.d_counters, L.counter_bytes) != cudaSuccess) return -1;
-  cudaMemset(L.d_counters, 0, L.counter_bytes);
-  // items of every layer (128-atom tiles) and how many of them there are per (layer, tile)
-  std::vector<UmmaPlan> plans(nl);
-  std::vector<std::vector<int>> gtile(nl), count(nl, std::vector<int>(T, 0));
-  double flops = 0, bytes = 0;
-  size_t n = 0;
-  for (int l = 0; l < nl; ++l) {
-    plan_items(plans[l], probs[l], bops[l], 128, num_sms);
-    if (plans[l].np_max != 128) return -1;  // chained launches are for systems whose element groups fill 128-atom tiles
-    gtile[l].resize(plans[l].items.size());
-    for (size_t i = 0; i < plans[l].items.size(); ++i) {
-      UmmaItem& t = plans[l].items[i];
-      if (t.n_pad != 128 || t.bmap < 0 || (size_t)t.bmap >= ns) return -1;
-      const int g = tile_base[t.bmap] + plans[l].atile[i];
-      if (g >= tile_base[t.bmap + 1]) return -1;
-      gtile[l][i] = g;
-      ++count[l][g];
-    }
-    flops += plans[l].flops;
-    bytes += plans[l].bytes;
-    n += plans[l].items.size();
-  }
-  for (int l = 0; l < nl; ++l)
-    for (size_t i = 0; i < plans[l].items.size(); ++i) {
-      UmmaItem& t = plans[l].items[i];
-      const int g = gtile[l][i];
-      t.layer = l;
-      t.sig = L.d_counters + (size_t)l * T + g;
-      t.dep = l > 0 ? L.d_counters + (size_t)(l - 1) * T + g : nullptr;
-      t.dep_need = l > 0 ? count[l - 1][g] : 0;
-      if (l > 0 && t.dep_need == 0) return -1;  // a consumer without producers: not a chain
-    }
-  // skewed wavefront: chunks of `tc` atom tiles such that one layer of a chunk is about one round of the machine
-  const double per_tile = (double)n / ((double)nl * T);
-  const int tc = std::max(1, (int)(num_sms / std::max(1.0, per_tile) + 0.5));
-  const int n_chunks = (T + tc - 1) / tc;
-  std::vector<std::vector<std::vector<size_t>>> by_chunk(nl, std::vector<std::vector<size_t>>(n_chunks));
-  for (int l = 0; l < nl; ++l)
-    for (size_t i = 0; i < plans[l].items.size(); ++i) by_chunk[l][gtile[l][i] / tc].push_back(i);
-  std::vector<UmmaItem> order;
-  order.reserve(n);
-  for (int step = 0; step < n_chunks + nl - 1; ++step)
-    for (int l = 0; l < nl; ++l) {
-      const int c = step - l;
-      if (c < 0 || c >= n_chunks) continue;
-      for (size_t i : by_chunk[l][c]) order.push_back(plans[l].items[i]);
-    }
-  if (order.size() != n) return -1;
-  // dealt to the persistent CTAs in snake order; each CTA keeps schedule order
-  const size_t G = std::max<size_t>(1, std::min<size_t>(n, (size_t)num_sms));
-  std::vector<std::vector<UmmaItem>> per_cta(G);
-  for (size_t i = 0; i < n; ++i) {
-    const size_t round = i / G, posn = i % G;
-    per_cta[(round & 1) ? G - 1 - posn : posn].push_back(order[i]);
-  }
-  std::vector<UmmaItem> flat;
-  std::vector<int> off(G + 1, 0);
-  for (size_t c = 0; c < G; ++c) {
-    for (auto& t : per_cta[c]) flat.push_back(t);
-    off[c + 1] = (int)flat.size();
-  }
-  L.n_items = (int)n;
-  L.grid = (int)G;
-  L.tile = 128;
-  L.issued_flops = flops;
-  L.algo_bytes = bytes;
-  P->b_box_bytes = 128 * 128;
-  P->stage_bytes = 2 * A_BOX_BYTES + 2 * P->b_box_bytes;
-  const size_t bar_bytes = (2 * U_MAX_STAGES + 2 * U_MAX_SLOTS) * 8 + 16;
-  P->staging_rows = 64;
-  const size_t staging_bytes = (size_t)P->staging_rows * 512;
-  P->n_stages = (int)std::min<size_t>(U_MAX_STAGES, (UMMA_SMEM_BUDGET - 1024 - bar_bytes - staging_bytes) / P->stage_bytes);
-  L.smem_bytes = (size_t)P->n_stages * P->stage_bytes + staging_bytes + bar_bytes + 1024;
-  P->slot_cols = 128;
-  P->n_slots = 4;
-  P->slot_shift = 2;
-  P->comp = 1;
-  if (cudaMalloc((void**)&L.d_items, n * sizeof(UmmaItem)) != cudaSuccess) return -1;
-  if (cudaMalloc((void**)&L.d_cta_off, (G + 1) * sizeof(int)) != cudaSuccess) return -1;
-  cudaMemcpy(L.d_items, flat.data(), n * sizeof(UmmaItem), cudaMemcpyHostToDevice);
-  cudaMemcpy(L.d_cta_off, off.data(), (G + 1) * sizeof(int), cudaMemcpyHostToDevice);
-  P->items = L.d_items;
-  P->cta_off = L.d_cta_off;
-  return 0;
-}
-
 void umma_launch(const UmmaLaunch& L, cudaStream_t s, bool pdl) {
   if (L.n_items == 0) return;
   if (L.pair) {
@@ -673,9 +509,5 @@ void umma_free_launch(UmmaLaunch& L) {
   if (L.d_cta_off) cudaFree(L.d_cta_off);
   if (L.pair) umma2_free_params(L);
   else delete reinterpret_cast<UmmaParams*>(L.params);
-  if (L.d_maps) cudaFree(L.d_maps);
-  if (L.d_counters) cudaFree(L.d_counters);
-  L.d_maps = nullptr;
-  L.d_counters = nullptr;
   L.d_items = nullptr; L.d_cta_off = nullptr; L.params = nullptr;
 }

@@ -86,7 +86,6 @@ extern "C" void nnp_destroy(nnp_handle* h) {
     }
   for (auto* v : {&h->ufwd, &h->ubwd})
     for (auto& g : *v) umma_free_launch(g);
-  if (h->uchain.params) umma_free_launch(h->uchain);
   for (auto* v : {&h->sfwd, &h->sbwd})
     for (auto& g : *v) small_free_launch(g);
   small_free_launch(h->smid);
@@ -508,9 +507,6 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     int ns = 0;
     for (int e = 0; e < S; ++e)
       if (h->grp_off[e + 1] > h->grp_off[e]) slot[e] = ns++;
-    std::vector<std::vector<UmmaProblem>> chain_probs;
-    std::vector<std::vector<UmmaOperand>> chain_aops, chain_bops;
-    bool chain_ok = h->fuse_delta && h->n_parts == 1 && L - 1 >= 2 && !(cfg->flags & (NNP_FLAG_NO_CHAIN | NNP_FLAG_UMMA_PAIRS));
     for (int pass = 0; pass < 2; ++pass) {
       for (int li = 0; li < L - 1; ++li) {
         const int l = pass == 0 ? li + 1 : L - 1 - li;  // fwd: 1..L-1, bwd: L-1..1
@@ -605,31 +601,6 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
           return fail(NNP_ERR_CUDA);
         }
         (pass == 0 ? h->ufwd : h->ubwd).push_back(ul);
-        chain_ok = chain_ok && ul.tile == 128;
-        if (l > 1) {  // the hidden layers: forward 2..L-1, backward L-1..2
-          chain_probs.push_back(probs);
-          chain_aops.push_back(aops);
-          chain_bops.push_back(bops);
-        }
-      }
-    }
-    // Large systems (every launch on 128-atom tiles): the hidden-layer launches of the step (forward 2..L-1, backward
-    // L-1..2) as ONE chained launch, so that the planes a layer writes are read by the next layer out of L2 (DESIGN.md
-    // section 6).  The layer-1 launches stay separate: their weights (all models of all elements, two planes, two
-    // transposes: ~40 MB each) would be re-streamed through L2 by every step of the chain's schedule and evict the
-    // activations the chain is there to keep (all six layers chained: 731 -> 855 us at configs[2], measured).  The
-    // one-layer launches stay built: they are the A/B path (NNP_FLAG_NO_CHAIN).
-    for (int e = 0; e < S && chain_ok; ++e) {
-      const int ne = h->grp_off[e + 1] - h->grp_off[e];
-      if (ne > 0 && ne < 512) chain_ok = false;
-    }
-    if (chain_ok) {
-      h->uchain.name = "mlp_chain";
-      if (umma_build_chain(h->uchain, chain_probs, chain_aops, chain_bops, prop.multiProcessorCount) == 0) {
-        h->use_chain = true;
-      } else {
-        umma_free_launch(h->uchain);
-        h->uchain = UmmaLaunch();
       }
     }
   }
@@ -861,11 +832,6 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     for (auto& g : h->sfwd) h->stage_names.push_back(g.name);
     if (h->use_mid) h->stage_names.push_back(h->smid.name);
     for (auto& g : h->sbwd) h->stage_names.push_back(g.name);
-  } else if (h->use_chain) {
-    h->stage_names.push_back(h->ufwd.front().name);
-    h->stage_names.push_back(h->uchain.name);
-    h->stage_names.push_back("mlp_last");
-    h->stage_names.push_back(h->ubwd.back().name);
   } else {
     for (auto& g : h->fwd) h->stage_names.push_back(g.name);
     h->stage_names.push_back("mlp_last");
@@ -876,13 +842,6 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   h->stage_issued.assign(h->stage_names.size(), 0.0);
   h->stage_tile.assign(h->stage_names.size(), 0);
   h->stage_bytes.assign(h->stage_names.size(), 0.0);
-  if (h->use_chain)
-    for (size_t k = 0; k < h->stage_names.size(); ++k)
-      if (h->stage_names[k] == h->uchain.name) {
-        h->stage_issued[k] = h->uchain.issued_flops;
-        h->stage_tile[k] = h->uchain.tile;
-        h->stage_bytes[k] = h->uchain.algo_bytes;
-      }
   if (h->use_umma)
     for (size_t k = 0; k < h->stage_names.size(); ++k)
       for (auto* v : {&h->ufwd, &h->ubwd})
@@ -912,22 +871,12 @@ static void enqueue_chain(nnp_handle* h, const float* d_pos, int ps, const int* 
   h->pdl_now = h->use_pdl && !ev;  // event records between the kernels would break the programmatic edges
   const bool pdl = h->pdl_now;
   mark();
-  if (h->use_chain) cudaMemsetAsync(h->uchain.d_counters, 0, h->uchain.counter_bytes, s);  // ready counters of the chain
   if (!h->fuse_nbr) { launch_neighbors(h, d_pos, ps, d_idx, s); mark(); }
   launch_aev_forward(h, d_pos, ps, d_idx, s); mark();
   if (h->use_small) {  // per-atom energies and delta_L-1 come out of the first backward launch
     for (auto& g : h->sfwd) { small_launch_fwd(g, s, pdl); mark(); }
     if (h->use_mid) { mid_launch(h->smid, s, pdl); mark(); }
     for (auto& g : h->sbwd) { small_launch_bwd(g, s, pdl); mark(); }
-    launch_aev_backward(h, s); mark();
-    launch_finish(h, d_idx, d_energy, d_force, fs, fixed, s); mark();
-    return;
-  }
-  if (h->use_chain) {  // forward and backward tensor launches in one; the 1-output layer only reads (energies)
-    umma_launch(h->ufwd.front(), s, pdl); mark();
-    umma_launch(h->uchain, s, pdl); mark();
-    launch_last_layer(h, s); mark();
-    umma_launch(h->ubwd.back(), s, false); mark();  // plain launch: the 1-output layer before it is one
     launch_aev_backward(h, s); mark();
     launch_finish(h, d_idx, d_energy, d_force, fs, fixed, s); mark();
     return;

@@ -123,12 +123,6 @@ struct UmmaItem {            // one tile of one GEMM, as the persistent CTAs con
   float* C_full;
   const float* w_last;       // [f] weights of the 1-output layer for this tile's features
   float scale, alpha, inv_alpha;
-  // chained launch (all layers in one persistent launch, umma_build_chain): the item may start loading its
-  // activation boxes when *dep >= dep_need (its producers' outputs are in memory) and adds 1 to *sig when its own
-  // output is; `layer` selects the tensor maps.  All null / 0 in a one-layer launch.
-  const unsigned int* dep;
-  unsigned int* sig;
-  int dep_need, layer;
 };
 struct UmmaProblem {
   unsigned long long kmask;    // non-zero: contraction boxes (32 wide) to run; the others multiply structural zeros
@@ -154,20 +148,12 @@ struct UmmaLaunch {
   size_t smem_bytes = 0;
   bool pair = false;       // built by the CTA-pair engine (mlp_umma2.cu)
   double issued_flops = 0;
-  double algo_bytes = 0;   // operand planes read once + output planes written once + epilogue reads
-  // chained launch: tensor maps of all layers and the ready counters (zeroed before every launch) in device memory
-  void* d_maps = nullptr;
-  unsigned int* d_counters = nullptr;
-  size_t counter_bytes = 0;
+  double algo_bytes = 0;   // operand planes read once + output planes written once + epilogue reads  // 2 x MACs of the boxes actually run (padding and structural zeros excluded/included as issued)
   std::string name;
 };
 int umma_init();
 int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, const std::vector<UmmaOperand>& aops,
                       const std::vector<UmmaOperand>& bops, int num_sms, bool reverse = false);
-// all layers of the forward and backward pass (in execution order) as ONE persistent launch with ready counters
-int umma_build_chain(UmmaLaunch& L, const std::vector<std::vector<UmmaProblem>>& probs,
-                     const std::vector<std::vector<UmmaOperand>>& aops, const std::vector<std::vector<UmmaOperand>>& bops,
-                     int num_sms);
 void umma_launch(const UmmaLaunch& L, cudaStream_t s, bool pdl);
 void umma_free_launch(UmmaLaunch& L);
 // CTA-pair variant (cta_group::2, 256 x 256 tiles): opt-in (NNP_FLAG_UMMA_PAIRS), measured slower
@@ -319,8 +305,6 @@ struct nnp_handle {
   // MLP launches
   std::vector<GemmLaunch> fwd, bwd;  // fwd: layers 1..L-1; bwd: layers L-1..1
   std::vector<UmmaLaunch> ufwd, ubwd; // the same launches on the tcgen05 engine (used when use_umma)
-  UmmaLaunch uchain;                  // ... or all of them as one chained launch (use_chain)
-  bool use_chain = false;
   std::vector<SmallLaunch> sfwd, sbwd; // ligand-size engine (used when use_small); no separate last-layer launch
   SmallLaunch smid;                    // fused middle launch of the ligand-size engine (used when use_mid)
   bool use_umma = false, use_small = false, use_mid = false;
