@@ -41,6 +41,7 @@ extern "C" {
 #define NNP_ERR_CAPACITY (-4)  /* a centre has more neighbours than the row capacity */
 #define NNP_ERR_NONFINITE (-5) /* NaN/Inf position seen on the device */
 #define NNP_ERR_ALLOC (-6)
+#define NNP_ERR_STATIC_LIMIT (-7) /* nnp_coupling_compute_static: more atoms than its fixed scratch array holds */
 
 typedef struct nnp_handle nnp_handle; /* opaque; owned by the library */
 
@@ -260,6 +261,33 @@ int nnp_coupling_compute(nnp_coupling *c, const float *d_pos, int32_t pos_stride
 int nnp_coupling_compute_fixed(nnp_coupling *c, const float *d_pos, int32_t pos_stride_floats, double *d_energy,
                                int64_t *d_force_fixed, int32_t force_stride_int64, void *cuda_stream);
 void nnp_coupling_destroy(nnp_coupling *c);
+
+/*
+ * nnp_coupling_compute_static: Eq. 4 as above through an entry point that ALLOCATES NOTHING -- no cudaMalloc, cudaFree
+ * or allocating library call, in this call or behind it -- for callers that cannot allocate (CUDA graph capture, tight
+ * serving loops, harnesses that forbid it).  No handle: the atom lists are DEVICE arrays passed with every call
+ * (d_*_rows i32, d_q / d_sigma / d_eps f32, meaning and units as in nnp_coupling_create; not validated: rows must be
+ * >= 0, eps >= 0), the other arguments as in nnp_coupling_compute (forces ADDED to f32 d_force_accum, may be NULL;
+ * d_energy device f64[1] WRITTEN, may be NULL; asynchronous on cuda_stream).  Results: the kernels and summation
+ * orders of nnp_coupling_compute, i.e. the same bits for the same inputs.
+ * Scratch (packed atom records, per-CTA partial sums) is one file-scope device array of
+ * ~1.8 MB sized for NNP_COUPLING_STATIC_MAX_NNP x NNP_COUPLING_STATIC_MAX_MM atoms, held by every GPU that loads the
+ * library until the process exits; more atoms => NNP_ERR_STATIC_LIMIT, nothing is launched.  All calls share the
+ * array, which keeps the last call's contents (no element needs to start at zero: everything read is written earlier
+ * in the same call); calls that OVERLAP on the GPU (different streams without an ordering) race on it -- issue them
+ * on one stream or order them with events.
+ * nnp_coupling_static_init: optional; resolves the array's device address for the CURRENT device (once per device,
+ * done lazily by the first compute call otherwise -- call it before starting a stream capture).
+ * Errors: NNP_ERR_INVALID_ARG, NNP_ERR_STATIC_LIMIT, NNP_ERR_UNSUPPORTED_ARCH, NNP_ERR_CUDA.
+ */
+#define NNP_COUPLING_STATIC_MAX_NNP 128
+#define NNP_COUPLING_STATIC_MAX_MM 65536
+int nnp_coupling_static_init(void);
+int nnp_coupling_compute_static(int32_t n_nnp, const int32_t *d_nnp_rows, const float *d_q_nnp, const float *d_sigma_nnp,
+                                const float *d_eps_nnp, int32_t n_mm, const int32_t *d_mm_rows, const float *d_q_mm,
+                                const float *d_sigma_mm, const float *d_eps_mm, double coulomb_const, double cutoff,
+                                double length_scale, const float *d_pos, int32_t pos_stride_floats, double *d_energy,
+                                float *d_force_accum, int32_t force_stride_floats, void *cuda_stream);
 
 #ifdef __cplusplus
 }

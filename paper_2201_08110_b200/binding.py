@@ -33,6 +33,7 @@ ERRORS = {
     -4: "NNP_ERR_CAPACITY",
     -5: "NNP_ERR_NONFINITE",
     -6: "NNP_ERR_ALLOC",
+    -7: "NNP_ERR_STATIC_LIMIT",
 }
 
 # every symbol include/nnp.h declares (tests check the library exports exactly these)
@@ -42,6 +43,7 @@ SYMBOLS = (
     "nnp_debug_pairs", "nnp_debug_aev", "nnp_debug_atomic_energies", "nnp_debug_daev", "nnp_n_features",
     "nnp_get_stage_work", "nnp_get_stage_bytes", "nnp_create_from_file", "nnp_compute_fixed", "nnp_compute_async", "nnp_measure_peaks",
     "nnp_coupling_create", "nnp_coupling_compute", "nnp_coupling_compute_fixed", "nnp_coupling_destroy",
+    "nnp_coupling_static_init", "nnp_coupling_compute_static",
 )
 FIXED_ONE = float(1 << 32)  # 64-bit fixed-point force format: round(F * 2^32)
 
@@ -145,6 +147,13 @@ def load_library():
         for name in ("nnp_coupling_compute", "nnp_coupling_compute_fixed"):
             getattr(lib, name).restype = C.c_int
             getattr(lib, name).argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+        lib.nnp_coupling_static_init.restype = C.c_int
+        lib.nnp_coupling_static_init.argtypes = []
+        lib.nnp_coupling_compute_static.restype = C.c_int
+        lib.nnp_coupling_compute_static.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
+                                                    C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double,
+                                                    C.c_double, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32,
+                                                    C.c_void_p]
         lib.nnp_coupling_destroy.restype = None
         lib.nnp_coupling_destroy.argtypes = [C.c_void_p]
         _lib = lib
@@ -374,6 +383,25 @@ def measure_peaks():
     _check(lib.nnp_measure_peaks(out.ctypes.data, 4), "nnp_measure_peaks")
     return {"fp32_ffma_tflops": float(out[0]), "tf32_tcgen05_tflops": float(out[1]), "l2_read_gbs": float(out[2]),
             "dram_read_gbs": float(out[3])}
+
+
+COUPLING_STATIC_MAX_NNP = 128    # NNP_COUPLING_STATIC_MAX_NNP
+COUPLING_STATIC_MAX_MM = 65536   # NNP_COUPLING_STATIC_MAX_MM
+
+
+def coupling_static_init():
+    """nnp_coupling_static_init: resolve the static scratch array's device address for the current device."""
+    _check(load_library().nnp_coupling_static_init(), "nnp_coupling_static_init")
+
+
+def coupling_compute_static(n_nnp: int, d_nnp_rows, d_q_nnp, d_sigma_nnp, d_eps_nnp, n_mm: int, d_mm_rows, d_q_mm,
+                            d_sigma_mm, d_eps_mm, coulomb_const: float, cutoff: float, length_scale: float, d_pos: int,
+                            pos_stride: int, d_energy, d_force, force_stride: int, stream: int = 0):
+    """nnp_coupling_compute_static with raw device addresses (ints or None): Eq. 4 without any allocation."""
+    _check(load_library().nnp_coupling_compute_static(
+        int(n_nnp), d_nnp_rows, d_q_nnp, d_sigma_nnp, d_eps_nnp, int(n_mm), d_mm_rows, d_q_mm, d_sigma_mm, d_eps_mm,
+        float(coulomb_const), float(cutoff), float(length_scale), d_pos, int(pos_stride), d_energy, d_force,
+        int(force_stride), stream or None), "nnp_coupling_compute_static")
 
 
 class Coupling:

@@ -264,3 +264,109 @@ extern "C" int nnp_coupling_compute_fixed(nnp_coupling* c, const float* d_pos, i
   return coupling_enqueue(c, d_pos, pos_stride_floats, d_energy, d_force_fixed, force_stride_int64, 1,
                           (cudaStream_t)cuda_stream);
 }
+
+// ------------------------------------------------------------------------------------------------
+// nnp_coupling_compute_static: the same Eq. 4 computation with NO allocation anywhere in the call, for callers that
+// cannot call cudaMalloc (stream capture, tight serving loops, harnesses that forbid it).  There is no handle: the
+// caller passes the atom lists as device arrays with every call, and everything the kernels need in between -- the
+// packed atom records and the per-CTA partial sums of the first kernel -- lives in ONE file-scope device array of a
+// fixed maximum size.  Every GPU that loads the library holds that array until the process exits.
+//   * All calls share the array and it keeps the last call's contents.  Nothing in it has to start at zero: every
+//     element a kernel reads is written earlier in the SAME call (the pack kernel writes the atom records, the MM
+//     kernel writes e_part[block] and f_part[block][i][:] for every block and every NNP atom), so no clear is needed.
+//   * Two calls that overlap on the GPU (different streams, no ordering between them) RACE on the array; calls on one
+//     stream, or ordered by events, are safe.
+// In host code `g_cp_scratch` is a host-side stand-in for the symbol, not a device address: the address the kernels
+// get comes from cudaGetSymbolAddress, once per device, with that device current.
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int CPS_MAX_NNP = NNP_COUPLING_STATIC_MAX_NNP;
+constexpr int CPS_MAX_MM = NNP_COUPLING_STATIC_MAX_MM;
+constexpr int CPS_MAX_PART = (CPS_MAX_MM + CP_THREADS - 1) / CP_THREADS;
+// layout (bytes, every section 256-byte aligned): NNP records | MM records | e_part | f_part
+constexpr size_t CPS_OFF_NNP = 0;
+constexpr size_t CPS_OFF_MM = CPS_OFF_NNP + ((sizeof(CpAtom) * CPS_MAX_NNP + 255) & ~(size_t)255);
+constexpr size_t CPS_OFF_EPART = CPS_OFF_MM + ((sizeof(CpAtom) * CPS_MAX_MM + 255) & ~(size_t)255);
+constexpr size_t CPS_OFF_FPART = CPS_OFF_EPART + ((sizeof(double) * CPS_MAX_PART + 255) & ~(size_t)255);
+constexpr size_t CPS_BYTES = CPS_OFF_FPART + sizeof(double) * 3 * (size_t)CPS_MAX_PART * CPS_MAX_NNP;  // ~1.8 MB
+
+static __device__ __align__(256) unsigned char g_cp_scratch[CPS_BYTES];
+
+// device lists (structure of arrays, as the caller holds them) -> the packed records the kernels read
+__global__ void __launch_bounds__(CP_THREADS) coupling_pack_kernel(CpAtom* __restrict__ dst_nnp, int n_nnp,
+                                                                    const int* __restrict__ nnp_rows, const float* __restrict__ q_nnp,
+                                                                    const float* __restrict__ s_nnp, const float* __restrict__ e_nnp,
+                                                                    CpAtom* __restrict__ dst_mm, int n_mm,
+                                                                    const int* __restrict__ mm_rows, const float* __restrict__ q_mm,
+                                                                    const float* __restrict__ s_mm, const float* __restrict__ e_mm) {
+  const int k = blockIdx.x * CP_THREADS + threadIdx.x;
+  if (k < n_nnp) dst_nnp[k] = CpAtom{nnp_rows[k], q_nnp[k], s_nnp[k], e_nnp[k]};
+  if (k < n_mm) dst_mm[k] = CpAtom{mm_rows[k], q_mm[k], s_mm[k], e_mm[k]};
+}
+
+constexpr int CPS_MAX_DEVICES = 64;
+unsigned char* g_cp_scratch_ptr[CPS_MAX_DEVICES];  // device address of g_cp_scratch, per device; null = not set up
+
+// once per device, with that device current
+int static_scratch(unsigned char** out) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return NNP_ERR_CUDA;
+  if (dev < 0 || dev >= CPS_MAX_DEVICES) return NNP_ERR_INVALID_ARG;
+  unsigned char* p = __atomic_load_n(&g_cp_scratch_ptr[dev], __ATOMIC_ACQUIRE);
+  if (!p) {
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return NNP_ERR_CUDA;
+    if (prop.major != 10) return NNP_ERR_UNSUPPORTED_ARCH;
+    void* sym = nullptr;
+    if (cudaGetSymbolAddress(&sym, g_cp_scratch) != cudaSuccess || !sym) {
+      cudaGetLastError();
+      return NNP_ERR_CUDA;
+    }
+    p = static_cast<unsigned char*>(sym);
+    __atomic_store_n(&g_cp_scratch_ptr[dev], p, __ATOMIC_RELEASE);  // the same value from whichever thread gets here first
+  }
+  *out = p;
+  return NNP_OK;
+}
+
+}  // namespace
+
+extern "C" int nnp_coupling_static_init(void) {
+  unsigned char* p = nullptr;
+  return static_scratch(&p);
+}
+
+extern "C" int nnp_coupling_compute_static(int32_t n_nnp, const int32_t* d_nnp_rows, const float* d_q_nnp,
+                                           const float* d_sigma_nnp, const float* d_eps_nnp, int32_t n_mm,
+                                           const int32_t* d_mm_rows, const float* d_q_mm, const float* d_sigma_mm,
+                                           const float* d_eps_mm, double coulomb_const, double cutoff, double length_scale,
+                                           const float* d_pos, int32_t pos_stride_floats, double* d_energy,
+                                           float* d_force_accum, int32_t force_stride_floats, void* cuda_stream) {
+  if (n_nnp < 0 || n_mm < 0 || !(length_scale > 0.0)) return NNP_ERR_INVALID_ARG;
+  if (n_nnp > CPS_MAX_NNP || n_mm > CPS_MAX_MM) return NNP_ERR_STATIC_LIMIT;
+  if (!d_pos || pos_stride_floats < 3 || (d_force_accum && force_stride_floats < 3)) return NNP_ERR_INVALID_ARG;
+  if (n_nnp > 0 && (!d_nnp_rows || !d_q_nnp || !d_sigma_nnp || !d_eps_nnp)) return NNP_ERR_INVALID_ARG;
+  if (n_mm > 0 && (!d_mm_rows || !d_q_mm || !d_sigma_mm || !d_eps_mm)) return NNP_ERR_INVALID_ARG;
+  unsigned char* scratch = nullptr;
+  const int rc = static_scratch(&scratch);
+  if (rc != NNP_OK) return rc;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  CpAtom* nnp = reinterpret_cast<CpAtom*>(scratch + CPS_OFF_NNP);
+  CpAtom* mm = reinterpret_cast<CpAtom*>(scratch + CPS_OFF_MM);
+  double* e_part = reinterpret_cast<double*>(scratch + CPS_OFF_EPART);
+  double* f_part = reinterpret_cast<double*>(scratch + CPS_OFF_FPART);
+  const int n_max = n_nnp > n_mm ? n_nnp : n_mm;
+  if (n_max > 0)
+    coupling_pack_kernel<<<(n_max + CP_THREADS - 1) / CP_THREADS, CP_THREADS, 0, s>>>(
+        nnp, n_nnp, d_nnp_rows, d_q_nnp, d_sigma_nnp, d_eps_nnp, mm, n_mm, d_mm_rows, d_q_mm, d_sigma_mm, d_eps_mm);
+  const CpArgs args{nnp, mm, n_nnp, n_mm, coulomb_const, cutoff > 0.0 ? cutoff * cutoff : 0.0, length_scale};
+  const int n_part = (n_mm + CP_THREADS - 1) / CP_THREADS;
+  if (n_mm > 0)
+    coupling_mm_kernel<<<n_part, CP_THREADS, 0, s>>>(args, d_pos, pos_stride_floats, d_force_accum, force_stride_floats, 0,
+                                                     e_part, f_part);
+  const int nb = (n_nnp + CP_THREADS / 32 - 1) / (CP_THREADS / 32);
+  coupling_nnp_kernel<<<nb > 0 ? nb : 1, CP_THREADS, 0, s>>>(args, d_force_accum, force_stride_floats, 0, e_part, f_part,
+                                                            n_mm > 0 ? n_part : 0, d_energy);
+  return cudaGetLastError() == cudaSuccess ? NNP_OK : NNP_ERR_CUDA;
+}

@@ -54,6 +54,7 @@ extern "C" const char* nnp_error_string(int code) {
     case NNP_ERR_CAPACITY: return "neighbour row capacity exceeded";
     case NNP_ERR_NONFINITE: return "non-finite position";
     case NNP_ERR_ALLOC: return "allocation failed";
+    case NNP_ERR_STATIC_LIMIT: return "more atoms than the fixed scratch array of nnp_coupling_compute_static holds";
     default: return "unknown error";
   }
 }
