@@ -547,13 +547,16 @@ __global__ void __launch_bounds__(AEV_THREADS, AEV_MINB) aev_forward_kernel(
 
 // ------------------------------------------------------------------------------------------------
 // A7: AEV backward.  One CTA per centre.  phi[i][slot] = dE/d(r_j - r_i) for every radial slot of i
-// (pair-gradient formulation: no atomics, the force gather happens per atom afterwards).
+// (pair-gradient formulation), added to the two atoms of the pair in 64-bit fixed point (integer atomics only).
 //   angular: one THREAD per triplet.  With G the n_shf_a x n_shf_z block of dE/dAEV of the triplet's
 //   species pair,  R0 = sum_a F2_a (G F1)_a,  R1 = sum_a dF2_a (G F1)_a,  R2 = sum_a F2_a (G dF1)_a  are
 //   register sums (4 powers + 8 Gaussians + 8 float4 shared-memory loads per triplet for ANI-2x); the
 //   triplet's two pair gradients go to a shared-memory buffer and one thread per (neighbour, component)
 //   adds them in triplet order (fixed order => bit-identical reruns).
 // ------------------------------------------------------------------------------------------------
+constexpr int FACC_BITS = 44;  // fixed-point force accumulator: 2^-44 model force units per count, range +-5e5
+constexpr double FACC_ONE = 17592186044416.0;  // 2^44
+
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
@@ -567,7 +570,7 @@ __global__ void __launch_bounds__(AEV_THREADS, MULTI ? 4 : AEV_MINB) aev_backwar
     const float4* __restrict__ pos4, const int* __restrict__ nbr_r, const int* __restrict__ nbr_a,
     const int* __restrict__ cnt_r, const int* __restrict__ cnt_a, const int* __restrict__ sortpos, int N,
     const __grid_constant__ AevConst c, int capR, int capA, int CH, const float* __restrict__ daev, int n_parts,
-    size_t part_stride, unsigned long long live_boxes, float* __restrict__ phi) {
+    size_t part_stride, unsigned long long live_boxes, unsigned long long* __restrict__ facc) {
   extern __shared__ __align__(16) float smem[];
   const int i = blockIdx.x;
   const CentreTab t = carve_tab(smem, capR, capA, c.S);
@@ -760,24 +763,47 @@ __global__ void __launch_bounds__(AEV_THREADS, MULTI ? 4 : AEV_MINB) aev_backwar
     __syncthreads();
   }
   __syncthreads();
-  float* out = phi + (size_t)i * capR * 3;
-  for (int f = threadIdx.x; f < 3 * nr; f += blockDim.x) out[f] = phr[f] + pha[f];
+  // A8, first half: phi[i][q] = dE/d(r_j - r_i) is a force of +phi on the centre i and of -phi on the neighbour j.
+  // Both go straight into the per-atom accumulator facc[N][3] as 64-bit fixed point (2^FACC_BITS per model force
+  // unit): integer adds commute, so the sum has the same bits in whatever order the centres arrive (bit-identical
+  // reruns without a gather pass; the previous design wrote phi[N][capR][3] and the finish kernel looked up, by binary
+  // search, the slot of every atom in the rows of its neighbours).  Centre: the threads add up their own terms, one
+  // shuffle tree per warp, three atomics per warp.
+  {
+    long long self[3] = {0, 0, 0};
+    const int* rowi = nbr_r + (size_t)i * capR;
+    for (int f = threadIdx.x; f < 3 * nr; f += blockDim.x) {
+      const int q = f / 3, comp = f - 3 * q;
+      const long long v = __double2ll_rn((double)(phr[f] + pha[f]) * FACC_ONE);
+      atomicAdd(facc + (size_t)rowi[q] * 3 + comp, (unsigned long long)(-v));
+      self[0] += comp == 0 ? v : 0;
+      self[1] += comp == 1 ? v : 0;
+      self[2] += comp == 2 ? v : 0;
+    }
+#pragma unroll
+    for (int comp = 0; comp < 3; ++comp) {
+      long long v = self[comp];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
+      if ((threadIdx.x & 31) == 0 && v != 0) atomicAdd(facc + (size_t)i * 3 + comp, (unsigned long long)v);
+    }
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
-// A8 + A5: F_a = sum_j phi[a][j] - sum_i phi[i][a], added into the caller's force buffer (mechanical
-// embedding); energies per molecule in FP64.  Blocks [0, n_force_blocks) do forces
-// (warp per atom), the remaining blocks do energies (warp per molecule).  Fixed reduction trees,
-// no atomics => bit-identical reruns.
+// A8 (second half) + A5: F_a = sum_j phi[a][j] - sum_i phi[i][a] sits in the fixed-point accumulator facc (filled by
+// the AEV backward kernel); it is converted, scaled, added into the caller's force buffer (mechanical embedding,
+// PAPER.md:50-71,75) and the accumulator entry is cleared for the next step.  Energies per molecule in FP64.  Blocks
+// [0, n_force_blocks) do forces (thread per atom), the remaining blocks do energies.  Integer accumulation and fixed
+// reduction trees => bit-identical reruns.
 // ------------------------------------------------------------------------------------------------
 constexpr int FIN_THREADS = 256;
 constexpr int FIN_WARPS = FIN_THREADS / 32;
 
 __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(
-    const int* __restrict__ nbr_r, const int* __restrict__ cnt_r, const float* __restrict__ phi, int N, int capR,
-    const int* __restrict__ atom_index, void* __restrict__ force, int force_stride, int fixed, float fscale,
-    int n_force_blocks, const double* __restrict__ eatom, const int* __restrict__ sortpos,
-    const int* __restrict__ species, const int* __restrict__ mol_off, int n_mol, int M,
+    unsigned long long* __restrict__ facc, int N, const int* __restrict__ atom_index, void* __restrict__ force,
+    int force_stride, int fixed, float fscale, int n_force_blocks, const double* __restrict__ eatom,
+    const int* __restrict__ sortpos, const int* __restrict__ species, const int* __restrict__ mol_off, int n_mol, int M,
     const double* __restrict__ self_energy, double escale, double* __restrict__ energy,
     const EnergyBlock* __restrict__ eblocks, int n_eblocks, double* __restrict__ epart, int* __restrict__ ecount) {
   const int lane = threadIdx.x & 31;
@@ -785,47 +811,31 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(
   pdl_trigger();
   pdl_wait();
   if ((int)blockIdx.x < n_force_blocks) {
-    const int a = blockIdx.x * FIN_WARPS + wib;
-    if (a >= N || force == nullptr) return;
-    const int n = cnt_r[a];
-    float fx = 0.f, fy = 0.f, fz = 0.f;
-    for (int s = lane; s < n; s += 32) {
-      const int i = nbr_r[(size_t)a * capR + s];
-      // slot of a in the (sorted) row of i: binary search
-      const int* rowi = nbr_r + (size_t)i * capR;
-      int lo = 0, hi = cnt_r[i] - 1, slot = -1;
-      while (lo <= hi) {
-        const int mid = (lo + hi) >> 1;
-        const int v = rowi[mid];
-        if (v == a) { slot = mid; break; }
-        if (v < a) lo = mid + 1; else hi = mid - 1;
-      }
-      const float* own = phi + ((size_t)a * capR + s) * 3;
-      fx += own[0]; fy += own[1]; fz += own[2];
-      if (slot >= 0) {
-        const float* oth = phi + ((size_t)i * capR + slot) * 3;
-        fx -= oth[0]; fy -= oth[1]; fz -= oth[2];
-      }
-    }
-    fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
-    if (lane == 0) {
-      const int row = atom_index ? atom_index[a] : a;
-      if (fixed & 1) {
-        // 64-bit fixed point (2^32 per force unit, the accumulation format of GPU MD engines): integer atomic adds
-        // commute, so MM kernels running CONCURRENTLY may add into the same buffer and the sum has the same bits in
-        // any order (NNP and MM concurrently instead of sequentially)
-        unsigned long long* f = reinterpret_cast<unsigned long long*>(force) + (size_t)row * force_stride;
-        const double sc = (double)fscale * 4294967296.0;
-        atomicAdd(f + 0, (unsigned long long)__double2ll_rn(sc * (double)fx));
-        atomicAdd(f + 1, (unsigned long long)__double2ll_rn(sc * (double)fy));
-        atomicAdd(f + 2, (unsigned long long)__double2ll_rn(sc * (double)fz));
-      } else if (fixed & 2) {  // nnp_compute_host: the buffer is the library's own, forces are WRITTEN
-        float* f = reinterpret_cast<float*>(force) + (size_t)row * force_stride;
+    const int a = blockIdx.x * FIN_THREADS + threadIdx.x;
+    if (a >= N) return;
+    unsigned long long* acc = facc + (size_t)a * 3;
+    const long long ix = (long long)acc[0], iy = (long long)acc[1], iz = (long long)acc[2];
+    acc[0] = 0ull; acc[1] = 0ull; acc[2] = 0ull;  // ready for the next step, whether or not forces were asked for
+    if (force == nullptr) return;
+    const double inv = 1.0 / FACC_ONE;
+    const int row = atom_index ? atom_index[a] : a;
+    if (fixed & 1) {
+      // 64-bit fixed point (2^32 per force unit, the accumulation format of GPU MD engines): integer atomic adds
+      // commute, so MM kernels running CONCURRENTLY may add into the same buffer and the sum has the same bits in
+      // any order (NNP and MM concurrently instead of sequentially)
+      unsigned long long* f = reinterpret_cast<unsigned long long*>(force) + (size_t)row * force_stride;
+      const double sc = (double)fscale * 4294967296.0 * inv;
+      atomicAdd(f + 0, (unsigned long long)__double2ll_rn(sc * (double)ix));
+      atomicAdd(f + 1, (unsigned long long)__double2ll_rn(sc * (double)iy));
+      atomicAdd(f + 2, (unsigned long long)__double2ll_rn(sc * (double)iz));
+    } else {
+      const float fx = (float)((double)ix * inv), fy = (float)((double)iy * inv), fz = (float)((double)iz * inv);
+      float* f = reinterpret_cast<float*>(force) + (size_t)row * force_stride;
+      if (fixed & 2) {  // nnp_compute_host: the buffer is the library's own, forces are WRITTEN
         f[0] = fscale * fx;
         f[1] = fscale * fy;
         f[2] = fscale * fz;
       } else {  // plain read-modify-write: safe only when every other adder is ordered with this stream
-        float* f = reinterpret_cast<float*>(force) + (size_t)row * force_stride;
         f[0] += fscale * fx;
         f[1] += fscale * fy;
         f[2] += fscale * fz;
@@ -844,6 +854,7 @@ __global__ void __launch_bounds__(FIN_THREADS) finish_kernel(
     for (int i = eb.a0 + (int)threadIdx.x; i < eb.a1; i += FIN_THREADS) {
       const double* e = eatom + (size_t)sortpos[i] * M;
       double s = 0.0;
+#pragma unroll 8
       for (int k = 0; k < M; ++k) s += e[k];
       acc += s / (double)M + (self_energy ? self_energy[species[i]] : 0.0);
     }
@@ -935,7 +946,7 @@ static void launch_aev_backward_t(nnp_handle* h, cudaStream_t s) {
   launch_kernel(h->pdl_now, aev_backward_kernel<NZ, NA, MULTI>, dim3(h->N), dim3(aev_block_threads(h, true)), aev_smem_bytes(h, true), s,
                 (const float4*)h->d_pos4, (const int*)h->d_nbr_r, (const int*)h->d_nbr_a, (const int*)h->d_cnt_r,
                 (const int*)h->d_cnt_a, (const int*)h->d_sortpos, h->N, h->aev, h->capR, h->capA, trip_chunk(h, true),
-                (const float*)h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->aev_live_boxes, h->d_phi);
+                (const float*)h->d_daev, h->n_parts, (size_t)h->N * h->n_feat, h->aev_live_boxes, h->d_facc);
 }
 
 void launch_aev_backward(nnp_handle* h, cudaStream_t s) {
@@ -953,11 +964,11 @@ void launch_aev_backward(nnp_handle* h, cudaStream_t s) {
 void launch_finish(nnp_handle* h, const int* d_atom_index, double* d_energy, void* d_force, int force_stride, int fixed,
                    cudaStream_t s) {
   if (h->N == 0) return;
-  const int nfb = (h->N + FIN_WARPS - 1) / FIN_WARPS;
+  const int nfb = (h->N + FIN_THREADS - 1) / FIN_THREADS;
   const int neb = h->n_eblocks;
   const float fscale = (float)(h->energy_scale * h->length_scale);
-  launch_kernel(h->pdl_now, finish_kernel, dim3(nfb + neb), dim3(FIN_THREADS), 0, s, h->d_nbr_r, h->d_cnt_r, h->d_phi,
-                h->N, h->capR, d_atom_index, d_force, force_stride, fixed, fscale, nfb, h->d_eatom, h->d_sortpos, h->d_species,
+  launch_kernel(h->pdl_now, finish_kernel, dim3(nfb + neb), dim3(FIN_THREADS), 0, s, h->d_facc, h->N, d_atom_index, d_force,
+                force_stride, fixed, fscale, nfb, h->d_eatom, h->d_sortpos, h->d_species,
                 h->d_mol_off, h->n_mol, h->M, h->d_self_energy, h->energy_scale, d_energy,
                 (const EnergyBlock*)h->d_eblocks, h->n_eblocks, h->d_epart, h->d_ecount);
 }

@@ -71,7 +71,7 @@ extern "C" void nnp_destroy(nnp_handle* h) {
   if (h->own_stream) cudaStreamDestroy(h->own_stream);
   for (auto e : h->events) cudaEventDestroy(e);
   void* ptrs[] = {h->d_eblocks, h->d_epart, h->d_ecount, h->d_mol_range, h->d_species, h->d_mol_off, h->d_mol_id, h->d_sortpos, h->d_perm, h->d_grp_off, h->d_self_energy,
-                  h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_aev, h->d_daev, h->d_phi,
+                  h->d_pos4, h->d_nbr_r, h->d_nbr_a, h->d_cnt_r, h->d_cnt_a, h->d_aev, h->d_daev, h->d_facc,
                   h->d_eatom, h->d_status, h->d_W, h->d_b,
                   h->d_aev_lo, h->d_Whi, h->d_Wlo, h->d_WThi, h->d_WTlo, h->d_act_full};
   for (void* p : ptrs)
@@ -331,7 +331,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   if (dev_alloc(&h->d_pos4, (size_t)N) || dev_alloc(&h->d_nbr_r, (size_t)N * h->capR) ||
       dev_alloc(&h->d_nbr_a, (size_t)N * h->capA) || dev_alloc(&h->d_cnt_r, (size_t)N) ||
       dev_alloc(&h->d_cnt_a, (size_t)N) || dev_alloc(&h->d_aev, (size_t)N * n_feat) ||
-      dev_alloc(&h->d_daev, (size_t)h->n_parts * N * n_feat) || dev_alloc(&h->d_phi, (size_t)N * h->capR * 3) ||
+      dev_alloc(&h->d_daev, (size_t)h->n_parts * N * n_feat) || dev_alloc(&h->d_facc, (size_t)N * 3) ||
       dev_alloc(&h->d_eatom, (size_t)N * M) || dev_alloc(&h->d_status, 1))
     return fail(NNP_ERR_ALLOC);
   h->hout_force_off = sizeof(double) * (size_t)n_molecules;
@@ -347,8 +347,9 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   // launch it saves (configs[2]: +36 us in the AEV forward against a 12 us neighbour kernel)
   h->fuse_nbr = N > 0 && N <= 512 && !h->use_cells && max_mol <= 512 && !(cfg->flags & NNP_FLAG_NO_NBR_FUSION);
   if (h->use_cells && cells_alloc(h) != 0) return fail(NNP_ERR_ALLOC);
-  {  // energy reduction blocks: chunks of <= 2048 atoms
-    const int ECH = 2048;
+  {  // energy reduction blocks: chunks of <= 512 atoms (two per thread: the loads of a thread are a dependent chain
+     // sortpos -> atomic energies, so short chunks on many CTAs beat long ones: configs[4] finish 18 -> see DESIGN.md)
+    const int ECH = 512;
     std::vector<EnergyBlock> eb;
     for (int m = 0; m < n_molecules; ++m) {
       const int a0 = mol_off[m], a1 = mol_off[m + 1];
@@ -366,7 +367,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   cudaMemset(h->d_nbr_a, 0, sizeof(int) * std::max<size_t>((size_t)N * h->capA, 1));
   cudaMemset(h->d_cnt_r, 0, sizeof(int) * std::max<size_t>(N, 1));
   cudaMemset(h->d_cnt_a, 0, sizeof(int) * std::max<size_t>(N, 1));
-  cudaMemset(h->d_phi, 0, sizeof(float) * std::max<size_t>((size_t)N * h->capR * 3, 1));
+  cudaMemset(h->d_facc, 0, sizeof(unsigned long long) * std::max<size_t>((size_t)N * 3, 1));
   cudaMemset(h->d_eatom, 0, sizeof(double) * std::max<size_t>((size_t)N * M, 1));
   cudaMemset(h->d_daev, 0, sizeof(float) * std::max<size_t>((size_t)h->n_parts * N * n_feat, 1));  // skipped tiles stay 0
 

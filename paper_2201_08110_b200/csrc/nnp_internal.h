@@ -275,7 +275,7 @@ struct nnp_handle {
   float* d_aev = nullptr;   // [N sorted][n_feat]
   float* d_aev_lo = nullptr;  // tensor engine: lo plane (d_aev then holds rna_tf32(G), d_aev_lo = G - that)
   float* d_daev = nullptr;  // [n_parts][N sorted][n_feat]
-  float* d_phi = nullptr;   // [N][capR][3]
+  unsigned long long* d_facc = nullptr;  // [N][3] fixed-point force accumulator (AEV backward adds, finish reads + clears)
   double* d_eatom = nullptr;  // [N sorted][M]
   EnergyBlock* d_eblocks = nullptr;  // energy reduction: large molecules are summed by several CTAs
   double* d_epart = nullptr;         // [n_eblocks] partial sums
