@@ -199,10 +199,10 @@ static int ang_row_pad(const nnp_handle* h) {  // floats per padded angular bloc
 }
 
 // shared memory (floats): table | asl[capA] | sp_off[S+1] | pair_st[n_pairs] | tmp[2 capA] | pres[n_pairs+1] |
-// r_off[S+1] | kernel part
+// r_off[S+1] | boff[n_pairs+1] | kernel part
 static size_t aev_common_floats(const nnp_handle* h) {
   const int S = h->S;
-  return (size_t)TAB_FIELDS * h->capR + 3 * (size_t)h->capA + 2 * (S + 1) + (size_t)S * (S + 1) + 1;
+  return (size_t)TAB_FIELDS * h->capR + 3 * (size_t)h->capA + 2 * (S + 1) + 3 * ((size_t)S * (S + 1) / 2) + 2;
 }
 static size_t aev_smem_bytes_ch(const nnp_handle* h, bool backward, int CH) {
   size_t fl = aev_common_floats(h);
@@ -256,6 +256,7 @@ struct CentreTab {
   int* pair_st;  // [n_pairs] (s << 8) | t of every species-pair block, s <= t
   int* tmp;      // [2 capA] scratch of build_tab: angular slots and their species in list order
   int* pres;     // [n_pairs + 1] species-pair blocks that have at least one triplet (ascending), count at [n_pairs]
+  int* boff;     // [n_pairs + 1] first triplet of every PRESENT block in the block-ordered triplet enumeration
   float* rest;   // kernel-specific part (16-byte aligned)
 };
 
@@ -271,7 +272,8 @@ __device__ __forceinline__ CentreTab carve_tab(float* smem, int capR, int capA, 
   t.tmp = t.pair_st + S * (S + 1) / 2;
   t.pres = t.tmp + 2 * capA;
   t.r_off = t.pres + S * (S + 1) / 2 + 1;
-  const int used = TAB_FIELDS * capR + 3 * capA + 2 * (S + 1) + S * (S + 1) + 1;
+  t.boff = t.r_off + (S + 1);
+  const int used = TAB_FIELDS * capR + 3 * capA + 2 * (S + 1) + 3 * (S * (S + 1) / 2) + 2;
   t.rest = smem + ((used + 3) & ~3);
   return t;
 }
@@ -384,6 +386,27 @@ __device__ __forceinline__ void build_tab(const CentreTab& t, int i, int nr, int
       count += __popc(b);
     }
     if (threadIdx.x == 0) t.pres[n_pairs] = count;
+    __syncwarp();
+    // block-ordered triplet enumeration: the triplets of present block pp are [boff[pp], boff[pp + 1]) (warp scan)
+    int carry = 0;
+    for (int base = 0; base < count; base += 32) {
+      const int pp = base + (int)threadIdx.x;
+      int cnt = 0;
+      if (pp < count) {
+        const int st = t.pair_st[t.pres[pp]], s = st >> 8, u = st & 255;
+        const int ns = t.sp_off[s + 1] - t.sp_off[s], nu = t.sp_off[u + 1] - t.sp_off[u];
+        cnt = s == u ? (ns * (ns - 1)) >> 1 : ns * nu;
+      }
+      int incl = cnt;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(FULL, incl, o);
+        if ((int)threadIdx.x >= o) incl += v;
+      }
+      if (pp < count) t.boff[pp + 1] = carry + incl;
+      carry += __shfl_sync(FULL, incl, 31);
+    }
+    if (threadIdx.x == 0) t.boff[0] = 0;
   }
   __syncthreads();
 }
@@ -483,11 +506,33 @@ __global__ void __launch_bounds__(AEV_THREADS, AEV_MINB) aev_forward_kernel(
 
   // ---- angular (O4)
   const int ntrip = (na * (na - 1)) >> 1;
+  const int n_pres = t.pres[(c.S * (c.S + 1)) >> 1];
   for (int c0 = 0; c0 < ntrip; c0 += CH) {
     const int cn = min(CH, ntrip - c0);
     for (int tl = threadIdx.x; tl < cn; tl += blockDim.x) {
+      // triplet number c0 + tl of the BLOCK-ORDERED enumeration (all triplets of the first present species-pair block,
+      // then the next ...; inside a block (a, b) row-major as before): the column sums below are then plain ranges
+      const int g = c0 + tl;
+      int lo_pp = 0, hi_pp = n_pres;  // boff[lo_pp] <= g < boff[hi_pp]
+      while (hi_pp - lo_pp > 1) {
+        const int mid = (lo_pp + hi_pp) >> 1;
+        if (t.boff[mid] <= g) lo_pp = mid; else hi_pp = mid;
+      }
       int a, b;
-      trip_decode(c0 + tl, na, a, b);
+      {
+        const int st = t.pair_st[t.pres[lo_pp]], s = st >> 8, u = st & 255;
+        const int local = g - t.boff[lo_pp];
+        const int a0 = t.sp_off[s];
+        if (s == u) {
+          trip_decode(local, t.sp_off[s + 1] - a0, a, b);
+          a += a0; b += a0;
+        } else {
+          const int b0 = t.sp_off[u], nu = t.sp_off[u + 1] - b0;
+          const int qa_ = local / nu;
+          a = a0 + qa_;
+          b = b0 + (local - qa_ * nu);
+        }
+      }
       const int qa = t.asl[a], qb = t.asl[b];
       const float cth = t.ux[qa] * t.ux[qb] + t.uy[qa] * t.uy[qb] + t.uz[qa] * t.uz[qb];
       const float cc = c.cos_scale * cth;
@@ -511,24 +556,17 @@ __global__ void __launch_bounds__(AEV_THREADS, AEV_MINB) aev_forward_kernel(
       }
     }
     __syncthreads();
-    const int n_out = t.pres[(c.S * (c.S + 1)) >> 1] * c.n_sub;  // columns of the blocks that have triplets
+    const int n_out = n_pres * c.n_sub;  // columns of the blocks that have triplets
     for (int fo = threadIdx.x; fo < n_out; fo += blockDim.x) {
       const int pp = fo / c.n_sub, sub = fo - pp * c.n_sub;
-      const int p = t.pres[pp], f = p * c.n_sub + sub;
+      const int f = t.pres[pp] * c.n_sub + sub;
       const int ia = sub / c.n_shf_z, iz = sub - ia * c.n_shf_z;
-      const int st = t.pair_st[p];
-      const int s = st >> 8, u = st & 255;
-      const int a0 = t.sp_off[s], a1 = t.sp_off[s + 1], b0 = t.sp_off[u], b1 = t.sp_off[u + 1];
-      const float* f1 = bF1 + iz * CHP;
-      const float* f2 = bF2 + ia * CHP;
+      const float* f1 = bF1 + iz * CHP - c0;
+      const float* f2 = bF2 + ia * CHP - c0;
+      const int lo = max(t.boff[pp], c0), hi = min(t.boff[pp + 1], c0 + cn);  // the block's triplets in this pass
       float acc = 0.0f;
-      for (int a = a0; a < a1; ++a) {
-        const int base = trip_row_start(a, na) - a - 1 - c0;  // local index of (a, b) is base + b
-        const int lo = max(s == u ? a + 1 : b0, -base);
-        const int hi = min(b1, cn - base);
 #pragma unroll 4
-        for (int b = lo; b < hi; ++b) acc = fmaf(f1[base + b], f2[base + b], acc);
-      }
+      for (int g = lo; g < hi; ++g) acc = fmaf(f1[g], f2[g], acc);
       row[f] += acc;
     }
     __syncthreads();
