@@ -592,7 +592,7 @@ __global__ void __launch_bounds__(AEV_THREADS, AEV_MINB) aev_forward_kernel(
 //   triplet's two pair gradients go to a shared-memory buffer and one thread per (neighbour, component)
 //   adds them in triplet order (fixed order => bit-identical reruns).
 // ------------------------------------------------------------------------------------------------
-constexpr int FACC_BITS = 44;  // fixed-point force accumulator: 2^-44 model force units per count, range +-5e5
+// fixed-point force accumulator: 2^-44 model force units per count, range +-5e5
 constexpr double FACC_ONE = 17592186044416.0;  // 2^44
 
 __device__ __forceinline__ float warp_sum(float v) {
