@@ -87,6 +87,7 @@ typedef struct {
 #define NNP_FLAG_FORCE_CELLS 128 /* neighbour search: cell binning even for small molecules (default: molecules >= 1024 atoms) */
 #define NNP_FLAG_NO_FWD1 256     /* ligand-size engine: row-pair layer-1 forward kernel instead of the persistent ring-fed one */
 #define NNP_FLAG_NO_NBR_FUSION 1024 /* small molecules: separate neighbour launch instead of building the rows inside the AEV forward kernel */
+#define NNP_FLAG_NO_TAIL_SPLIT 8192 /* tensor engine: whole tiles only (default: the tiles of a layer-1 backward launch that do not fill a round of the machine are cut along the contraction into parts on different SMs) */
 #define NNP_FLAG_UMMA_PAIRS 4096 /* tensor engine, opt-in: the two layer-1 launches of a large system (every element >= 512 atoms) on CTA pairs (tcgen05 cta_group::2, 256 x 256 tiles); correct and measured SLOWER than the default one-CTA tiles */
 #define NNP_FLAG_NO_SWEEP_REVERSAL 512 /* tensor engine: every launch sweeps the (element, model) blocks in the same direction (A/B switch for the L2 reuse between consecutive launches) */
 #define NNP_FLAG_NO_ZERO_SKIP 2048 /* tensor engine: run layer 1 densely even over AEV columns that are structurally zero */

@@ -26,6 +26,7 @@ NNP_FLAG_NO_SWEEP_REVERSAL = 512
 NNP_FLAG_NO_NBR_FUSION = 1024
 NNP_FLAG_NO_ZERO_SKIP = 2048
 NNP_FLAG_UMMA_PAIRS = 4096
+NNP_FLAG_NO_TAIL_SPLIT = 8192
 ERRORS = {
     -1: "NNP_ERR_INVALID_ARG",
     -2: "NNP_ERR_CUDA",

@@ -69,7 +69,7 @@ __device__ __forceinline__ void drain_sync() { asm volatile("bar.sync 1, %0;" ::
 template <int NP>
 __device__ __forceinline__ void drain_item(const UmmaItem& t, const UmmaParams& P, uint32_t tmem, uint64_t* slot_full,
                                            uint64_t* slot_empty, float* staging, uint32_t slot_ctr, int quarter, int half,
-                                           int lane, int dt) {
+                                           int lane, int dt, int* split_last) {
   constexpr int CT = NP >= 32 ? NP / 2 : NP;       // columns per thread
   constexpr bool TWO_LEVEL = NP <= 64;
   const bool active = NP >= 32 || half == 0;
@@ -122,6 +122,47 @@ __device__ __forceinline__ void drain_item(const UmmaItem& t, const UmmaParams& 
   }
   // ---- epilogue, one half of the tile per round
   constexpr int ROUNDS = NP >= 32 ? 2 : 1;
+  if (NP == 128 && t.split_n > 0) {
+    // K-split part (EPI_SCALE): the raw partial tile goes to scratch; the part that draws the last ticket adds all
+    // parts in index order and scales.  [part][atom][feature], 16-byte accesses, the thread -> element map of
+    // epilogue_rows (every thread reads back only what the same thread position of the other parts wrote).
+    const int g = dt & 31, r0 = dt >> 5;
+    float* mine = t.scratch + (size_t)t.split_idx * 128 * 128;
+#pragma unroll
+    for (int h = 0; h < ROUNDS; ++h) {
+      if (active && half == h) {
+        float* dst = staging + quarter * 32 + lane;
+#pragma unroll
+        for (int j = 0; j < CT; ++j) dst[j * 128] = tot[j];
+      }
+      drain_sync();
+      for (int r = r0; r < 64; r += U_DRAIN_THREADS / 32) st4(mine + (size_t)(h * 64 + r) * 128 + 4 * g, ld4(staging + r * 128 + 4 * g));
+      drain_sync();
+    }
+    __threadfence();
+    drain_sync();
+    if (dt == 0) {
+      const unsigned int ticket = atomicAdd(t.ticket, 1u);
+      *split_last = ticket == (unsigned int)t.split_n - 1u;
+      if (*split_last) *t.ticket = 0u;  // all parts have arrived; the next launch is ordered after this kernel
+    }
+    drain_sync();
+    if (*split_last) {
+      __threadfence();
+      if (4 * g < t.f_valid)
+        for (int r = r0; r < t.n_valid; r += U_DRAIN_THREADS / 32) {
+          float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
+          for (int q = 0; q < t.split_n; ++q) {
+            const float4 v = __ldcg(reinterpret_cast<const float4*>(t.scratch + ((size_t)q * 128 + r) * 128 + 4 * g));
+            x.x += v.x; x.y += v.y; x.z += v.z; x.w += v.w;
+          }
+          x.x *= t.scale; x.y *= t.scale; x.z *= t.scale; x.w *= t.scale;
+          st4(t.C + (size_t)r * t.ldc + 4 * g, x);
+        }
+    }
+    drain_sync();  // split_last is read above and rewritten by the next split item
+    return;
+  }
 #pragma unroll
   for (int h = 0; h < ROUNDS; ++h) {
     if (active && half == h) {
@@ -146,6 +187,7 @@ __global__ void __launch_bounds__(U_THREADS, 1) gemm_umma_kernel(const __grid_co
   uint64_t* slot_full = empty + U_MAX_STAGES;       // [U_MAX_SLOTS]  slot accumulated
   uint64_t* slot_empty = slot_full + U_MAX_SLOTS;   // [U_MAX_SLOTS]  slot drained
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(slot_empty + U_MAX_SLOTS);
+  int* split_last = reinterpret_cast<int*>(tmem_slot + 1);  // K-split items: "this part drew the last ticket"
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
     for (int s = 0; s < P.n_stages; ++s) {
@@ -188,8 +230,11 @@ __global__ void __launch_bounds__(U_THREADS, 1) gemm_umma_kernel(const __grid_co
                 nkb = __shfl_sync(0xffffffffu, t.nkb, 0);
       const uint32_t tx = 2u * A_BOX_BYTES + 2u * (uint32_t)__shfl_sync(0xffffffffu, t.n_pad, 0) * 128u;
       unsigned long long live = __shfl_sync(0xffffffffu, t.kmask, 0);
+      const int kb_skip = __shfl_sync(0xffffffffu, t.kb_skip, 0);  // K-split part: its first box within the tile
+      if (live)
+        for (int q = 0; q < kb_skip; ++q) live &= live - 1;
       for (int kbi = 0; kbi < nkb; ++kbi) {
-        int kb = kbi;
+        int kb = kb_skip + kbi;
         if (live) {  // skip the contraction boxes that only hold structural zeros
           kb = __ffsll((long long)live) - 1;
           live &= live - 1;
@@ -272,10 +317,10 @@ __global__ void __launch_bounds__(U_THREADS, 1) gemm_umma_kernel(const __grid_co
     for (int it = it0; it < it1; ++it) {
       const UmmaItem t = P.items[it];
       switch (t.n_pad) {
-        case 16: drain_item<16>(t, P, tmem, slot_full, slot_empty, staging, slot_ctr, quarter, half, lane, dt); break;
-        case 32: drain_item<32>(t, P, tmem, slot_full, slot_empty, staging, slot_ctr, quarter, half, lane, dt); break;
-        case 64: drain_item<64>(t, P, tmem, slot_full, slot_empty, staging, slot_ctr, quarter, half, lane, dt); break;
-        default: drain_item<128>(t, P, tmem, slot_full, slot_empty, staging, slot_ctr, quarter, half, lane, dt); break;
+        case 16: drain_item<16>(t, P, tmem, slot_full, slot_empty, staging, slot_ctr, quarter, half, lane, dt, split_last); break;
+        case 32: drain_item<32>(t, P, tmem, slot_full, slot_empty, staging, slot_ctr, quarter, half, lane, dt, split_last); break;
+        case 64: drain_item<64>(t, P, tmem, slot_full, slot_empty, staging, slot_ctr, quarter, half, lane, dt, split_last); break;
+        default: drain_item<128>(t, P, tmem, slot_full, slot_empty, staging, slot_ctr, quarter, half, lane, dt, split_last); break;
       }
       slot_ctr += (uint32_t)t.nkb;
     }
@@ -416,7 +461,7 @@ static void plan_items(UmmaPlan& pl, const std::vector<UmmaProblem>& probs, cons
 }
 
 int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, const std::vector<UmmaOperand>& aops,
-                      const std::vector<UmmaOperand>& bops, int num_sms, bool reverse) {
+                      const std::vector<UmmaOperand>& bops, int num_sms, bool reverse, bool tail_split) {
   UmmaParams* P = new UmmaParams();
   memset(P, 0, sizeof(*P));
   L.params = P;
@@ -453,9 +498,69 @@ int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, cons
   if (reverse) std::reverse(order.begin(), order.end());
   const size_t G = std::max<size_t>(1, std::min<size_t>(n, (size_t)num_sms));
   std::vector<std::vector<UmmaItem>> per_cta(G);
-  for (size_t i = 0; i < n; ++i) {
+  // Tail of a launch with few, long items (layer-1 backward: 48-64 boxes per tile, 4.1 tiles per SM at configs[2] -- a
+  // fifth round for 14 of 606 tiles): the tiles that do not fill a round are cut along the contraction into split_n
+  // parts on different SMs, so the last round is 1/split_n of a tile long.  The parts exchange partial tiles through
+  // scratch memory; the part that arrives last adds them in index order and runs the epilogue (see UmmaItem).
+  size_t n_whole = n;
+  int split_n = 0;
+  {
+    bool scale_only = tail_split && n > 0 && np_max == 128;
+    int min_nkb = 1 << 30;
+    for (const UmmaItem& t : items) {
+      scale_only = scale_only && t.epi == EPI_SCALE && t.n_pad == 128;
+      min_nkb = std::min(min_nkb, t.nkb);
+    }
+    // r tiles are left after the whole rounds.  Cut into s parts each, an SM runs ceil(r s / G) parts of 1/s of a tile
+    // plus the fixed cost of a part (its own drain, the scratch traffic, a fence and the ticket: about 10 boxes' worth
+    // of time, measured: configs[4], 92 tiles left of 240, LOST 40 us with 8 parts and 5 us with 3) instead of one
+    // tile.  Take the s <= 8 with the shortest tail, if that saves at least 5 % of a round (configs[2]: 14 tiles left
+    // of 606, 8 parts, layer-1 backward 191 -> 179 us).
+    const size_t r = n % G;
+    if (scale_only && n >= G && r > 0 && !reverse) {
+      double best = 0.95;
+      const double ovh = 10.0 / (double)min_nkb;
+      for (int s_try = 2; s_try <= 8 && min_nkb >= 4 * s_try; ++s_try) {
+        const double tail = (double)((r * (size_t)s_try + G - 1) / G) * (1.0 / s_try + ovh);
+        if (tail < best - 1e-9) { best = tail; split_n = s_try; }
+      }
+      if (split_n) n_whole = n - r;
+    }
+  }
+  for (size_t i = 0; i < n_whole; ++i) {
     const size_t round = i / G, posn = i % G;
     per_cta[(round & 1) ? G - 1 - posn : posn].push_back(items[order[i]]);
+  }
+  if (split_n) {
+    const size_t r = n - n_whole;
+    L.n_split_tiles = (int)r;
+    L.split_n = split_n;
+    if (cudaMalloc((void**)&L.d_split_scratch, r * split_n * 128 * 128 * sizeof(float)) != cudaSuccess) return -1;
+    if (cudaMalloc((void**)&L.d_split_tickets, r * sizeof(unsigned int)) != cudaSuccess) return -1;
+    cudaMemset(L.d_split_tickets, 0, r * sizeof(unsigned int));
+    // the parts go to the CTAs with the least work so far (all equal after whole rounds: plain order)
+    std::vector<long long> load(G, 0);
+    for (size_t c = 0; c < G; ++c)
+      for (const UmmaItem& t : per_cta[c]) load[c] += (long long)t.nkb;
+    std::vector<size_t> by_load(G);
+    for (size_t c = 0; c < G; ++c) by_load[c] = c;
+    std::stable_sort(by_load.begin(), by_load.end(), [&](size_t a, size_t b) { return load[a] < load[b]; });
+    size_t next = 0;
+    for (size_t k = 0; k < r; ++k) {
+      const UmmaItem& whole = items[order[n_whole + k]];
+      for (int q = 0; q < split_n; ++q) {
+        UmmaItem t = whole;
+        const int b0 = (int)((long long)whole.nkb * q / split_n), b1 = (int)((long long)whole.nkb * (q + 1) / split_n);
+        t.kb_skip = b0;
+        t.nkb = b1 - b0;
+        t.split_n = split_n;
+        t.split_idx = q;
+        t.scratch = L.d_split_scratch + (size_t)k * split_n * 128 * 128;
+        t.ticket = L.d_split_tickets + k;
+        per_cta[by_load[next % G]].push_back(t);
+        ++next;
+      }
+    }
   }
   std::vector<UmmaItem> flat;
   std::vector<int> off(G + 1, 0);
@@ -463,7 +568,8 @@ int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, cons
     for (auto& t : per_cta[c]) flat.push_back(t);
     off[c + 1] = (int)flat.size();
   }
-  L.n_items = (int)n;
+  const size_t n_flat = n_whole + (size_t)L.n_split_tiles * (size_t)L.split_n;
+  L.n_items = (int)n_flat;
   L.grid = n ? (int)G : 0;
   L.tile = np_max;
   L.issued_flops = best.flops;
@@ -479,9 +585,9 @@ int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, cons
   P->n_slots = std::min(U_MAX_SLOTS, 512 / np_max);
   P->slot_shift = P->n_slots == 8 ? 3 : 2;
   P->comp = 1;
-  if (cudaMalloc((void**)&L.d_items, std::max<size_t>(1, n) * sizeof(UmmaItem)) != cudaSuccess) return -1;
+  if (cudaMalloc((void**)&L.d_items, std::max<size_t>(1, n_flat) * sizeof(UmmaItem)) != cudaSuccess) return -1;
   if (cudaMalloc((void**)&L.d_cta_off, (G + 1) * sizeof(int)) != cudaSuccess) return -1;
-  if (n) cudaMemcpy(L.d_items, flat.data(), n * sizeof(UmmaItem), cudaMemcpyHostToDevice);
+  if (n_flat) cudaMemcpy(L.d_items, flat.data(), n_flat * sizeof(UmmaItem), cudaMemcpyHostToDevice);
   cudaMemcpy(L.d_cta_off, off.data(), (G + 1) * sizeof(int), cudaMemcpyHostToDevice);
   P->items = L.d_items;
   P->cta_off = L.d_cta_off;
@@ -507,6 +613,10 @@ int umma_init() {
 void umma_free_launch(UmmaLaunch& L) {
   if (L.d_items) cudaFree(L.d_items);
   if (L.d_cta_off) cudaFree(L.d_cta_off);
+  if (L.d_split_scratch) cudaFree(L.d_split_scratch);
+  if (L.d_split_tickets) cudaFree(L.d_split_tickets);
+  L.d_split_scratch = nullptr;
+  L.d_split_tickets = nullptr;
   if (L.pair) umma2_free_params(L);
   else delete reinterpret_cast<UmmaParams*>(L.params);
   L.d_items = nullptr; L.d_cta_off = nullptr; L.params = nullptr;

@@ -598,7 +598,8 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
         // opt-in: the two layer-1 launches of large systems on CTA pairs (cta_group::2, 256 x 256 tiles)
         const bool pair = l == 1 && (cfg->flags & NNP_FLAG_UMMA_PAIRS) && umma2_suits(probs) && umma2_init() == 0;
         if (pair ? umma2_build_launch(ul, probs, aops, bops, prop.multiProcessorCount)
-                 : umma_build_launch(ul, probs, aops, bops, prop.multiProcessorCount, reverse)) {
+                 : umma_build_launch(ul, probs, aops, bops, prop.multiProcessorCount, reverse,
+                                     !(cfg->flags & NNP_FLAG_NO_TAIL_SPLIT))) {
           umma_free_launch(ul);
           return fail(NNP_ERR_CUDA);
         }

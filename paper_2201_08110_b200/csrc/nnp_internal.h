@@ -123,6 +123,14 @@ struct UmmaItem {            // one tile of one GEMM, as the persistent CTAs con
   float* C_full;
   const float* w_last;       // [f] weights of the 1-output layer for this tile's features
   float scale, alpha, inv_alpha;
+  // K-split tail items (EPI_SCALE launches): the item is one of split_n parts of a tile's contraction.  A part runs
+  // nkb boxes starting at box kb_skip of the tile's (live) box list, writes its raw partial tile to
+  // scratch[split_idx][128 atoms][128 features] and takes a ticket; the part that draws the last ticket adds the
+  // split_n partial tiles in index order (fixed order => bit-identical reruns) and runs the epilogue.  split_n = 0:
+  // a whole tile.
+  int kb_skip, split_n, split_idx;
+  float* scratch;
+  unsigned int* ticket;
 };
 struct UmmaProblem {
   unsigned long long kmask;    // non-zero: contraction boxes (32 wide) to run; the others multiply structural zeros
@@ -149,11 +157,15 @@ struct UmmaLaunch {
   bool pair = false;       // built by the CTA-pair engine (mlp_umma2.cu)
   double issued_flops = 0;
   double algo_bytes = 0;   // operand planes read once + output planes written once + epilogue reads  // 2 x MACs of the boxes actually run (padding and structural zeros excluded/included as issued)
+  float* d_split_scratch = nullptr;        // partial tiles of the K-split tail items
+  unsigned int* d_split_tickets = nullptr; // one arrival counter per split tile (zero between launches)
+  int n_split_tiles = 0, split_n = 0;
   std::string name;
 };
 int umma_init();
 int umma_build_launch(UmmaLaunch& L, const std::vector<UmmaProblem>& probs, const std::vector<UmmaOperand>& aops,
-                      const std::vector<UmmaOperand>& bops, int num_sms, bool reverse = false);
+                      const std::vector<UmmaOperand>& bops, int num_sms, bool reverse = false,
+                      bool tail_split = true);
 void umma_launch(const UmmaLaunch& L, cudaStream_t s, bool pdl);
 void umma_free_launch(UmmaLaunch& L);
 // CTA-pair variant (cta_group::2, 256 x 256 tiles): opt-in (NNP_FLAG_UMMA_PAIRS), measured slower

@@ -17,6 +17,7 @@ from paper_2201_08110_b200 import workloads as wl  # noqa: E402
 from paper_2201_08110_b200.binding import (NNP, NNP_FLAG_FORCE_CELLS, NNP_FLAG_NO_CELLS, NNP_FLAG_NO_GRAPH,  # noqa: E402
                                             NNP_FLAG_NO_FWD1, NNP_FLAG_NO_MID, NNP_FLAG_NO_NBR_FUSION, NNP_FLAG_NO_PDL, NNP_FLAG_NO_SMALL,
                                             NNP_FLAG_NO_UMMA, NNP_FLAG_NO_ZERO_SKIP, NNP_FLAG_NO_SWEEP_REVERSAL, NNP_FLAG_UMMA_PAIRS,
+                                            NNP_FLAG_NO_TAIL_SPLIT,
                                             NNPError)
 
 # MLP engines: ligand-size weight-streaming FFMA (default at these sizes; with the fused middle launch or
@@ -342,6 +343,26 @@ def test_cta_pair_engine_matches_the_one_cta_engine():
     assert abs(ra["E"][0] - rb["E"][0]) / w.n_atoms <= 1e-6
     assert np.abs(ra["F"] - rb["F"]).max() <= 1e-4
     assert np.abs(rb["F"]).max() > 1.0
+    a.destroy(); b.destroy()
+
+
+@pytest.mark.parametrize("cfg", [3])
+def test_k_split_tail_tiles_match_whole_tiles(cfg):
+    """Layer-1 backward: the tiles that do not fill a round of the machine are cut along the contraction into parts on
+    different SMs; the part that arrives last adds the partial tiles in index order.  Against whole tiles
+    (NNP_FLAG_NO_TAIL_SPLIT): same energies (the forward pass is untouched), dE/dAEV and forces equal up to the
+    regrouping of the FP32 slot sums; bit-identical from run to run whatever the arrival order."""
+    w = wl.get_config(cfg)
+    W, B = w.weights()
+    a = NNP(w.params, W, B, w.species, mol_offsets=w.mol_offsets)
+    b = NNP(w.params, W, B, w.species, mol_offsets=w.mol_offsets, flags=NNP_FLAG_NO_TAIL_SPLIT)
+    ra, rb = gpu_eval(a, w.positions, n_mol=w.n_molecules, stages=True), gpu_eval(b, w.positions, n_mol=w.n_molecules, stages=True)
+    assert np.array_equal(ra["E"], rb["E"])
+    assert np.abs(ra["dG"] - rb["dG"]).max() <= 1e-6 and np.abs(ra["F"] - rb["F"]).max() <= 2e-4
+    assert np.any(ra["dG"] != rb["dG"])  # the split is active at these sizes (else this test tests nothing)
+    for _ in range(3):
+        rc = gpu_eval(a, w.positions, n_mol=w.n_molecules, stages=True)
+        assert np.array_equal(rc["dG"], ra["dG"]) and np.array_equal(rc["F"], ra["F"])
     a.destroy(); b.destroy()
 
 
