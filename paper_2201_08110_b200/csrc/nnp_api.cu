@@ -262,11 +262,17 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     if (upload(&h->d_W, Wh) || upload(&h->d_b, B)) return fail(NNP_ERR_ALLOC);
   }
 
-  // ---- MLP engine: the tensor-core engine needs hidden widths that are whole 32-float TMA boxes
+  // ---- MLP engine: the tensor-core engine takes hidden widths that are multiples of 16.  A contraction that is not
+  // a whole number of 32-float TMA boxes is padded by the tensor maps: the WEIGHT operand of every GEMM is a tensor
+  // whose contraction extent is exactly K, so its box columns beyond K are zero-filled by TMA, and whatever the
+  // activation box holds there (the next model's activations, finite) is multiplied by zero.  ANI-1x: 144 and 112.
   bool box_ok = n_feat % 4 == 0 && N > 0;
-  for (int e = 0; e < S && box_ok; ++e)
+  for (int e = 0; e < S && box_ok; ++e) {
     for (int l = 1; l < L; ++l)
-      if (h->dims[e * (L + 1) + l] % 32 != 0) box_ok = false;
+      if (h->dims[e * (L + 1) + l] % 16 != 0) box_ok = false;
+    // layer-1 backward: the contraction runs over all models of the element, M * H1 must be whole boxes
+    if (((long long)M * h->dims[e * (L + 1) + 1]) % 32 != 0) box_ok = false;
+  }
   // ligand-size engine: every element group is small, so the layers are weight-streaming problems
   int max_grp = 0, max_dim = n_feat;
   for (int e = 0; e < S; ++e) {
@@ -286,9 +292,16 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     // AEV backward kernel sums (as it does at ligand sizes).
     long long tiles = 0;
     for (int e = 0; e < S; ++e) tiles += ((h->grp_off[e + 1] - h->grp_off[e] + 127) / 128) * (long long)((n_feat + 127) / 128);
+    // a group of models must be whole boxes of every element's contraction (the weight tensor of the layer-1 backward
+    // spans ALL models, so nothing zero-fills a box that runs into the next group)
+    auto group_ok = [&](int p) {
+      for (int e = 0; e < S; ++e)
+        if (((long long)(M / p) * h->dims[e * (L + 1) + 1]) % 32 != 0) return false;
+      return true;
+    };
     int parts = 1;
     while (parts < M && M % (2 * parts) == 0 && tiles * parts < 2LL * prop.multiProcessorCount &&
-           (size_t)N * (2 * parts) * n_feat * 4 <= ((size_t)64 << 20))
+           (size_t)N * (2 * parts) * n_feat * 4 <= ((size_t)64 << 20) && group_ok(2 * parts))
       parts *= 2;
     h->n_parts = parts;
     // 3xTF32 operand planes: weights hi = rna_tf32(w), lo = rna_tf32(w - hi), in the forward layout and transposed

@@ -199,8 +199,8 @@ def test_parameter_file_species_order_and_one_nn(tmp_path):
 @pytest.mark.parametrize("n,n_models", [(48, 8), (48, 1), (600, 2)])
 def test_ani1x_parameter_set(n, n_models):
     """NEXT-4: ANI-1x -- 4 elements, 384 features, Zeta = 32, 8 angular sections, its network
-    shapes -- on the ligand engine (48 atoms) and, at 600 atoms, on the grouped FFMA engine (hidden widths that are
-    not multiples of 32 are outside the tensor engine)."""
+    shapes -- on the ligand engine (48 atoms) and, at 600 atoms, on the tensor engine: its hidden widths 144 and 112
+    are not whole 32-float TMA boxes, the boxes that run past a contraction are zero-filled on the weight side."""
     w = wl.ani1x_ligand(n, n_models) if n == 48 else wl.random_molecule(n, 4, seed=640, params=wl.ani1x_params(), n_models=n_models)
     assert w.params.n_features == 384
     W, B = wl.make_weights(w.params, n_models, seed=31, random_biases=True)
@@ -224,6 +224,14 @@ def test_ani1x_parameter_set(n, n_models):
     bound = max(1e-5, float(np.abs(ref["dG"] * ref["G"]).sum(axis=1).mean()) * 1.5e-6 * zeta_factor * w.params.energy_scale)
     print(f"[parity] ani1x n={n} M={n_models}: |dE|/N={e_err:.2e} (bound {bound:.2e}) max|dF|={f_err:.2e}")
     assert e_err <= bound and f_err <= F_TOL
+    if n == 600:
+        assert any(fl > 0 for fl, _ in nnp.stage_work().values())  # tensor-engine launches, not the FFMA fallback
+        alt = NNP(w.params, W, B, w.species, flags=binding.NNP_FLAG_NO_UMMA)
+        E2 = torch.zeros(1, dtype=torch.float64, device=DEV)
+        F2 = torch.zeros((w.n_atoms, 3), dtype=torch.float32, device=DEV)
+        alt.compute_torch(pos, E2, F2); alt.check()
+        assert abs(E2.item() - E.item()) / w.n_atoms <= 2e-6 and (F2 - F).abs().max().item() <= 2e-4
+        alt.destroy()
     nnp.destroy()
 
 
