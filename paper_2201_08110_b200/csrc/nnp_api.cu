@@ -270,8 +270,6 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
   for (int e = 0; e < S && box_ok; ++e) {
     for (int l = 1; l < L; ++l)
       if (h->dims[e * (L + 1) + l] % 16 != 0) box_ok = false;
-    // layer-1 backward: the contraction runs over all models of the element, M * H1 must be whole boxes
-    if (((long long)M * h->dims[e * (L + 1) + 1]) % 32 != 0) box_ok = false;
   }
   // ligand-size engine: every element group is small, so the layers are weight-streaming problems
   int max_grp = 0, max_dim = n_feat;
@@ -293,7 +291,7 @@ extern "C" int nnp_create(nnp_handle** out, const nnp_config* cfg, int32_t n_ato
     long long tiles = 0;
     for (int e = 0; e < S; ++e) tiles += ((h->grp_off[e + 1] - h->grp_off[e] + 127) / 128) * (long long)((n_feat + 127) / 128);
     // a group of models must be whole boxes of every element's contraction (the weight tensor of the layer-1 backward
-    // spans ALL models, so nothing zero-fills a box that runs into the next group)
+    // spans ALL models, so nothing zero-fills a box that runs into the next group; one group = the whole extent: any K)
     auto group_ok = [&](int p) {
       for (int e = 0; e < S; ++e)
         if (((long long)(M / p) * h->dims[e * (L + 1) + 1]) % 32 != 0) return false;
