@@ -243,9 +243,51 @@ __global__ void __launch_bounds__(128) last_layer_kernel(const __grid_constant__
   if (lane == 0) a.e_out[(size_t)row * a.M + m] = acc + (double)a.bias[a.b_off[e] + m];
 }
 
+// Tensor engine (delta already written by the forward epilogue): only the energies e[a][m] = b[m] + w[m] . h[a][m][:]
+// are left, a pure read of the one-plane copy of h.  Half a warp per (atom, model): 16-byte loads, all of a lane's loads
+// (up to four of h, four of w) in flight before the first use, FP64 dot product, four shuffle steps.
+__global__ void __launch_bounds__(128) last_energy_kernel(const __grid_constant__ LastLayerArgs a) {
+  const int hw = (blockIdx.x * blockDim.x + threadIdx.x) >> 4;  // half-warp index = (atom row, model)
+  const int l16 = threadIdx.x & 15;
+  const bool live = hw < a.n_sorted * a.M;
+  const int row = live ? hw / a.M : 0, m = live ? hw % a.M : 0;
+  int e = 0;
+  while (e + 1 < a.S && row >= a.grp_off[e + 1]) ++e;
+  const int H4 = a.H[e] >> 2;
+  const float4* hf = reinterpret_cast<const float4*>(a.act_full + a.act_off[e] + ((size_t)(row - a.grp_off[e]) * a.M + m) * a.H[e]);
+  const float4* wv = reinterpret_cast<const float4*>(a.W + a.w_off[e] + (size_t)m * a.H[e]);
+  float4 x[4], w[4];
+#pragma unroll
+  for (int u = 0; u < 4; ++u) {
+    const int q = l16 + 16 * u;
+    const bool on = live && q < H4;
+    x[u] = on ? hf[q] : make_float4(0.f, 0.f, 0.f, 0.f);
+    w[u] = on ? wv[q] : make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  double acc = 0.0;
+#pragma unroll
+  for (int u = 0; u < 4; ++u) {
+    acc += (double)w[u].x * (double)x[u].x;
+    acc += (double)w[u].y * (double)x[u].y;
+    acc += (double)w[u].z * (double)x[u].z;
+    acc += (double)w[u].w * (double)x[u].w;
+  }
+#pragma unroll
+  for (int o = 8; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if (live && l16 == 0) a.e_out[(size_t)row * a.M + m] = acc + (double)a.bias[a.b_off[e] + m];
+}
+
 void launch_last_layer(nnp_handle* h, cudaStream_t s) {
   const long warps = (long)h->N * h->M;
   if (warps == 0) return;
+  {
+    bool wide_ok = h->last.act_full != nullptr;
+    for (int e = 0; e < h->last.S; ++e) wide_ok = wide_ok && h->last.H[e] % 4 == 0 && h->last.H[e] <= 256 && h->last.act_off[e] % 4 == 0 && h->last.w_off[e] % 4 == 0;
+    if (wide_ok) {
+      last_energy_kernel<<<(int)((warps * 16 + 127) / 128), 128, 0, s>>>(h->last);
+      return;
+    }
+  }
   const int blocks = (int)((warps + 3) / 4);
   last_layer_kernel<<<blocks, 128, 0, s>>>(h->last);
 }
