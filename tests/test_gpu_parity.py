@@ -521,6 +521,18 @@ def test_status_capacity_and_nonfinite():
     bad[3, 1] = np.nan
     nnp.compute_torch(torch.from_numpy(bad).to(dev), E, F)
     assert nnp.status() == -5  # NNP_ERR_NONFINITE
+    # the handle recovers: the force accumulators are cleared by the step that read them, whatever they held, so the
+    # next step with finite input is the step of a fresh handle, bit for bit
+    F.zero_()
+    nnp.compute_torch(pos, E, F)
+    assert nnp.status() == 0
+    fresh = NNP(p, W, B, w.species)
+    E2 = torch.zeros(1, dtype=torch.float64, device=dev)
+    F2 = torch.zeros((20, 3), dtype=torch.float32, device=dev)
+    fresh.compute_torch(pos, E2, F2)
+    assert fresh.status() == 0
+    assert torch.equal(E, E2) and torch.equal(F, F2) and bool(torch.isfinite(F).all())
+    fresh.destroy()
     nnp.destroy()
     with pytest.raises(NNPError):
         NNP(p, W, B, np.array([0, 5], np.int32))  # species out of range
