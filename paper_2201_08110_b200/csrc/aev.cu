@@ -4,8 +4,9 @@
 // Definitions: DESIGN.md O1-O4, O6, O7 (the paper names ANI-2x, and gives no formulas).
 // Design: one CTA per centre atom; the centre's feature row (or dE/dAEV row) and the geometry of its
 // neighbours live in shared memory; the angular work is one thread per TRIPLET (its powers and Gaussians
-// are evaluated once and combined in registers), summed in a fixed order with no atomics anywhere; forces
-// leave the kernel as one "pair gradient" phi_ij per directed pair, gathered per atom afterwards.
+// are evaluated once and combined in registers), every floating-point sum has a fixed order (no float atomics
+// anywhere); a centre's "pair gradients" phi_ij are added to the two atoms of each pair in 64-bit fixed point
+// (integer atomics: order-independent), which the finish kernel converts into the caller's force buffer.
 #include <math_constants.h>
 
 #include "nnp_internal.h"
